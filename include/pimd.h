@@ -1,0 +1,138 @@
+/*
+ * pimd.h -- C-ABI of the B200-native PIMD hot path (libpimd_b200.so).
+ *
+ * One ring-polymer path-integral MD step over all P beads, as stated in
+ * arXiv 2503.23728 (citations "P:Lnnn" = line of the paper text, "S:x" = reading
+ * listed in DESIGN.md / SURVEY.md section 8(c)):
+ *
+ *   (a) per-bead periodic cell-list neighbour build        (cutoff only: P:L394)
+ *   (b) bead-batched, back-propagation-free GFN force net   (eqs; S:G0-G6)
+ *   (c) normal-mode transform, exact free-ring-polymer step
+ *       and PILE-L thermostat with Philox noise            (S:N1-N5)
+ *
+ * Every step runs in hand-written sm_100a CUDA kernels; there is no CPU fallback.
+ * No torch / C++ types cross this boundary: plain pointers and sizes only.  Each
+ * pointer argument says whether it is HOST or DEVICE memory.
+ *
+ * Units: Angstrom, fs, amu, K, eV, eV/A; centroid friction in ps^-1.
+ * Layout: every per-bead array is [replica][bead][atom][xyz], row id = (r*P + k)*N + i.
+ *
+ * Errors: every call returns 0 on success or
+ *   PIMD_ERR_ARG   (-1) invalid argument (null pointer, P < 1 or > 256, periodic box edge
+ *                        < 2 r_cut, weight count mismatch, workspace too small, unsupported
+ *                        (n_rbf, hidden) pair)
+ *   PIMD_ERR_CUDA  (-2) a CUDA call failed
+ *   PIMD_ERR_PAIRS (-3) pair capacity (or 512 neighbours per atom) exceeded
+ *   PIMD_ERR_NAN   (-4) non-finite force or position met on the device
+ * Device-detected conditions (-3, -4) are latched in a device word and returned by the
+ * next synchronising call (pimd_estimators, pimd_get_state, pimd_nlist, pimd_sync).
+ * pimd_last_error() returns a thread-local description.  After an error the context is
+ * only good for pimd_destroy.
+ */
+#ifndef PIMD_B200_H
+#define PIMD_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PIMD_OK 0
+#define PIMD_ERR_ARG (-1)
+#define PIMD_ERR_CUDA (-2)
+#define PIMD_ERR_PAIRS (-3)
+#define PIMD_ERR_NAN (-4)
+
+typedef struct pimd_ctx pimd_ctx; /* opaque; host object that owns nothing but views into the workspace */
+
+/* Network / potential description.  `weights` is a HOST pointer, copied by pimd_create. */
+typedef struct {
+    int32_t kind;       /* 0 GFN net; 1 harmonic test well V = 1/2 m w^2 |r|^2 per atom;
+                           2 none (free ring polymer) */
+    int32_t n_species;  /* S */
+    int32_t n_rbf;      /* K  Gaussian radial basis functions on [0, r_cut] (S:G1) */
+    int32_t hidden;     /* H  feature width ("Feat. Dim.") */
+    int32_t n_layers;   /* L  interaction layers ("N_inter") */
+    int32_t gemm_dtype; /* 0: fp32 everywhere.  1: bf16 operands + fp32 accumulation on the
+                           tensor cores for the dense contractions (tolerance 2e-2) */
+    float r_cut;        /* A (0.6 nm) */
+    float agg_norm;     /* constant multiplying every neighbour sum (S:G6) */
+    float force_scale;  /* eV/A per unit network output (S:G6) */
+    double harmonic_omega; /* rad/fs, kind 1 only */
+    const float *weights;  /* HOST, packed fp32 in the order of S:G0:
+                              Emb[S][H]; W_e1[H][K], b_e1[H], W_e2[H][H], b_e2[H];
+                              per layer: W_s, W_vn, W_vm [H][H], b_v1[H], W_v2[H][H], b_v2[H], W_a[H][H], b_a[H];
+                              W_f1[H][H], b_f1[H], w_f2[H], b_f2[1]; matrices row-major [out][in] */
+    int64_t n_weights;
+} pimd_net_params;
+
+/* Per-replica estimators (bead averages), eV except t_centroid (K).
+ * k_prim: primitive, k_vir: virial, k_cvir: centroid-virial kinetic energy (S:E1-E3);
+ * v_pot: bead-averaged potential for kinds 1-2, NaN for the GFN (it has no energy). */
+typedef struct {
+    double k_prim, k_vir, k_cvir, v_pot, t_centroid;
+} pimd_estimators_t;
+
+/* Bytes of DEVICE workspace pimd_create needs for these sizes.  `out` is HOST. */
+int pimd_workspace_bytes(int n_atoms, int n_replicas, int P, const double box[3], const pimd_net_params *net,
+                         size_t *out);
+
+/*
+ * Creates a context (system + potential + NMPIMD integrator).
+ *   species      HOST  [N]      type index 0..S-1
+ *   masses_amu   HOST  [S]      mass per type
+ *   positions    HOST  [R][N][3] A; every bead of replica r starts here (S:N5)
+ *   box          HOST  [3]      orthorhombic edge lengths, {0,0,0} = non-periodic
+ *   P, T_kelvin, dt_fs          beads, temperature, time step
+ *   gamma_centroid_per_ps       PILE-L centroid friction; < 0 switches the thermostat off (NVE)
+ *   seed                        Philox4x32-10 key (S:N4)
+ *   d_workspace  DEVICE         caller-allocated (e.g. a torch tensor), >= pimd_workspace_bytes,
+ *                               256-byte aligned; the library never allocates or frees device memory
+ *   cuda_stream                 cudaStream_t on which every kernel and copy is enqueued
+ * Host inputs are copied (synchronously) before the call returns.  Initial momenta are drawn
+ * on the device per normal mode (S:N5); forces are evaluated lazily by the first call that
+ * needs them.
+ */
+int pimd_create(pimd_ctx **out, int n_atoms, int n_replicas, const int32_t *species, const double *masses_amu,
+                const double *positions, const double box[3], int P, double T_kelvin, double dt_fs,
+                double gamma_centroid_per_ps, uint64_t seed, const pimd_net_params *net, void *d_workspace,
+                size_t workspace_bytes, void *cuda_stream);
+
+/* n steps of O(dt/2) B(dt/2) A(dt) [neighbour list, forces] B(dt/2) O(dt/2) (S:N3).
+ * Asynchronous on the stream; no host synchronisation. */
+int pimd_step(pimd_ctx *ctx, int n);
+
+/* Rebuilds the neighbour list and evaluates the forces at the current positions.
+ * d_out DEVICE float [R][P][N][3] eV/A.  Asynchronous. */
+int pimd_forces(pimd_ctx *ctx, float *d_out);
+
+/* h_out HOST [R].  Synchronises the stream. */
+int pimd_estimators(pimd_ctx *ctx, pimd_estimators_t *h_out);
+
+/* State access for parity tests and checkpoint/resume.  d_q, d_p DEVICE double [R][P][N][3]
+ * (A, amu*A/fs * 103.6426965268 i.e. eV fs/A); either may be NULL.  `step` HOST.
+ * pimd_get_state synchronises; pimd_set_state is asynchronous and invalidates the cached forces. */
+int pimd_get_state(pimd_ctx *ctx, double *d_q, double *d_p, int64_t *step);
+int pimd_set_state(pimd_ctx *ctx, const double *d_q, const double *d_p, int64_t step);
+
+/* Builds the neighbour list at the current positions and exports it as CSR over all rows.
+ *   d_row_ptr DEVICE int32 [R*P*N + 1]; d_col DEVICE int32 [col_capacity] holds the atom index j
+ *   (0..N-1, within the bead-system of the row), ascending within each row (S:L1);
+ *   h_n_pairs HOST.  Synchronises. */
+int pimd_nlist(pimd_ctx *ctx, int32_t *d_row_ptr, int32_t *d_col, int64_t col_capacity, int64_t *h_n_pairs);
+
+/* Waits for the stream and returns any latched device error. */
+int pimd_sync(pimd_ctx *ctx);
+
+/* Number of kernels the library has launched on this context so far (HOST counter). */
+int64_t pimd_launch_count(const pimd_ctx *ctx);
+
+const char *pimd_last_error(void);
+void pimd_destroy(pimd_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PIMD_B200_H */

@@ -5,7 +5,11 @@ Argument marshalling only; every number is produced by the C file.
 from __future__ import annotations
 
 import ctypes as C
+import os
 from dataclasses import dataclass
+
+# libgomp's default active spin-wait is very slow on shared/cgroup-limited hosts (many short parallel regions)
+os.environ.setdefault("OMP_WAIT_POLICY", "passive")
 
 import numpy as np
 

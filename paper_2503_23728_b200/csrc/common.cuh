@@ -1,0 +1,115 @@
+// common.cuh -- shared declarations of the sm_100a PIMD library (host context, device views).
+// Product code: shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+
+#include "../../include/pimd.h"
+
+// CODATA 2018; hard-coded independently of the oracle.
+#define PIMD_KB 8.617333262145e-5      // eV / K
+#define PIMD_HBAR 0.658211956548       // eV fs
+#define PIMD_AMU 103.6426965268        // 1 amu A^2/fs^2 in eV
+
+#define PIMD_MAX_P 256
+#define PIMD_MAX_NBR 512               // neighbours per atom the fill kernel can sort
+
+// device error word bits
+#define PIMD_FLAG_PAIRS 1
+#define PIMD_FLAG_NAN 2
+
+struct GfnLayerW {
+    const float *WsT, *WvnT, *WvmT, *bv1, *Wv2T, *bv2, *WaT, *ba;  // transposed [in][out]
+};
+
+// Device-side view of the network (all pointers into the workspace).
+struct GfnDev {
+    int S, K, H, L;
+    float r_cut, agg_norm, force_scale;
+    const float *Emb;                  // [S][H]
+    const float *We1T, *be1;           // [K][H]
+    const float *We2T, *be2;           // [H][H]
+    const float *WfeT, *bfe;           // (W_f1 W_e2)^T [H][H], W_f1 b_e2 + b_f1
+    const float *Wf1T;                 // [H][H]  (G = W_f1 E)
+    const float *wf2;                  // [H]
+    float bf2;
+    GfnLayerW layer[8];
+};
+
+struct NlistDev {
+    int ncell[3];
+    int ncell_tot;                     // per bead-system
+    int *cell_id;                      // [rows]
+    int *cell_count;                   // [nsys*ncell_tot]
+    int *cell_start;                   // [nsys*(ncell_tot+1)] relative to the system's first row
+    int *cell_cursor;                  // [nsys*ncell_tot]
+    int *sorted_atom;                  // [rows] local atom index in cell order
+    double *sorted_q;                  // [rows][3]
+    int *nnz;                          // [rows]
+    int *row_ptr;                      // [rows+1]
+    int *block_sums;                   // [ceil(rows/1024)+1]
+    int *col;                          // [pair_cap] local atom index j
+    int *pair_row;                     // [pair_cap] global row i
+    int64_t pair_cap;
+};
+
+struct pimd_ctx {
+    int N, R, P, periodic;
+    int64_t rows;                      // R*P*N
+    double box[3];
+    double T, dt, gamma_fs;            // gamma_fs < 0: NVE
+    uint64_t seed;
+    int64_t step;
+    int kind, gemm_dtype;
+    double harmonic_omega;
+    cudaStream_t stream;
+    int forces_valid;
+    int64_t launches;
+    int num_sms;
+
+    // workspace views
+    double *q, *p, *F;                 // [rows][3]
+    int *species;                      // [N]
+    double *mass;                      // [N] internal units
+    double *Cmat, *CmatT;              // [P][P]: C[j*P+k]; CT[k*P+j]
+    double *omega_k;                   // [P]
+    int *err;                          // [4] device error word
+    double *est_partial;               // [R][EST_BLOCKS][8]
+    double *est_out;                   // [R][8]
+    NlistDev nl;
+    GfnDev net;
+    float *weights_dev;                // raw + derived weights
+    float *nfeat, *xfeat, *mfeat, *Efeat, *Gfeat;   // [rows][H]
+    float *carry_m;                    // [n_gran_m][2][H]
+    float *carry_f;                    // [n_gran_f][2][4]
+    float *Fraw;                       // [rows][4] complete-row partial force sums
+    int gran_m, gran_f;                // pairs per reduction granule
+    int64_t n_gran_m, n_gran_f;
+};
+
+void pimd_set_error(const char *fmt, ...);
+
+#define PIMD_CUDA_CHECK(call)                                                            \
+    do {                                                                                 \
+        cudaError_t e_ = (call);                                                         \
+        if (e_ != cudaSuccess) {                                                         \
+            pimd_set_error("%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); \
+            return PIMD_ERR_CUDA;                                                        \
+        }                                                                                \
+    } while (0)
+
+// kernel launchers (each returns 0 or PIMD_ERR_CUDA)
+int pimd_launch_init_momenta(pimd_ctx *c);
+int pimd_launch_nm_pre(pimd_ctx *c, uint32_t t);
+int pimd_launch_nm_post(pimd_ctx *c, uint32_t t);
+int pimd_launch_simple_forces(pimd_ctx *c);          // kinds 1, 2
+int pimd_launch_estimators(pimd_ctx *c);
+int pimd_launch_check_finite(pimd_ctx *c);
+int pimd_launch_nlist(pimd_ctx *c);
+int pimd_launch_gfn_forces(pimd_ctx *c);
+int pimd_launch_copy_forces_f32(pimd_ctx *c, float *d_out);
+size_t pimd_gfn_smem_bytes(int K, int H);
+bool pimd_gfn_supported(int K, int H);
+
+static inline size_t pimd_align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }

@@ -1,0 +1,81 @@
+// gfn_fp32.cuh -- building blocks of the fp32 (FFMA) GFN kernels: 128-row register-tiled GEMM on
+// shared-memory operands, swizzled k-major A buffers, activation.
+#pragma once
+#include "common.cuh"
+
+namespace gfn {
+
+constexpr int TP = 128;   // pairs (or rows) per tile
+constexpr int NT = 256;   // threads per CTA
+constexpr int TX = 16;    // channel groups per tile
+
+// k-major A buffer [k][TP]; column index XOR-swizzled in units of 4 floats by the k row, so that
+// transposing float4 stores from the 16 channel groups hit distinct banks.
+__device__ __forceinline__ int swz(int k) { return ((k >> 2) & 7) << 2; }
+
+__device__ __forceinline__ float silu_f(float x) { return __fdividef(x, 1.0f + __expf(-x)); }
+
+template <int H>
+struct Tile {
+    static constexpr int CPT = H / TX;        // channels per thread (8 for H=128, 4 for H=64)
+    static constexpr int NCG = CPT / 4;       // float4 channel groups per thread
+    // channel of (group g, element e) for this thread
+    __device__ static __forceinline__ int chan(int tx, int g, int e) { return g * (H / 2) + tx * 4 + e; }
+    // local pair (row) of (group g, element e)
+    __device__ static __forceinline__ int pair(int ty, int g, int e) { return g * (TP / 2) + ty * 4 + e; }
+};
+
+// acc[p][c] += sum_k A[k][p] * W[k][c];  A swizzled [KD][TP], W [KD][H]
+template <int KD, int H>
+__device__ __forceinline__ void tile_gemm(const float *__restrict__ sA, const float *__restrict__ sW,
+                                          float (&acc)[8][Tile<H>::CPT], int tx, int ty)
+{
+    constexpr int CPT = Tile<H>::CPT;
+#pragma unroll 4
+    for (int k = 0; k < KD; ++k) {
+        const int sw = swz(k);
+        float a[8], b[CPT];
+        *(float4 *)&a[0] = *(const float4 *)&sA[k * TP + ((ty * 4) ^ sw)];
+        *(float4 *)&a[4] = *(const float4 *)&sA[k * TP + ((TP / 2 + ty * 4) ^ sw)];
+        *(float4 *)&b[0] = *(const float4 *)&sW[k * H + tx * 4];
+        if (CPT == 8) *(float4 *)&b[CPT - 4] = *(const float4 *)&sW[k * H + H / 2 + tx * 4];
+#pragma unroll
+        for (int p = 0; p < 8; ++p)
+#pragma unroll
+            for (int c = 0; c < CPT; ++c) acc[p][c] = fmaf(a[p], b[c], acc[p][c]);
+    }
+}
+
+template <int H>
+__device__ __forceinline__ void zero_acc(float (&acc)[8][Tile<H>::CPT])
+{
+#pragma unroll
+    for (int p = 0; p < 8; ++p)
+#pragma unroll
+        for (int c = 0; c < Tile<H>::CPT; ++c) acc[p][c] = 0.f;
+}
+
+// writes v[p][c] (this thread's 8 x CPT sub-tile) into a swizzled k-major buffer as A[c][p]
+template <int H>
+__device__ __forceinline__ void store_as_A(float *sA, const float (&v)[8][Tile<H>::CPT], int tx, int ty)
+{
+    constexpr int CPT = Tile<H>::CPT;
+#pragma unroll
+    for (int c = 0; c < CPT; ++c) {
+        const int ch = Tile<H>::chan(tx, c >> 2, c & 3);
+        const int sw = swz(ch);
+        *(float4 *)&sA[ch * TP + ((ty * 4) ^ sw)] = make_float4(v[0][c], v[1][c], v[2][c], v[3][c]);
+        *(float4 *)&sA[ch * TP + ((TP / 2 + ty * 4) ^ sw)] = make_float4(v[4][c], v[5][c], v[6][c], v[7][c]);
+    }
+}
+
+// cooperative copy of a [rows][H] fp32 matrix from global into shared memory
+template <int H>
+__device__ __forceinline__ void load_matrix(float *sW, const float *__restrict__ g, int rows)
+{
+    const float4 *g4 = (const float4 *)g;
+    float4 *s4 = (float4 *)sW;
+    for (int i = threadIdx.x; i < rows * H / 4; i += NT) s4[i] = __ldg(g4 + i);
+}
+
+}  // namespace gfn

@@ -1,0 +1,267 @@
+// nlist_kernels.cu -- per-bead-system periodic cell list -> CSR pair list (rows a1-a3 of SURVEY 8(a)).
+//
+// bin (wrapped fraction -> cell) -> counting sort (histogram, per-system exclusive scan, scatter of
+// atom index + fp64 position into cell order) -> warp-per-row stencil scan, twice: count, then fill
+// with an in-shared-memory rank sort so that every CSR row lists j ascending.  The inclusion test is
+// the fp64 sequence of S:L3 written with explicit round-to-nearest intrinsics (no FMA contraction), so
+// the list is bit-identical to the oracle's.  Integer atomics only order the scatter inside a cell;
+// the sorted rows make the CSR deterministic.
+#include "common.cuh"
+
+namespace {
+
+struct NlArgs {
+    int N, nsys, periodic;
+    int64_t rows;
+    double box[3];
+    double rc2;
+    int nc[3], nct;
+    const double *q;
+    NlistDev d;
+    int *err;
+};
+
+__global__ void bin_kernel(NlArgs a)
+{
+    int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (row >= a.rows) return;
+    int cell = 0;
+    if (a.periodic) {
+        int c[3];
+#pragma unroll
+        for (int ax = 0; ax < 3; ++ax) {
+            double x = a.q[row * 3 + ax] / a.box[ax];
+            double f = x - floor(x);
+            int ci = (int)(f * a.nc[ax]);
+            if (ci > a.nc[ax] - 1) ci = a.nc[ax] - 1;
+            if (ci < 0) ci = 0;   // NaN positions
+            c[ax] = ci;
+        }
+        cell = (c[0] * a.nc[1] + c[1]) * a.nc[2] + c[2];
+    }
+    a.d.cell_id[row] = cell;
+    int sys = (int)(row / a.N);
+    atomicAdd(&a.d.cell_count[(size_t)sys * a.nct + cell], 1);
+}
+
+// block-wide exclusive scan of one value per thread (blockDim.x multiple of 32, <= 1024)
+__device__ __forceinline__ int block_exclusive_scan(int v, int *total)
+{
+    __shared__ int warp_tot[32];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    int inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        int t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (lane == 31) warp_tot[wid] = inc;
+    __syncthreads();
+    if (wid == 0) {
+        int w = (lane < nw) ? warp_tot[lane] : 0, winc = w;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            int t = __shfl_up_sync(0xffffffffu, winc, o);
+            if (lane >= o) winc += t;
+        }
+        warp_tot[lane] = winc - w;  // exclusive warp offsets
+        if (lane == 31) *total = winc;
+    }
+    __syncthreads();
+    int res = warp_tot[wid] + inc - v;
+    __syncthreads();
+    return res;
+}
+
+// one block per bead-system: cell_start (relative) = exclusive scan of cell_count; zero the cursors
+__global__ void __launch_bounds__(256) scan_cells_kernel(NlArgs a)
+{
+    __shared__ int tot;
+    const int sys = blockIdx.x;
+    const int *cnt = a.d.cell_count + (size_t)sys * a.nct;
+    int *start = a.d.cell_start + (size_t)sys * (a.nct + 1);
+    int *cur = a.d.cell_cursor + (size_t)sys * a.nct;
+    int carry = 0;
+    for (int base = 0; base < a.nct; base += blockDim.x) {
+        int c = base + threadIdx.x;
+        int v = (c < a.nct) ? cnt[c] : 0;
+        int ex = block_exclusive_scan(v, &tot);
+        if (c < a.nct) { start[c] = carry + ex; cur[c] = 0; }
+        carry += tot;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) start[a.nct] = carry;
+}
+
+__global__ void scatter_kernel(NlArgs a)
+{
+    int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (row >= a.rows) return;
+    int sys = (int)(row / a.N), i = (int)(row - (int64_t)sys * a.N);
+    int cell = a.d.cell_id[row];
+    int slot = atomicAdd(&a.d.cell_cursor[(size_t)sys * a.nct + cell], 1);
+    int64_t pos = (int64_t)sys * a.N + a.d.cell_start[(size_t)sys * (a.nct + 1) + cell] + slot;
+    a.d.sorted_atom[pos] = i;
+    a.d.sorted_q[pos * 3 + 0] = a.q[row * 3 + 0];
+    a.d.sorted_q[pos * 3 + 1] = a.q[row * 3 + 1];
+    a.d.sorted_q[pos * 3 + 2] = a.q[row * 3 + 2];
+}
+
+// S:L3 predicate, explicit IEEE round-to-nearest operations in the stated order
+__device__ __forceinline__ bool within_cutoff(const double qi[3], const double *__restrict__ qj, const NlArgs &a)
+{
+    double d[3];
+#pragma unroll
+    for (int ax = 0; ax < 3; ++ax) {
+        double dx = __dsub_rn(qj[ax], qi[ax]);
+        if (a.periodic) dx = __dsub_rn(dx, __dmul_rn(a.box[ax], round(__ddiv_rn(dx, a.box[ax]))));
+        d[ax] = dx;
+    }
+    double d2 = __dadd_rn(__dadd_rn(__dmul_rn(d[0], d[0]), __dmul_rn(d[1], d[1])), __dmul_rn(d[2], d[2]));
+    return d2 < a.rc2;
+}
+
+// Walks the de-duplicated 3x3x3 stencil of `row` with one warp.  FILL = false: returns the hit count.
+// FILL = true: also stores the hit atom indices in buf (capacity PIMD_MAX_NBR), unsorted.
+template <bool FILL>
+__device__ __forceinline__ int stencil_scan(const NlArgs &a, int64_t row, int *buf)
+{
+    const int lane = threadIdx.x & 31;
+    const int sys = (int)(row / a.N), i = (int)(row - (int64_t)sys * a.N);
+    double qi[3] = {a.q[row * 3], a.q[row * 3 + 1], a.q[row * 3 + 2]};
+    int cell = a.d.cell_id[row];
+    int cc[3];
+    cc[2] = cell % a.nc[2]; cc[1] = (cell / a.nc[2]) % a.nc[1]; cc[0] = cell / (a.nc[2] * a.nc[1]);
+    int lst[3][3], cnt[3];
+#pragma unroll
+    for (int ax = 0; ax < 3; ++ax) {
+        cnt[ax] = 0;
+        for (int o = -1; o <= 1; ++o) {
+            int c = cc[ax] + o;
+            if (a.periodic) c = ((c % a.nc[ax]) + a.nc[ax]) % a.nc[ax];
+            else if (c < 0 || c >= a.nc[ax]) continue;
+            bool dup = false;
+            for (int t = 0; t < cnt[ax]; ++t) dup |= (lst[ax][t] == c);
+            if (!dup) lst[ax][cnt[ax]++] = c;
+        }
+    }
+    const int *start = a.d.cell_start + (size_t)sys * (a.nct + 1);
+    const int64_t sbase = (int64_t)sys * a.N;
+    int total = 0;
+    for (int ix = 0; ix < cnt[0]; ++ix)
+        for (int iy = 0; iy < cnt[1]; ++iy)
+            for (int iz = 0; iz < cnt[2]; ++iz) {
+                int c = (lst[0][ix] * a.nc[1] + lst[1][iy]) * a.nc[2] + lst[2][iz];
+                int s0 = start[c], s1 = start[c + 1];
+                for (int s = s0 + lane; s - lane < s1; s += 32) {
+                    bool hit = false;
+                    int j = -1;
+                    if (s < s1) {
+                        j = a.d.sorted_atom[sbase + s];
+                        hit = (j != i) && within_cutoff(qi, a.d.sorted_q + (sbase + s) * 3, a);
+                    }
+                    unsigned m = __ballot_sync(0xffffffffu, hit);
+                    if (FILL && hit) {
+                        int idx = total + __popc(m & ((1u << lane) - 1u));
+                        if (idx < PIMD_MAX_NBR) buf[idx] = j;
+                    }
+                    total += __popc(m);
+                }
+            }
+    return total;
+}
+
+__global__ void __launch_bounds__(256) count_kernel(NlArgs a)
+{
+    int64_t row = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
+    if (row >= a.rows) return;
+    int n = stencil_scan<false>(a, row, nullptr);
+    if ((threadIdx.x & 31) == 0) a.d.nnz[row] = n;
+}
+
+// row_ptr: three-kernel exclusive scan over rows (1024 rows per block)
+__global__ void __launch_bounds__(1024) scan_rows_local_kernel(NlArgs a)
+{
+    __shared__ int tot;
+    int64_t row = (int64_t)blockIdx.x * 1024 + threadIdx.x;
+    int v = (row < a.rows) ? a.d.nnz[row] : 0;
+    int ex = block_exclusive_scan(v, &tot);
+    if (row < a.rows) a.d.row_ptr[row] = ex;
+    if (threadIdx.x == 0) a.d.block_sums[blockIdx.x] = tot;
+}
+
+__global__ void __launch_bounds__(1024) scan_block_sums_kernel(NlArgs a, int nblocks)
+{
+    __shared__ int tot;
+    long long carry = 0;
+    for (int base = 0; base < nblocks; base += 1024) {
+        int b = base + threadIdx.x;
+        int v = (b < nblocks) ? a.d.block_sums[b] : 0;
+        int ex = block_exclusive_scan(v, &tot);
+        if (b < nblocks) a.d.block_sums[b] = (int)(carry + ex);
+        carry += tot;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        if (carry > a.d.pair_cap || carry > 2147483647LL) {
+            atomicOr(a.err, PIMD_FLAG_PAIRS);
+            carry = 0;   // downstream kernels see an empty list instead of reading out of bounds
+        }
+        a.d.row_ptr[a.rows] = (int)carry;
+    }
+}
+
+__global__ void scan_rows_add_kernel(NlArgs a)
+{
+    int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (row < a.rows) a.d.row_ptr[row] += a.d.block_sums[row >> 10];
+}
+
+__global__ void __launch_bounds__(256) fill_kernel(NlArgs a)
+{
+    __shared__ int sbuf[8][PIMD_MAX_NBR];
+    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    int64_t row = (int64_t)blockIdx.x * 8 + w;
+    if (row >= a.rows) return;
+    if (a.d.row_ptr[a.rows] == 0) return;   // empty or overflowed list
+    int *buf = sbuf[w];
+    int n = stencil_scan<true>(a, row, buf);
+    __syncwarp();
+    if (n > PIMD_MAX_NBR) {
+        if (lane == 0) atomicOr(a.err, PIMD_FLAG_PAIRS);
+        n = PIMD_MAX_NBR;
+    }
+    const int64_t base = a.d.row_ptr[row];
+    for (int e = lane; e < n; e += 32) {   // rank sort: j values in a row are distinct (box >= 2 r_c)
+        int v = buf[e], rank = 0;
+        for (int t = 0; t < n; ++t) rank += (buf[t] < v);
+        a.d.col[base + rank] = v;
+        a.d.pair_row[base + rank] = (int)row;
+    }
+}
+
+}  // namespace
+
+int pimd_launch_nlist(pimd_ctx *c)
+{
+    NlArgs a;
+    a.N = c->N; a.nsys = c->R * c->P; a.periodic = c->periodic; a.rows = c->rows;
+    for (int k = 0; k < 3; ++k) { a.box[k] = c->box[k]; a.nc[k] = c->nl.ncell[k]; }
+    a.rc2 = (double)c->net.r_cut * (double)c->net.r_cut;
+    a.nct = c->nl.ncell_tot; a.q = c->q; a.d = c->nl; a.err = c->err;
+    const int64_t rows = c->rows;
+    const unsigned gthr = (unsigned)((rows + 255) / 256), gwarp = (unsigned)((rows + 7) / 8);
+    const int nblk = (int)((rows + 1023) / 1024);
+    PIMD_CUDA_CHECK(cudaMemsetAsync(c->nl.cell_count, 0, sizeof(int) * (size_t)a.nsys * a.nct, c->stream));
+    bin_kernel<<<gthr, 256, 0, c->stream>>>(a);
+    scan_cells_kernel<<<a.nsys, 256, 0, c->stream>>>(a);
+    scatter_kernel<<<gthr, 256, 0, c->stream>>>(a);
+    count_kernel<<<gwarp, 256, 0, c->stream>>>(a);
+    scan_rows_local_kernel<<<nblk, 1024, 0, c->stream>>>(a);
+    scan_block_sums_kernel<<<1, 1024, 0, c->stream>>>(a, nblk);
+    scan_rows_add_kernel<<<gthr, 256, 0, c->stream>>>(a);
+    fill_kernel<<<gwarp, 256, 0, c->stream>>>(a);
+    c->launches += 8;
+    PIMD_CUDA_CHECK(cudaGetLastError());
+    return 0;
+}

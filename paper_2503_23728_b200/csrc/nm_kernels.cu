@@ -1,0 +1,311 @@
+// nm_kernels.cu -- ring-polymer normal-mode integrator kernels (rows a8-a11 of SURVEY 8(a)).
+//
+// pimd_nm: one CTA owns TC (atom,dim) columns of one replica and all P beads of them, staged in
+// shared memory as [P][TC] fp64 slabs; global accesses are coalesced over the column index
+// (contiguous inside a bead).  The P x P orthogonal transform (S:N2) is applied slab-wise;
+// PILE-L noise is Philox4x32-10 + Box-Muller keyed by (seed; atom, r*P+mode, step, tag) (S:N4).
+// HBM-bound: ~(q,p read+write, F read) 8-byte words per bead-atom-dim per step.
+#include "common.cuh"
+#include <math.h>
+
+namespace {
+
+constexpr int NM_TY = 8;
+
+struct NmArgs {
+    int N, R, P, TC;
+    double dt, gamma_fs, kT_P;   // kT_P = k_B T P = 1/beta_P
+    unsigned long long seed;
+    const double *C, *CT, *omega_k, *mass;
+    double *q, *p;
+    const double *F;
+    int *err;
+};
+
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0,
+                                              uint32_t k1, uint32_t out[4])
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        if (r > 0) { k0 += 0x9E3779B9u; k1 += 0xBB67AE85u; }
+        uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+        uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+        uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// component a (0,1,2) of the three normals of counter (atom, sysmode, step, tag)  (S:N4)
+__device__ __forceinline__ double normal_component(unsigned long long seed, uint32_t atom, uint32_t sysmode,
+                                                   uint32_t step, uint32_t tag, int a)
+{
+    uint32_t x[4];
+    philox4x32_10(atom, sysmode, step, tag, (uint32_t)(seed & 0xFFFFFFFFull), (uint32_t)(seed >> 32), x);
+    const double s = 1.0 / 4294967296.0;
+    const double two_pi = 6.283185307179586476925286766559;
+    uint32_t xr = (a == 2) ? x[2] : x[0], xa = (a == 2) ? x[3] : x[1];
+    double u1 = ((double)xr + 0.5) * s, u2 = ((double)xa + 0.5) * s;
+    double rad = sqrt(-2.0 * log(u1));
+    double ang = two_pi * u2;
+    return rad * ((a == 1) ? sin(ang) : cos(ang));
+}
+
+// out[k][c] = sum_j M[k*P + j] * in[j][c]
+__device__ __forceinline__ void xform(const double *__restrict__ M, const double *in, double *out, int P, int TC)
+{
+    const int c = threadIdx.x;
+    for (int k = threadIdx.y; k < P; k += NM_TY) {
+        const double *m = M + (size_t)k * P;
+        double s = 0.0;
+        for (int j = 0; j < P; ++j) s += __ldg(m + j) * in[j * TC + c];
+        out[k * TC + c] = s;
+    }
+}
+
+__device__ __forceinline__ void pile_O(const NmArgs &a, double *pt, int r, int col, uint32_t t, uint32_t tag)
+{
+    const int c = threadIdx.x;
+    const int atom = col / 3, dim = col - 3 * atom;
+    const double hdt = 0.5 * a.dt;
+    const double sig = sqrt(a.mass[atom] * a.kT_P);
+    for (int k = threadIdx.y; k < a.P; k += NM_TY) {
+        double gam = (k == 0) ? a.gamma_fs : 2.0 * a.omega_k[k];
+        double c1 = exp(-gam * hdt), c2 = sqrt(1.0 - c1 * c1);
+        double xi = normal_component(a.seed, (uint32_t)atom, (uint32_t)(r * a.P + k), t, tag, dim);
+        pt[k * a.TC + c] = c1 * pt[k * a.TC + c] + sig * c2 * xi;
+    }
+}
+
+// mode: 0 = pre (O,B,A), 1 = post (B,O), 2 = initial momenta (S:N5)
+template <int MODE>
+__global__ void __launch_bounds__(32 * NM_TY) nm_kernel(NmArgs a, uint32_t t)
+{
+    extern __shared__ double sm[];
+    const int P = a.P, TC = a.TC;
+    double *bP = sm, *bT = sm + (size_t)P * TC, *bQ = bT + (size_t)P * TC, *bQ2 = bQ + (size_t)P * TC;
+    const int c = threadIdx.x, r = blockIdx.y;
+    const int ncol = 3 * a.N;
+    const int col = blockIdx.x * TC + c;
+    const bool live = col < ncol;
+    const int colc = live ? col : 0;
+    const size_t base = (size_t)r * P * ncol + colc;
+    const bool thermo = a.gamma_fs >= 0.0;
+    const double hdt = 0.5 * a.dt;
+
+    if (MODE == 2) {
+        const int atom = colc / 3, dim = colc - 3 * atom;
+        const double sig = sqrt(a.mass[atom] * a.kT_P);
+        for (int k = threadIdx.y; k < P; k += NM_TY)
+            bT[k * TC + c] = sig * normal_component(a.seed, (uint32_t)atom, (uint32_t)(r * P + k), 0u, 2u, dim);
+        __syncthreads();
+        xform(a.C, bT, bP, P, TC);
+        __syncthreads();
+        if (live)
+            for (int j = threadIdx.y; j < P; j += NM_TY) a.p[base + (size_t)j * ncol] = bP[j * TC + c];
+        return;
+    }
+
+    bool bad = false;
+    for (int j = threadIdx.y; j < P; j += NM_TY) {
+        double pv = live ? a.p[base + (size_t)j * ncol] : 0.0;
+        if (MODE == 1) {  // B(dt/2) first
+            double f = live ? a.F[base + (size_t)j * ncol] : 0.0;
+            bad |= !isfinite(f);
+            pv += hdt * f;
+        }
+        bP[j * TC + c] = pv;
+        if (MODE == 0) bQ[j * TC + c] = live ? a.q[base + (size_t)j * ncol] : 0.0;
+    }
+    __syncthreads();
+    if (thermo) {
+        xform(a.CT, bP, bT, P, TC);
+        __syncthreads();
+        pile_O(a, bT, r, colc, t, MODE == 0 ? 0u : 1u);
+        __syncthreads();
+        xform(a.C, bT, bP, P, TC);
+        __syncthreads();
+    }
+    if (MODE == 1) {
+        if (live)
+            for (int j = threadIdx.y; j < P; j += NM_TY) a.p[base + (size_t)j * ncol] = bP[j * TC + c];
+        if (bad) atomicOr(a.err, PIMD_FLAG_NAN);
+        return;
+    }
+    // MODE 0: B(dt/2), then A(dt) exact in normal modes
+    for (int j = threadIdx.y; j < P; j += NM_TY) {
+        double f = live ? a.F[base + (size_t)j * ncol] : 0.0;
+        bP[j * TC + c] += hdt * f;
+    }
+    __syncthreads();
+    xform(a.CT, bQ, bQ2, P, TC);
+    xform(a.CT, bP, bT, P, TC);
+    __syncthreads();
+    {
+        const double mi = a.mass[colc / 3];
+        for (int k = threadIdx.y; k < P; k += NM_TY) {
+            double qt = bQ2[k * TC + c], pt = bT[k * TC + c];
+            if (k == 0) {
+                qt = qt + a.dt * pt / mi;
+            } else {
+                double w = a.omega_k[k], sn, cs;
+                sincos(w * a.dt, &sn, &cs);
+                double pn = cs * pt - mi * w * sn * qt;
+                double qn = sn / (mi * w) * pt + cs * qt;
+                pt = pn; qt = qn;
+            }
+            bQ2[k * TC + c] = qt; bT[k * TC + c] = pt;
+        }
+    }
+    __syncthreads();
+    xform(a.C, bQ2, bQ, P, TC);
+    xform(a.C, bT, bP, P, TC);
+    __syncthreads();
+    if (live)
+        for (int j = threadIdx.y; j < P; j += NM_TY) {
+            double qv = bQ[j * TC + c];
+            bad |= !isfinite(qv);
+            a.q[base + (size_t)j * ncol] = qv;
+            a.p[base + (size_t)j * ncol] = bP[j * TC + c];
+        }
+    if (bad) atomicOr(a.err, PIMD_FLAG_NAN);
+}
+
+NmArgs make_args(const pimd_ctx *c)
+{
+    NmArgs a;
+    a.N = c->N; a.R = c->R; a.P = c->P; a.TC = (c->P <= 128) ? 32 : 16;
+    a.dt = c->dt; a.gamma_fs = c->gamma_fs; a.kT_P = PIMD_KB * c->T * c->P;
+    a.seed = c->seed; a.C = c->Cmat; a.CT = c->CmatT; a.omega_k = c->omega_k; a.mass = c->mass;
+    a.q = c->q; a.p = c->p; a.F = c->F; a.err = c->err;
+    return a;
+}
+
+template <int MODE>
+int launch_nm(pimd_ctx *c, uint32_t t)
+{
+    NmArgs a = make_args(c);
+    size_t smem = (size_t)4 * c->P * a.TC * sizeof(double);
+    static bool attr_set[3] = {false, false, false};
+    if (!attr_set[MODE]) {
+        PIMD_CUDA_CHECK(cudaFuncSetAttribute(nm_kernel<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+        attr_set[MODE] = true;
+    }
+    dim3 grid((3 * c->N + a.TC - 1) / a.TC, c->R), block(a.TC, NM_TY);
+    nm_kernel<MODE><<<grid, block, smem, c->stream>>>(a, t);
+    c->launches++;
+    PIMD_CUDA_CHECK(cudaGetLastError());
+    return 0;
+}
+
+// ---------------------------------------------------------------------------------------------
+__global__ void simple_forces_kernel(int kind, int N, int64_t n3, double w2, const double *__restrict__ mass,
+                                     const double *__restrict__ q, double *__restrict__ F)
+{
+    int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n3) return;
+    if (kind == 2) { F[t] = 0.0; return; }
+    int atom = (int)((t / 3) % N);
+    F[t] = -(mass[atom] * w2) * q[t];
+}
+
+__global__ void copy_forces_f32_kernel(int64_t n3, const double *__restrict__ F, float *__restrict__ out)
+{
+    int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t < n3) out[t] = (float)F[t];
+}
+
+// estimators (S:E1-E4): partial sums per (replica, block of atoms), fixed-order tree reduction
+constexpr int EST_BLOCKS = 64, EST_THREADS = 128;
+
+__global__ void __launch_bounds__(EST_THREADS)
+estimators_partial_kernel(int N, int P, int kind, double omega_P, double w_h, const double *__restrict__ mass,
+                          const double *__restrict__ q, const double *__restrict__ p, const double *__restrict__ F,
+                          double *__restrict__ partial)
+{
+    __shared__ double red[5][EST_THREADS];
+    const int r = blockIdx.y;
+    double acc[5] = {0, 0, 0, 0, 0};  // spring, vir, cvir, vpot, tc
+    for (int i = blockIdx.x * EST_THREADS + threadIdx.x; i < N; i += EST_BLOCKS * EST_THREADS) {
+        const double mi = mass[i];
+        double qbar[3] = {0, 0, 0}, pc[3] = {0, 0, 0};
+        for (int k = 0; k < P; ++k) {
+            size_t o = (((size_t)r * P + k) * N + i) * 3;
+            for (int a = 0; a < 3; ++a) { qbar[a] += q[o + a]; pc[a] += p[o + a]; }
+        }
+        const double rs = 1.0 / sqrt((double)P);
+        for (int a = 0; a < 3; ++a) { qbar[a] /= P; pc[a] *= rs; }
+        for (int k = 0; k < P; ++k) {
+            size_t o = (((size_t)r * P + k) * N + i) * 3;
+            size_t on = (((size_t)r * P + (k + 1) % P) * N + i) * 3;
+            for (int a = 0; a < 3; ++a) {
+                double qk = q[o + a], dq = qk - q[on + a], f = F[o + a];
+                acc[0] += 0.5 * mi * omega_P * omega_P * dq * dq;
+                acc[1] += qk * f;
+                acc[2] += (qk - qbar[a]) * f;
+                if (kind == 1) acc[3] += 0.5 * mi * w_h * w_h * qk * qk;
+            }
+        }
+        for (int a = 0; a < 3; ++a) acc[4] += pc[a] * pc[a] / mi;
+    }
+    for (int v = 0; v < 5; ++v) red[v][threadIdx.x] = acc[v];
+    __syncthreads();
+    for (int s = EST_THREADS / 2; s > 0; s >>= 1) {
+        if (threadIdx.x < s)
+            for (int v = 0; v < 5; ++v) red[v][threadIdx.x] += red[v][threadIdx.x + s];
+        __syncthreads();
+    }
+    if (threadIdx.x < 5) partial[((size_t)r * EST_BLOCKS + blockIdx.x) * 8 + threadIdx.x] = red[threadIdx.x][0];
+}
+
+__global__ void estimators_final_kernel(int R, int N, int P, int kind, double kT, const double *__restrict__ partial,
+                                        double *__restrict__ out)
+{
+    int r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= R) return;
+    double s[5] = {0, 0, 0, 0, 0};
+    for (int b = 0; b < EST_BLOCKS; ++b)
+        for (int v = 0; v < 5; ++v) s[v] += partial[((size_t)r * EST_BLOCKS + b) * 8 + v];
+    out[r * 8 + 0] = 1.5 * N * P * kT - s[0] / P;
+    out[r * 8 + 1] = -s[1] / (2.0 * P);
+    out[r * 8 + 2] = 1.5 * N * kT - s[2] / (2.0 * P);
+    out[r * 8 + 3] = (kind == 0) ? nan("") : s[3] / P;
+    out[r * 8 + 4] = s[4] / (3.0 * N * PIMD_KB * P);
+}
+
+}  // namespace
+
+int pimd_launch_init_momenta(pimd_ctx *c) { return launch_nm<2>(c, 0u); }
+int pimd_launch_nm_pre(pimd_ctx *c, uint32_t t) { return launch_nm<0>(c, t); }
+int pimd_launch_nm_post(pimd_ctx *c, uint32_t t) { return launch_nm<1>(c, t); }
+
+int pimd_launch_simple_forces(pimd_ctx *c)
+{
+    int64_t n3 = c->rows * 3;
+    double w2 = c->harmonic_omega * c->harmonic_omega;
+    simple_forces_kernel<<<(unsigned)((n3 + 255) / 256), 256, 0, c->stream>>>(c->kind, c->N, n3, w2, c->mass, c->q, c->F);
+    c->launches++;
+    PIMD_CUDA_CHECK(cudaGetLastError());
+    return 0;
+}
+
+int pimd_launch_copy_forces_f32(pimd_ctx *c, float *d_out)
+{
+    int64_t n3 = c->rows * 3;
+    copy_forces_f32_kernel<<<(unsigned)((n3 + 255) / 256), 256, 0, c->stream>>>(n3, c->F, d_out);
+    c->launches++;
+    PIMD_CUDA_CHECK(cudaGetLastError());
+    return 0;
+}
+
+int pimd_launch_estimators(pimd_ctx *c)
+{
+    double kT = PIMD_KB * c->T, omega_P = c->P * kT / PIMD_HBAR;
+    estimators_partial_kernel<<<dim3(EST_BLOCKS, c->R), EST_THREADS, 0, c->stream>>>(
+        c->N, c->P, c->kind, omega_P, c->harmonic_omega, c->mass, c->q, c->p, c->F, c->est_partial);
+    estimators_final_kernel<<<(c->R + 127) / 128, 128, 0, c->stream>>>(c->R, c->N, c->P, c->kind, kT, c->est_partial,
+                                                                        c->est_out);
+    c->launches += 2;
+    PIMD_CUDA_CHECK(cudaGetLastError());
+    return 0;
+}

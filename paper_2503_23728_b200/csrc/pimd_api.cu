@@ -1,0 +1,465 @@
+// pimd_api.cu -- the C-ABI of include/pimd.h: workspace layout, context life cycle, step sequencing.
+// Host logic only; every numerical step is a kernel in nm_kernels.cu / nlist_kernels.cu / gfn_*.cu.
+#include "common.cuh"
+
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+#include <vector>
+
+static thread_local char g_err[512] = "";
+
+void pimd_set_error(const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+}
+
+extern "C" const char *pimd_last_error(void) { return g_err; }
+
+namespace {
+
+struct Layout {
+    size_t q, p, F, species, mass, C, CT, omega, err, est_partial, est_out;
+    size_t cell_id, cell_count, cell_start, cell_cursor, sorted_atom, sorted_q, nnz, row_ptr, block_sums, col, pair_row;
+    size_t weights, nfeat, xfeat, mfeat, Efeat, Gfeat, carry_m, carry_f, Fraw;
+    size_t total;
+    int ncell[3], nct;
+    int64_t pair_cap, n_gran_m, n_gran_f, n_wfloats;
+    int gran_m, gran_f;
+};
+
+size_t take(size_t &cur, size_t bytes)
+{
+    size_t o = cur;
+    cur = pimd_align_up(cur + bytes);
+    return o;
+}
+
+int64_t derived_weight_floats(int S, int K, int H, int L)
+{
+    return (int64_t)S * H + (int64_t)K * H + H + 3LL * H * H + 4LL * H + (int64_t)L * (5LL * H * H + 3LL * H);
+}
+
+int64_t packed_weight_floats(int S, int K, int H, int L)
+{
+    return (int64_t)S * H + (int64_t)H * K + H + (int64_t)H * H + H + (int64_t)L * (5LL * H * H + 3LL * H) +
+           (int64_t)H * H + H + H + 1;
+}
+
+int compute_layout(int N, int R, int P, const double box[3], const pimd_net_params *net, Layout *L)
+{
+    if (N < 1 || R < 1 || P < 1 || P > PIMD_MAX_P || !net || !box) {
+        pimd_set_error("invalid sizes: N=%d R=%d P=%d (1 <= P <= %d)", N, R, P, PIMD_MAX_P);
+        return PIMD_ERR_ARG;
+    }
+    if (net->kind < 0 || net->kind > 2) { pimd_set_error("invalid net kind %d", net->kind); return PIMD_ERR_ARG; }
+    const bool periodic = box[0] > 0.0 || box[1] > 0.0 || box[2] > 0.0;
+    if (periodic && !(box[0] > 0.0 && box[1] > 0.0 && box[2] > 0.0)) {
+        pimd_set_error("box must be all zero (open) or all positive");
+        return PIMD_ERR_ARG;
+    }
+    const int64_t rows = (int64_t)R * P * N;
+    const int nsys = R * P;
+    memset(L, 0, sizeof(*L));
+    L->ncell[0] = L->ncell[1] = L->ncell[2] = 1;
+    int H = 4;
+    if (net->kind == 0) {
+        if (!pimd_gfn_supported(net->n_rbf, net->hidden)) {
+            pimd_set_error("unsupported (n_rbf, hidden) = (%d, %d); built: (32,64), (64,128)", net->n_rbf, net->hidden);
+            return PIMD_ERR_ARG;
+        }
+        if (net->n_layers < 0 || net->n_layers > 8 || net->n_species < 1 || !(net->r_cut > 0.f)) {
+            pimd_set_error("invalid network description");
+            return PIMD_ERR_ARG;
+        }
+        H = net->hidden;
+        double expect;
+        if (periodic) {
+            for (int a = 0; a < 3; ++a) {
+                if (box[a] < 2.0 * (double)net->r_cut) {
+                    pimd_set_error("periodic box edge %g < 2 r_cut", box[a]);
+                    return PIMD_ERR_ARG;
+                }
+                int nc = (int)floor(box[a] / (double)net->r_cut);
+                L->ncell[a] = nc < 1 ? 1 : nc;
+            }
+            double vol = box[0] * box[1] * box[2], rc = net->r_cut;
+            expect = (double)N / vol * 4.18879020478639 * rc * rc * rc;
+        } else {
+            expect = 256.0;
+        }
+        int64_t cap_row = (int64_t)ceil(2.0 * expect) + 32;
+        if (cap_row > N - 1) cap_row = N - 1;
+        if (cap_row > PIMD_MAX_NBR) cap_row = PIMD_MAX_NBR;
+        if (cap_row < 1) cap_row = 1;
+        L->pair_cap = (rows * cap_row + 255) / 256 * 256;
+        if (L->pair_cap > 2000000000LL) { pimd_set_error("pair capacity exceeds int32 range"); return PIMD_ERR_ARG; }
+        L->gran_m = H / 2;   // pairs per message-reduction granule: TP * H / NT
+        L->gran_f = 32;
+        L->n_gran_m = L->pair_cap / L->gran_m + 2;
+        L->n_gran_f = L->pair_cap / L->gran_f + 2;
+        L->n_wfloats = derived_weight_floats(net->n_species, net->n_rbf, H, net->n_layers);
+    }
+    L->nct = L->ncell[0] * L->ncell[1] * L->ncell[2];
+    size_t cur = 0;
+    L->q = take(cur, sizeof(double) * rows * 3);
+    L->p = take(cur, sizeof(double) * rows * 3);
+    L->F = take(cur, sizeof(double) * rows * 3);
+    L->species = take(cur, sizeof(int) * N);
+    L->mass = take(cur, sizeof(double) * N);
+    L->C = take(cur, sizeof(double) * P * P);
+    L->CT = take(cur, sizeof(double) * P * P);
+    L->omega = take(cur, sizeof(double) * P);
+    L->err = take(cur, sizeof(int) * 4);
+    L->est_partial = take(cur, sizeof(double) * (size_t)R * 64 * 8);
+    L->est_out = take(cur, sizeof(double) * (size_t)R * 8);
+    if (net->kind == 0) {
+        L->cell_id = take(cur, sizeof(int) * rows);
+        L->cell_count = take(cur, sizeof(int) * (size_t)nsys * L->nct);
+        L->cell_start = take(cur, sizeof(int) * (size_t)nsys * (L->nct + 1));
+        L->cell_cursor = take(cur, sizeof(int) * (size_t)nsys * L->nct);
+        L->sorted_atom = take(cur, sizeof(int) * rows);
+        L->sorted_q = take(cur, sizeof(double) * rows * 3);
+        L->nnz = take(cur, sizeof(int) * rows);
+        L->row_ptr = take(cur, sizeof(int) * (rows + 1));
+        L->block_sums = take(cur, sizeof(int) * ((rows + 1023) / 1024 + 1));
+        L->col = take(cur, sizeof(int) * L->pair_cap);
+        L->pair_row = take(cur, sizeof(int) * L->pair_cap);
+        L->weights = take(cur, sizeof(float) * L->n_wfloats);
+        L->nfeat = take(cur, sizeof(float) * rows * H);
+        L->xfeat = take(cur, sizeof(float) * rows * H);
+        L->mfeat = take(cur, sizeof(float) * rows * H);
+        L->Efeat = take(cur, sizeof(float) * rows * H);
+        L->Gfeat = take(cur, sizeof(float) * rows * H);
+        L->carry_m = take(cur, sizeof(float) * L->n_gran_m * 2 * H);
+        L->carry_f = take(cur, sizeof(float) * L->n_gran_f * 2 * 4);
+        L->Fraw = take(cur, sizeof(float) * rows * 4);
+    }
+    L->total = cur;
+    return 0;
+}
+
+// derived, transposed fp32 weights in the order the kernels use (S:G0 is the input order)
+void build_weights(const pimd_net_params *net, std::vector<float> &out, std::vector<size_t> &offs)
+{
+    const int S = net->n_species, K = net->n_rbf, H = net->hidden, L = net->n_layers;
+    const float *w = net->weights;
+    auto mat = [&](int n_out, int n_in) { const float *m = w; w += (size_t)n_out * n_in; return m; };
+    auto vec = [&](int n) { const float *v = w; w += n; return v; };
+    auto pushT = [&](const float *m, int n_out, int n_in) {   // [out][in] -> [in][out]
+        offs.push_back(out.size());
+        for (int k = 0; k < n_in; ++k)
+            for (int o = 0; o < n_out; ++o) out.push_back(m[(size_t)o * n_in + k]);
+    };
+    auto pushV = [&](const float *v, int n) { offs.push_back(out.size()); out.insert(out.end(), v, v + n); };
+    const float *Emb = mat(S, H), *We1 = mat(H, K), *be1 = vec(H), *We2 = mat(H, H), *be2 = vec(H);
+    struct Lw { const float *Ws, *Wvn, *Wvm, *bv1, *Wv2, *bv2, *Wa, *ba; };
+    std::vector<Lw> lw(L);
+    for (int l = 0; l < L; ++l) {
+        lw[l].Ws = mat(H, H); lw[l].Wvn = mat(H, H); lw[l].Wvm = mat(H, H); lw[l].bv1 = vec(H);
+        lw[l].Wv2 = mat(H, H); lw[l].bv2 = vec(H); lw[l].Wa = mat(H, H); lw[l].ba = vec(H);
+    }
+    const float *Wf1 = mat(H, H), *bf1 = vec(H), *wf2 = vec(H);
+    // W_fe = W_f1 W_e2 and b_fe = W_f1 b_e2 + b_f1, formed in fp64 then rounded once
+    std::vector<float> Wfe((size_t)H * H), bfe(H);
+    for (int o = 0; o < H; ++o) {
+        for (int k = 0; k < H; ++k) {
+            double s = 0.0;
+            for (int t = 0; t < H; ++t) s += (double)Wf1[(size_t)o * H + t] * (double)We2[(size_t)t * H + k];
+            Wfe[(size_t)o * H + k] = (float)s;
+        }
+        double s = (double)bf1[o];
+        for (int t = 0; t < H; ++t) s += (double)Wf1[(size_t)o * H + t] * (double)be2[t];
+        bfe[o] = (float)s;
+    }
+    pushV(Emb, S * H);            // 0
+    pushT(We1, H, K);             // 1
+    pushV(be1, H);                // 2
+    pushT(We2, H, H);             // 3
+    pushV(be2, H);                // 4
+    pushT(Wfe.data(), H, H);      // 5
+    pushV(bfe.data(), H);         // 6
+    pushT(Wf1, H, H);             // 7
+    pushV(wf2, H);                // 8
+    for (int l = 0; l < L; ++l) { // 9 + 8 l
+        pushT(lw[l].Ws, H, H); pushT(lw[l].Wvn, H, H); pushT(lw[l].Wvm, H, H); pushV(lw[l].bv1, H);
+        pushT(lw[l].Wv2, H, H); pushV(lw[l].bv2, H); pushT(lw[l].Wa, H, H); pushV(lw[l].ba, H);
+    }
+}
+
+int check_device_error(pimd_ctx *c)
+{
+    int flags[4] = {0, 0, 0, 0};
+    PIMD_CUDA_CHECK(cudaMemcpyAsync(flags, c->err, sizeof(flags), cudaMemcpyDeviceToHost, c->stream));
+    PIMD_CUDA_CHECK(cudaStreamSynchronize(c->stream));
+    if (flags[0] & PIMD_FLAG_PAIRS) {
+        pimd_set_error("pair capacity (%lld pairs, or %d neighbours per atom) exceeded", (long long)c->nl.pair_cap,
+                       PIMD_MAX_NBR);
+        return PIMD_ERR_PAIRS;
+    }
+    if (flags[0] & PIMD_FLAG_NAN) { pimd_set_error("non-finite force or position"); return PIMD_ERR_NAN; }
+    return 0;
+}
+
+int compute_forces(pimd_ctx *c)
+{
+    int rc;
+    if (c->kind == 0) {
+        if ((rc = pimd_launch_nlist(c))) return rc;
+        if ((rc = pimd_launch_gfn_forces(c))) return rc;
+    } else {
+        if ((rc = pimd_launch_simple_forces(c))) return rc;
+    }
+    c->forces_valid = 1;
+    return 0;
+}
+
+}  // namespace
+
+extern "C" int pimd_workspace_bytes(int n_atoms, int n_replicas, int P, const double box[3],
+                                    const pimd_net_params *net, size_t *out)
+{
+    if (!out) { pimd_set_error("null out"); return PIMD_ERR_ARG; }
+    Layout L;
+    int rc = compute_layout(n_atoms, n_replicas, P, box, net, &L);
+    if (rc) return rc;
+    *out = L.total;
+    return 0;
+}
+
+extern "C" int pimd_create(pimd_ctx **out, int n_atoms, int n_replicas, const int32_t *species,
+                           const double *masses_amu, const double *positions, const double box[3], int P,
+                           double T_kelvin, double dt_fs, double gamma_centroid_per_ps, uint64_t seed,
+                           const pimd_net_params *net, void *d_workspace, size_t workspace_bytes, void *cuda_stream)
+{
+    if (!out || !species || !masses_amu || !positions || !box || !net || !d_workspace) {
+        pimd_set_error("null argument");
+        return PIMD_ERR_ARG;
+    }
+    if (!(T_kelvin > 0.0) || !(dt_fs > 0.0)) { pimd_set_error("T and dt must be positive"); return PIMD_ERR_ARG; }
+    Layout L;
+    int rc = compute_layout(n_atoms, n_replicas, P, box, net, &L);
+    if (rc) return rc;
+    if (workspace_bytes < L.total) {
+        pimd_set_error("workspace too small: %zu < %zu", workspace_bytes, L.total);
+        return PIMD_ERR_ARG;
+    }
+    if (((uintptr_t)d_workspace) % 256 != 0) { pimd_set_error("workspace must be 256-byte aligned"); return PIMD_ERR_ARG; }
+    const int N = n_atoms, R = n_replicas;
+    for (int i = 0; i < N; ++i)
+        if (species[i] < 0 || (net->kind == 0 && species[i] >= net->n_species)) {
+            pimd_set_error("species[%d] = %d out of range", i, species[i]);
+            return PIMD_ERR_ARG;
+        }
+    if (net->kind == 0) {
+        if (!net->weights || net->n_weights != packed_weight_floats(net->n_species, net->n_rbf, net->hidden, net->n_layers)) {
+            pimd_set_error("n_weights = %lld, expected %lld", (long long)net->n_weights,
+                           (long long)packed_weight_floats(net->n_species, net->n_rbf, net->hidden, net->n_layers));
+            return PIMD_ERR_ARG;
+        }
+    }
+    pimd_ctx *c = new pimd_ctx();
+    memset(c, 0, sizeof(*c));
+    c->N = N; c->R = R; c->P = P; c->rows = (int64_t)R * P * N;
+    c->periodic = box[0] > 0.0;
+    for (int a = 0; a < 3; ++a) c->box[a] = box[a];
+    c->T = T_kelvin; c->dt = dt_fs; c->gamma_fs = gamma_centroid_per_ps < 0.0 ? -1.0 : gamma_centroid_per_ps * 1e-3;
+    c->seed = seed; c->step = 0; c->kind = net->kind; c->gemm_dtype = net->gemm_dtype;
+    c->harmonic_omega = net->harmonic_omega;
+    c->stream = (cudaStream_t)cuda_stream;
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) {
+        pimd_set_error("no CUDA device: %s", cudaGetErrorString(e));
+        delete c;
+        return PIMD_ERR_CUDA;
+    }
+    char *ws = (char *)d_workspace;
+    c->q = (double *)(ws + L.q); c->p = (double *)(ws + L.p); c->F = (double *)(ws + L.F);
+    c->species = (int *)(ws + L.species); c->mass = (double *)(ws + L.mass);
+    c->Cmat = (double *)(ws + L.C); c->CmatT = (double *)(ws + L.CT); c->omega_k = (double *)(ws + L.omega);
+    c->err = (int *)(ws + L.err);
+    c->est_partial = (double *)(ws + L.est_partial); c->est_out = (double *)(ws + L.est_out);
+
+    // host staging
+    std::vector<double> mass(N), Cm((size_t)P * P), CT((size_t)P * P), om(P), q0((size_t)c->rows * 3);
+    for (int i = 0; i < N; ++i) mass[i] = masses_amu[species[i]] * PIMD_AMU;
+    const double pi = 3.14159265358979323846264338327950288;
+    for (int j = 0; j < P; ++j)   // S:N2
+        for (int k = 0; k < P; ++k) {
+            double v;
+            if (k == 0) v = 1.0 / sqrt((double)P);
+            else if (2 * k < P) v = sqrt(2.0 / P) * cos(2.0 * pi * j * k / P);
+            else if (2 * k == P) v = ((j & 1) ? -1.0 : 1.0) / sqrt((double)P);
+            else v = sqrt(2.0 / P) * sin(2.0 * pi * j * k / P);
+            Cm[(size_t)j * P + k] = v; CT[(size_t)k * P + j] = v;
+        }
+    const double omega_P = P * PIMD_KB * T_kelvin / PIMD_HBAR;   // S:N1
+    for (int k = 0; k < P; ++k) om[k] = 2.0 * omega_P * sin(k * pi / P);
+    for (int r = 0; r < R; ++r)
+        for (int k = 0; k < P; ++k)
+            memcpy(&q0[(((size_t)r * P + k) * N) * 3], positions + (size_t)r * N * 3, sizeof(double) * N * 3);
+
+#define CREATE_CHECK(call)                                                                  \
+    do {                                                                                    \
+        cudaError_t e_ = (call);                                                            \
+        if (e_ != cudaSuccess) {                                                            \
+            pimd_set_error("%s failed: %s", #call, cudaGetErrorString(e_));                 \
+            delete c;                                                                       \
+            return PIMD_ERR_CUDA;                                                           \
+        }                                                                                   \
+    } while (0)
+    cudaStream_t st = c->stream;
+    CREATE_CHECK(cudaMemsetAsync(c->err, 0, sizeof(int) * 4, st));
+    CREATE_CHECK(cudaMemsetAsync(c->F, 0, sizeof(double) * c->rows * 3, st));
+    CREATE_CHECK(cudaMemcpyAsync(c->q, q0.data(), sizeof(double) * q0.size(), cudaMemcpyHostToDevice, st));
+    CREATE_CHECK(cudaMemcpyAsync(c->species, species, sizeof(int) * N, cudaMemcpyHostToDevice, st));
+    CREATE_CHECK(cudaMemcpyAsync(c->mass, mass.data(), sizeof(double) * N, cudaMemcpyHostToDevice, st));
+    CREATE_CHECK(cudaMemcpyAsync(c->Cmat, Cm.data(), sizeof(double) * P * P, cudaMemcpyHostToDevice, st));
+    CREATE_CHECK(cudaMemcpyAsync(c->CmatT, CT.data(), sizeof(double) * P * P, cudaMemcpyHostToDevice, st));
+    CREATE_CHECK(cudaMemcpyAsync(c->omega_k, om.data(), sizeof(double) * P, cudaMemcpyHostToDevice, st));
+
+    std::vector<float> wd;
+    if (net->kind == 0) {
+        const int H = net->hidden;
+        NlistDev &nl = c->nl;
+        for (int a = 0; a < 3; ++a) nl.ncell[a] = L.ncell[a];
+        nl.ncell_tot = L.nct;
+        nl.cell_id = (int *)(ws + L.cell_id); nl.cell_count = (int *)(ws + L.cell_count);
+        nl.cell_start = (int *)(ws + L.cell_start); nl.cell_cursor = (int *)(ws + L.cell_cursor);
+        nl.sorted_atom = (int *)(ws + L.sorted_atom); nl.sorted_q = (double *)(ws + L.sorted_q);
+        nl.nnz = (int *)(ws + L.nnz); nl.row_ptr = (int *)(ws + L.row_ptr); nl.block_sums = (int *)(ws + L.block_sums);
+        nl.col = (int *)(ws + L.col); nl.pair_row = (int *)(ws + L.pair_row); nl.pair_cap = L.pair_cap;
+        c->weights_dev = (float *)(ws + L.weights);
+        c->nfeat = (float *)(ws + L.nfeat); c->xfeat = (float *)(ws + L.xfeat); c->mfeat = (float *)(ws + L.mfeat);
+        c->Efeat = (float *)(ws + L.Efeat); c->Gfeat = (float *)(ws + L.Gfeat);
+        c->carry_m = (float *)(ws + L.carry_m); c->carry_f = (float *)(ws + L.carry_f); c->Fraw = (float *)(ws + L.Fraw);
+        c->gran_m = L.gran_m; c->gran_f = L.gran_f; c->n_gran_m = L.n_gran_m; c->n_gran_f = L.n_gran_f;
+        std::vector<size_t> offs;
+        build_weights(net, wd, offs);
+        if ((int64_t)wd.size() != L.n_wfloats) {
+            pimd_set_error("internal: derived weight count %zu != %lld", wd.size(), (long long)L.n_wfloats);
+            delete c;
+            return PIMD_ERR_ARG;
+        }
+        CREATE_CHECK(cudaMemcpyAsync(c->weights_dev, wd.data(), sizeof(float) * wd.size(), cudaMemcpyHostToDevice, st));
+        GfnDev &g = c->net;
+        g.S = net->n_species; g.K = net->n_rbf; g.H = H; g.L = net->n_layers;
+        g.r_cut = net->r_cut; g.agg_norm = net->agg_norm; g.force_scale = net->force_scale;
+        const float *b = c->weights_dev;
+        g.Emb = b + offs[0]; g.We1T = b + offs[1]; g.be1 = b + offs[2]; g.We2T = b + offs[3]; g.be2 = b + offs[4];
+        g.WfeT = b + offs[5]; g.bfe = b + offs[6]; g.Wf1T = b + offs[7]; g.wf2 = b + offs[8];
+        g.bf2 = net->weights[net->n_weights - 1];
+        for (int l = 0; l < g.L; ++l) {
+            const size_t *o = &offs[9 + 8 * l];
+            g.layer[l].WsT = b + o[0]; g.layer[l].WvnT = b + o[1]; g.layer[l].WvmT = b + o[2]; g.layer[l].bv1 = b + o[3];
+            g.layer[l].Wv2T = b + o[4]; g.layer[l].bv2 = b + o[5]; g.layer[l].WaT = b + o[6]; g.layer[l].ba = b + o[7];
+        }
+        CREATE_CHECK(cudaMemsetAsync(nl.row_ptr, 0, sizeof(int) * (c->rows + 1), st));
+    }
+    rc = pimd_launch_init_momenta(c);   // S:N5
+    if (rc) { delete c; return rc; }
+    CREATE_CHECK(cudaStreamSynchronize(st));   // host staging buffers go out of scope below
+#undef CREATE_CHECK
+    c->forces_valid = 0;
+    *out = c;
+    return 0;
+}
+
+extern "C" void pimd_destroy(pimd_ctx *c)
+{
+    if (!c) return;
+    cudaStreamSynchronize(c->stream);
+    delete c;
+}
+
+extern "C" int pimd_step(pimd_ctx *c, int n)
+{
+    if (!c || n < 0) { pimd_set_error("invalid argument"); return PIMD_ERR_ARG; }
+    int rc;
+    if (!c->forces_valid && (rc = compute_forces(c))) return rc;
+    for (int s = 0; s < n; ++s) {
+        const uint32_t t = (uint32_t)c->step;
+        if ((rc = pimd_launch_nm_pre(c, t))) return rc;     // O(dt/2) B(dt/2) A(dt)
+        if ((rc = compute_forces(c))) return rc;            // neighbour list + forces at the new positions
+        if ((rc = pimd_launch_nm_post(c, t))) return rc;    // B(dt/2) O(dt/2)
+        c->step += 1;
+    }
+    return 0;
+}
+
+extern "C" int pimd_forces(pimd_ctx *c, float *d_out)
+{
+    if (!c || !d_out) { pimd_set_error("null argument"); return PIMD_ERR_ARG; }
+    int rc;
+    if ((rc = compute_forces(c))) return rc;
+    return pimd_launch_copy_forces_f32(c, d_out);
+}
+
+extern "C" int pimd_estimators(pimd_ctx *c, pimd_estimators_t *h_out)
+{
+    if (!c || !h_out) { pimd_set_error("null argument"); return PIMD_ERR_ARG; }
+    int rc;
+    if (!c->forces_valid && (rc = compute_forces(c))) return rc;
+    if ((rc = pimd_launch_estimators(c))) return rc;
+    std::vector<double> tmp((size_t)c->R * 8);
+    PIMD_CUDA_CHECK(cudaMemcpyAsync(tmp.data(), c->est_out, sizeof(double) * tmp.size(), cudaMemcpyDeviceToHost, c->stream));
+    if ((rc = check_device_error(c))) return rc;   // synchronises
+    for (int r = 0; r < c->R; ++r) {
+        h_out[r].k_prim = tmp[r * 8 + 0]; h_out[r].k_vir = tmp[r * 8 + 1]; h_out[r].k_cvir = tmp[r * 8 + 2];
+        h_out[r].v_pot = tmp[r * 8 + 3]; h_out[r].t_centroid = tmp[r * 8 + 4];
+    }
+    return 0;
+}
+
+extern "C" int pimd_get_state(pimd_ctx *c, double *d_q, double *d_p, int64_t *step)
+{
+    if (!c) { pimd_set_error("null context"); return PIMD_ERR_ARG; }
+    const size_t bytes = sizeof(double) * (size_t)c->rows * 3;
+    if (d_q) PIMD_CUDA_CHECK(cudaMemcpyAsync(d_q, c->q, bytes, cudaMemcpyDeviceToDevice, c->stream));
+    if (d_p) PIMD_CUDA_CHECK(cudaMemcpyAsync(d_p, c->p, bytes, cudaMemcpyDeviceToDevice, c->stream));
+    if (step) *step = c->step;
+    return check_device_error(c);
+}
+
+extern "C" int pimd_set_state(pimd_ctx *c, const double *d_q, const double *d_p, int64_t step)
+{
+    if (!c) { pimd_set_error("null context"); return PIMD_ERR_ARG; }
+    const size_t bytes = sizeof(double) * (size_t)c->rows * 3;
+    if (d_q) PIMD_CUDA_CHECK(cudaMemcpyAsync(c->q, d_q, bytes, cudaMemcpyDeviceToDevice, c->stream));
+    if (d_p) PIMD_CUDA_CHECK(cudaMemcpyAsync(c->p, d_p, bytes, cudaMemcpyDeviceToDevice, c->stream));
+    c->step = step;
+    c->forces_valid = 0;
+    return 0;
+}
+
+extern "C" int pimd_nlist(pimd_ctx *c, int32_t *d_row_ptr, int32_t *d_col, int64_t col_capacity, int64_t *h_n_pairs)
+{
+    if (!c || !d_row_ptr || !d_col || !h_n_pairs) { pimd_set_error("null argument"); return PIMD_ERR_ARG; }
+    if (c->kind != 0) { pimd_set_error("no neighbour list for this potential kind"); return PIMD_ERR_ARG; }
+    int rc;
+    if ((rc = pimd_launch_nlist(c))) return rc;
+    int n = 0;
+    PIMD_CUDA_CHECK(cudaMemcpyAsync(&n, c->nl.row_ptr + c->rows, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    if ((rc = check_device_error(c))) return rc;
+    *h_n_pairs = n;
+    if (n > col_capacity) { pimd_set_error("col_capacity %lld < %d pairs", (long long)col_capacity, n); return PIMD_ERR_PAIRS; }
+    PIMD_CUDA_CHECK(cudaMemcpyAsync(d_row_ptr, c->nl.row_ptr, sizeof(int) * (c->rows + 1), cudaMemcpyDeviceToDevice, c->stream));
+    PIMD_CUDA_CHECK(cudaMemcpyAsync(d_col, c->nl.col, sizeof(int) * (size_t)n, cudaMemcpyDeviceToDevice, c->stream));
+    PIMD_CUDA_CHECK(cudaStreamSynchronize(c->stream));
+    return 0;
+}
+
+extern "C" int pimd_sync(pimd_ctx *c)
+{
+    if (!c) { pimd_set_error("null context"); return PIMD_ERR_ARG; }
+    return check_device_error(c);
+}
+
+extern "C" int64_t pimd_launch_count(const pimd_ctx *c) { return c ? c->launches : 0; }

@@ -1,0 +1,187 @@
+"""ctypes binding of include/pimd.h (argument marshalling only; same names as the C-ABI)."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(HERE, "libpimd_b200.so")
+_lib = None
+
+
+class PimdError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"pimd error {code}: {msg}")
+        self.code = code
+
+
+class NetParams(C.Structure):
+    """Mirror of `pimd_net_params`."""
+    _fields_ = [
+        ("kind", C.c_int32), ("n_species", C.c_int32), ("n_rbf", C.c_int32), ("hidden", C.c_int32),
+        ("n_layers", C.c_int32), ("gemm_dtype", C.c_int32),
+        ("r_cut", C.c_float), ("agg_norm", C.c_float), ("force_scale", C.c_float),
+        ("harmonic_omega", C.c_double),
+        ("weights", C.POINTER(C.c_float)), ("n_weights", C.c_int64),
+    ]
+
+
+class Estimators(C.Structure):
+    """Mirror of `pimd_estimators_t`."""
+    _fields_ = [("k_prim", C.c_double), ("k_vir", C.c_double), ("k_cvir", C.c_double), ("v_pot", C.c_double),
+                ("t_centroid", C.c_double)]
+
+
+def library_path() -> str:
+    return _LIB_PATH
+
+
+def load_library():
+    """Loads libpimd_b200.so (built in-tree by paper_2503_23728_b200/build.py).  Raises if absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise ImportError(f"{_LIB_PATH} is missing: run `python -m paper_2503_23728_b200.build` "
+                          "(there is no CPU fallback)")
+    L = C.CDLL(_LIB_PATH)
+    vp, dp, ip = C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int32)
+    L.pimd_workspace_bytes.argtypes = [C.c_int, C.c_int, C.c_int, dp, C.POINTER(NetParams), C.POINTER(C.c_size_t)]
+    L.pimd_create.argtypes = [C.POINTER(vp), C.c_int, C.c_int, ip, dp, dp, dp, C.c_int, C.c_double, C.c_double,
+                              C.c_double, C.c_uint64, C.POINTER(NetParams), vp, C.c_size_t, vp]
+    L.pimd_step.argtypes = [vp, C.c_int]
+    L.pimd_forces.argtypes = [vp, vp]
+    L.pimd_estimators.argtypes = [vp, C.POINTER(Estimators)]
+    L.pimd_get_state.argtypes = [vp, vp, vp, C.POINTER(C.c_int64)]
+    L.pimd_set_state.argtypes = [vp, vp, vp, C.c_int64]
+    L.pimd_nlist.argtypes = [vp, vp, vp, C.c_int64, C.POINTER(C.c_int64)]
+    L.pimd_sync.argtypes = [vp]
+    L.pimd_launch_count.argtypes = [vp]
+    L.pimd_launch_count.restype = C.c_int64
+    L.pimd_last_error.restype = C.c_char_p
+    L.pimd_destroy.argtypes = [vp]
+    L.pimd_destroy.restype = None
+    _lib = L
+    return L
+
+
+def _check(rc):
+    if rc != 0:
+        raise PimdError(rc, load_library().pimd_last_error().decode())
+
+
+def _net_struct(net, keep):
+    """net: any object with the NetSpec fields (duck-typed)."""
+    w = np.ascontiguousarray(net.weights if net.weights is not None else np.zeros(0), dtype=np.float32)
+    keep.append(w)
+    return NetParams(int(net.kind), int(net.n_species), int(net.n_rbf), int(net.hidden), int(net.n_layers),
+                     int(getattr(net, "gemm_dtype", 0)), float(net.r_cut), float(net.agg_norm),
+                     float(net.force_scale), float(net.harmonic_omega),
+                     w.ctypes.data_as(C.POINTER(C.c_float)), int(w.size if int(net.kind) == 0 else 0))
+
+
+class PIMD:
+    """Owns the torch workspace tensor and the `pimd_ctx*`; methods are the C-ABI calls."""
+
+    def __init__(self, species, masses_amu, positions, box, P, T, dt, gamma, seed, net, device="cuda:0",
+                 stream=None):
+        import torch
+
+        L = load_library()
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2503_23728_b200 needs a CUDA device (no CPU fallback)")
+        self._torch = torch
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        species = np.ascontiguousarray(species, dtype=np.int32)
+        masses = np.ascontiguousarray(masses_amu, dtype=np.float64)
+        pos = np.ascontiguousarray(positions, dtype=np.float64)
+        if pos.ndim == 2:
+            pos = pos[None]
+        box = np.ascontiguousarray(box, dtype=np.float64)
+        self.R, self.N, self.P = int(pos.shape[0]), int(pos.shape[1]), int(P)
+        self.rows = self.R * self.P * self.N
+        self.shape = (self.R, self.P, self.N, 3)
+        self._keep = []
+        npar = _net_struct(net, self._keep)
+        self.kind = int(net.kind)
+        dp, ip = C.POINTER(C.c_double), C.POINTER(C.c_int32)
+        nbytes = C.c_size_t()
+        _check(L.pimd_workspace_bytes(self.N, self.R, self.P, box.ctypes.data_as(dp), C.byref(npar), C.byref(nbytes)))
+        self.workspace_bytes = int(nbytes.value)
+        self.workspace = torch.empty(self.workspace_bytes + 256, dtype=torch.uint8, device=self.device)
+        base = self.workspace.data_ptr()
+        self._ws_ptr = (base + 255) // 256 * 256
+        self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        h = C.c_void_p()
+        _check(L.pimd_create(C.byref(h), self.N, self.R, species.ctypes.data_as(ip), masses.ctypes.data_as(dp),
+                             pos.ctypes.data_as(dp), box.ctypes.data_as(dp), self.P, float(T), float(dt), float(gamma),
+                             int(seed), C.byref(npar), C.c_void_p(self._ws_ptr), self.workspace_bytes,
+                             C.c_void_p(self.stream.cuda_stream)))
+        self._h = h
+
+    @classmethod
+    def from_workload(cls, w, **kw):
+        return cls(w.species, w.masses_amu, w.positions, w.box, w.P, w.T, w.dt, w.gamma, w.seed, w.net, **kw)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            load_library().pimd_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- C-ABI calls -------------------------------------------------------------------------
+    def step(self, n=1):
+        _check(load_library().pimd_step(self._h, int(n)))
+
+    def forces(self, out=None):
+        t = self._torch
+        if out is None:
+            out = t.empty(self.shape, dtype=t.float32, device=self.device)
+        _check(load_library().pimd_forces(self._h, C.c_void_p(out.data_ptr())))
+        return out
+
+    def estimators(self):
+        out = (Estimators * self.R)()
+        _check(load_library().pimd_estimators(self._h, out))
+        return np.array([[e.k_prim, e.k_vir, e.k_cvir, e.v_pot, e.t_centroid] for e in out])
+
+    def get_state(self):
+        t = self._torch
+        q = t.empty(self.shape, dtype=t.float64, device=self.device)
+        p = t.empty(self.shape, dtype=t.float64, device=self.device)
+        st = C.c_int64()
+        _check(load_library().pimd_get_state(self._h, C.c_void_p(q.data_ptr()), C.c_void_p(p.data_ptr()), C.byref(st)))
+        return q, p, int(st.value)
+
+    def set_state(self, q, p, step):
+        t = self._torch
+        q = t.as_tensor(q, dtype=t.float64, device=self.device).contiguous()
+        p = t.as_tensor(p, dtype=t.float64, device=self.device).contiguous()
+        assert q.numel() == self.rows * 3 and p.numel() == self.rows * 3
+        _check(load_library().pimd_set_state(self._h, C.c_void_p(q.data_ptr()), C.c_void_p(p.data_ptr()), int(step)))
+        self.sync()  # q, p temporaries may be freed by the caller right after
+
+    def nlist(self, cap_per_row=None):
+        t = self._torch
+        cap = int(self.rows * (cap_per_row if cap_per_row else min(max(self.N - 1, 1), 512)))
+        row_ptr = t.empty(self.rows + 1, dtype=t.int32, device=self.device)
+        col = t.empty(max(cap, 1), dtype=t.int32, device=self.device)
+        n = C.c_int64()
+        _check(load_library().pimd_nlist(self._h, C.c_void_p(row_ptr.data_ptr()), C.c_void_p(col.data_ptr()), cap,
+                                         C.byref(n)))
+        return row_ptr, col[: n.value]
+
+    def sync(self):
+        _check(load_library().pimd_sync(self._h))
+
+    def launch_count(self) -> int:
+        return int(load_library().pimd_launch_count(self._h))

@@ -1,0 +1,113 @@
+"""GPU parity: GFN direct forces and full PIMD trajectories vs the fp64 oracle (through the C-ABI).
+
+Tolerances (BASELINE.json north_star): forces within 1e-4 relative + 1e-4 eV/A absolute in fp32,
+2e-2 relative on the bf16 configs; bead positions after 200 steps within 1e-4 A.
+"""
+import numpy as np
+import pytest
+
+import oracle
+import pimd_inputs as pi
+from gpu_util import make_pair, pair_from_workload, spread_beads, gpu_state, assert_forces_close
+
+pytestmark = pytest.mark.gpu
+
+RTOL32, ATOL32 = 1e-4, 1e-4
+RTOL16 = 2e-2
+
+
+def _forces_pair(gpu, ref):
+    return gpu.forces().cpu().numpy().astype(np.float64), ref.forces()
+
+
+def _biased_spec(K, H, L, rc, agg, fs, seed=4):
+    return pi.NetSpec(0, 3, K, H, L, 0, rc, agg, fs, 0.0, pi.pack_weights(seed, 3, K, H, L, bias_scale=0.2))
+
+
+@pytest.mark.parametrize("K,H", [(32, 64), (64, 128)])
+@pytest.mark.parametrize("L", [0, 1, 3])
+def test_small_systems_with_biases(cuda_device, K, H, L):
+    rng = np.random.default_rng(L)
+    # open cluster (one cell) and a periodic box with 2 cells per edge; sizes give ragged tiles
+    for box, n_at, P in [(np.zeros(3), 23, 3), (np.array([6.5, 7.0, 9.2]), 77, 2)]:
+        x = rng.uniform(0, 1, (2, n_at, 3)) * (box if box[0] > 0 else 4.5)
+        sp = rng.integers(0, 3, n_at).astype(np.int32)
+        gpu, ref = make_pair(sp, x, box, P, 300.0, 0.25, 1.0, 0, _biased_spec(K, H, L, 3.0, 1.0 / 12.0, 0.2))
+        spread_beads(gpu, ref, scale=0.05)
+        Fg, Fr = _forces_pair(gpu, ref)
+        assert np.abs(Fr).max() > 1e-3
+        assert_forces_close(Fg, Fr, RTOL32, ATOL32, f"K{K} H{H} L{L} box{box[0]}")
+        assert np.abs(Fg.sum(axis=2)).max() < 1e-4  # momentum conservation per bead-system
+
+
+@pytest.mark.parametrize("name", ["fad_p8", "fad_x64_p32", "water64"])
+def test_fp32_workload_forces(cuda_device, name):
+    w = pi.make_workload(name)
+    gpu, ref = pair_from_workload(w)
+    spread_beads(gpu, ref, scale=0.03)
+    Fg, Fr = _forces_pair(gpu, ref)
+    assert 0.2 < np.sqrt((Fr ** 2).sum(-1).mean()) < 3.0
+    assert_forces_close(Fg, Fr, RTOL32, ATOL32, name)
+
+
+@pytest.mark.parametrize("name,beads", [("ice512", [0, 13, 31]), ("water4096", [7])])
+def test_full_size_forces_on_sampled_beads(cuda_device, name, beads):
+    """Full workload in the launch configuration bench.py times; the oracle evaluates sampled
+    bead-systems one by one (forces of a bead depend only on that bead's positions)."""
+    import paper_2503_23728_b200 as pb
+    w = pi.make_workload(name)
+    gpu = pb.PIMD.from_workload(w)
+    q, p, st = gpu_state(gpu)
+    q = q + 0.03 * np.random.default_rng(3).standard_normal(q.shape)
+    gpu.set_state(q, p, st)
+    Fg = gpu.forces().cpu().numpy().astype(np.float64)
+    rtol = RTOL16 if w.net.gemm_dtype == 1 else RTOL32
+    atol = 2e-2 if w.net.gemm_dtype == 1 else ATOL32
+    for k in beads:
+        ref = oracle.RefPIMD(w.species, w.masses_amu, q[0, k][None], w.box, 1, w.T, w.dt, -1.0, 0,
+                             oracle.RefNet.from_spec(w.net))
+        Fr = ref.forces()[0, 0]
+        assert_forces_close(Fg[0, k], Fr, rtol, atol, f"{name} bead {k}")
+    assert np.isfinite(Fg).all()
+    assert np.abs(Fg.sum(axis=2)).max() < 5e-2
+
+
+def test_forces_are_bitwise_deterministic(cuda_device):
+    import torch
+    w = pi.make_workload("water64")
+    gpu, ref = pair_from_workload(w)
+    spread_beads(gpu, ref, scale=0.03)
+    a = gpu.forces().clone()
+    for _ in range(3):
+        assert torch.equal(a, gpu.forces())
+
+
+def test_fad_trajectory_200_steps(cuda_device):
+    """configs[0]: 200 PIMD steps with PILE-L; bead positions within 1e-4 A of the oracle."""
+    w = pi.make_workload("fad_p8")
+    gpu, ref = pair_from_workload(w)
+    gpu.step(w.n_steps); ref.step(w.n_steps)
+    qg, pg, sg = gpu_state(gpu)
+    qr, pr, sr = ref.get_state()
+    assert sg == sr == 200
+    assert np.abs(qg - qr).max() < 1e-4, np.abs(qg - qr).max()
+    assert np.abs(qr - w.positions[0][None, None]).max() > 0.01  # the system actually moved
+
+
+def test_replica_batch_trajectory(cuda_device):
+    """configs[1] launch configuration (64 replicas x 32 beads), 20 steps, vs the oracle."""
+    w = pi.make_workload("fad_x64_p32")
+    gpu, ref = pair_from_workload(w)
+    gpu.step(20); ref.step(20)
+    qg, _, _ = gpu_state(gpu); qr, _, _ = ref.get_state()
+    assert np.abs(qg - qr).max() < 1e-4
+
+
+def test_water64_trajectory_short(cuda_device):
+    w = pi.make_workload("water64")
+    gpu, ref = pair_from_workload(w)
+    gpu.step(4); ref.step(4)
+    qg, _, _ = gpu_state(gpu); qr, _, _ = ref.get_state()
+    assert np.abs(qg - qr).max() < 1e-4
+    eg, er = gpu.estimators(), ref.estimators()
+    assert np.allclose(eg[:, :3], er[:, :3], rtol=1e-3, atol=1e-3) and np.isnan(eg[0, 3])
