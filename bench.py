@@ -1,0 +1,288 @@
+#!/usr/bin/env python
+"""bench.py -- headline benchmark of the PIMD hot path (BASELINE.json metric).
+
+A "step" is one pass of the whole hot path (neighbour list -> GFN forces -> normal-mode
+propagation + PILE-L) over all beads of the workload, i.e. one `pimd_step(1)`.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload ice512] [--impl ours|reference]
+
+Prints ONE JSON line (rank 0).  N > 1 runs N independent replicas of the workload, one per GPU
+("replicas only": the path has no data-path collective), value = all ranks' units / max-over-ranks time.
+`--impl reference` times the fp64 CPU oracle as it stands on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import os
+
+os.environ.setdefault("OMP_WAIT_POLICY", "passive")
+
+import argparse
+import json
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import pimd_inputs as pi  # noqa: E402
+
+METRIC = "pimd_atom_bead_steps_per_s"
+UNIT = "atom*bead*steps/s"
+FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12  # 74.4: SMs x FP32 lanes x 2 (FMA) x clocks.max.sm
+
+
+def measured_peaks():
+    try:
+        return json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        sm, smax, reasons = [], [], set()
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); smax.append(float(f[1]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def flops_per_pair_pass(K, H):
+    """Algorithmic flops of one directed pair in one pair pass: 2KH + 2H^2 + ~8H."""
+    return 2 * K * H + 2 * H * H + 8 * H
+
+
+# ------------------------------------------------------------------------------------------------
+def run_reference(args):
+    """The oracle, as it stands, on the host cores; each step = one PIMD step of a bounded sample."""
+    import oracle
+    w = pi.make_workload(args.workload)
+    P_s = min(w.P, args.ref_beads)
+    ref = oracle.RefPIMD(w.species, w.masses_amu, w.positions[:1], w.box, P_s, w.T, w.dt, w.gamma, w.seed,
+                         oracle.RefNet.from_spec(w.net))
+    ref.forces()
+    for _ in range(args.warmup):
+        ref.step(1)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        ref.step(1)
+    dt = time.perf_counter() - t0
+    units = w.n_atoms * P_s * args.steps
+    v = units / dt
+    sample = f"{args.workload}: first {P_s} of {w.P} bead-systems of replica 0 (a P={P_s} ring at the same T), all {w.n_atoms} atoms"
+    out = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+           "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": {"workload": args.workload, "sample": sample},
+           "cpu_baseline": {"value": v, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle", "sample": sample},
+           "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(out))
+
+
+def cpu_baseline(w, budget_beads):
+    import oracle
+    P_s = min(w.P, budget_beads)
+    ref = oracle.RefPIMD(w.species, w.masses_amu, w.positions[:1], w.box, P_s, w.T, w.dt, w.gamma, w.seed,
+                         oracle.RefNet.from_spec(w.net))
+    ref.forces()
+    t0 = time.perf_counter()
+    n = 0
+    while True:
+        ref.step(1)
+        n += 1
+        if time.perf_counter() - t0 > 10.0 or n >= 200:
+            break
+    dt = time.perf_counter() - t0
+    return {"value": w.n_atoms * P_s * n / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": f"{n} oracle step(s) of {w.name} restricted to the first {P_s} of {w.P} bead-systems "
+                      f"({w.n_atoms} atoms each), {dt:.1f} s"}
+
+
+# ------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import paper_2503_23728_b200 as pb
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    dev = torch.device(f"cuda:{local}")
+    torch.cuda.set_device(dev)
+
+    w = pi.make_workload(args.workload)
+    if world > 1:  # independent replica per rank: different thermostat stream, same workload shape
+        w.seed = w.seed + rank
+    sim = pb.PIMD.from_workload(w, device=str(dev))
+    stream = torch.cuda.current_stream(dev)
+    flush = torch.empty(512 * 1024 * 1024 // 4, dtype=torch.float32, device=dev)  # 512 MB > 126 MB L2
+
+    def barrier():
+        torch.cuda.synchronize(dev)
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    # ---- device-resident timing: K steps, CUDA events around each step, L2 flushed between steps
+    sim.step(args.warmup)
+    sim.sync()
+    rp0, _ = sim.nlist()
+    pairs_first = int(rp0[-1].item())
+    sampler = ClockSampler(local)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    barrier()
+    if rank == 0:
+        sampler.start()
+    l0 = sim.launch_count()
+    sim.profile(True)
+    wall0 = time.perf_counter()
+    for a, b in ev:
+        flush.add_(1.0)
+        a.record(stream)
+        sim.step(1)
+        b.record(stream)
+    barrier()
+    wall = time.perf_counter() - wall0
+    prof = sim.profile_read()
+    sim.profile(False)
+    launches = sim.launch_count() - l0
+    clocks = sampler.stop() if rank == 0 else None
+    t_dev = sum(a.elapsed_time(b) for a, b in ev) * 1e-3
+    sim.sync()
+    rp1, _ = sim.nlist()
+    pairs_last = int(rp1[-1].item())
+
+    # ---- end to end: host state -> H2D -> pimd_set_state -> pimd_step(1) -> pimd_get_state -> D2H, every step
+    q, p, st = sim.get_state()
+    hq, hp = q.cpu().pin_memory(), p.cpu().pin_memory()
+    dq, dp = torch.empty_like(q), torch.empty_like(p)
+    e2e_steps = max(3, min(args.steps, 10))
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for i in range(e2e_steps):
+        dq.copy_(hq, non_blocking=True); dp.copy_(hp, non_blocking=True)
+        sim.set_state(dq, dp, st + i)
+        sim.step(1)
+        q2, p2, _ = sim.get_state()
+        hq.copy_(q2, non_blocking=True); hp.copy_(p2, non_blocking=True)
+        stream.synchronize()
+    e1.record(stream)
+    barrier()
+    t_e2e = e0.elapsed_time(e1) * 1e-3
+    state_bytes = int(q.numel() * 8 * 2)
+
+    times = torch.tensor([t_dev, t_e2e], dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(times, op=dist.ReduceOp.MAX)
+    t_dev, t_e2e = float(times[0]), float(times[1])
+
+    if rank == 0:
+        units = w.rows * args.steps * world
+        value = units / t_dev
+        K, H, L = w.net.n_rbf, w.net.hidden, w.net.n_layers
+        pairs = 0.5 * (pairs_first + pairs_last)
+        pair_ms, pair_n = prof["gfn.pair"]
+        head_ms, head_n = prof["gfn.head"]
+        # dominant kernel: the pair kernel (message passes + force head share one code path)
+        n_launch = pair_n + head_n
+        avg_s = (pair_ms + head_ms) * 1e-3 / max(n_launch, 1)
+        achieved = pairs * flops_per_pair_pass(K, H) / avg_s / 1e12 if n_launch else 0.0
+        traffic = None
+        try:
+            traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(args.workload)
+        except Exception:
+            pass
+        out = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": 1e3 * t_dev / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": args.workload, "atoms": w.n_atoms, "beads": w.P, "replicas_per_gpu": w.n_replicas,
+                       "rows_per_gpu": w.rows, "n_rbf": K, "hidden": H, "layers": L, "r_cut": w.net.r_cut,
+                       "pairs_per_row_first": pairs_first / w.rows, "pairs_per_row_last": pairs_last / w.rows,
+                       "l2": "512 MB buffer rewritten between timed steps (flush)", "parallelism": f"replicas x{world}",
+                       "timing": "sum of per-step CUDA-event intervals on the launch stream"},
+            "ns_per_day": args.steps / t_dev * w.dt * 86400e-6,
+            "wall_ms_per_step_incl_flush": 1e3 * wall / args.steps,
+            "e2e": {"value": w.rows * e2e_steps * world / t_e2e, "unit": UNIT, "h2d_bytes_per_step": state_bytes,
+                    "d2h_bytes_per_step": state_bytes, "steps": e2e_steps,
+                    "path": "pinned host q,p -> H2D -> pimd_set_state -> pimd_step(1) -> pimd_get_state -> D2H"},
+            "gpu_launches": int(launches),
+            "clocks": clocks,
+            "kernel_ms_per_step": {k: v[0] / args.steps for k, v in prof.items()},
+            "roofline": {"kernel": "gfn::pair_kernel (message + head passes)", "bound": "alu", "achieved": achieved,
+                         "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP32_PEAK_TFLOPS,
+                         "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (MEASURED_PEAKS has no fp32 figure)",
+                         "launches_timed": n_launch, "avg_launch_ms": avg_s * 1e3,
+                         "flops_per_launch": pairs * flops_per_pair_pass(K, H), "traffic": traffic},
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            out["cpu_baseline"] = cpu_baseline(w, args.ref_beads)
+        print(json.dumps(out))
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="ice512", choices=pi.workload_names())
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--ref-beads", type=int, default=2, help="bead-systems in the oracle's bounded sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        if int(os.environ.get("RANK", "0")) == 0:
+            run_reference(args)
+        return
+    run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -126,6 +126,15 @@ int pimd_nlist(pimd_ctx *ctx, int32_t *d_row_ptr, int32_t *d_col, int64_t col_ca
 /* Waits for the stream and returns any latched device error. */
 int pimd_sync(pimd_ctx *ctx);
 
+/* Per-kernel-class device timing with CUDA events recorded on the context's stream around each launch
+ * (classes: 0 pimd_nm, 1 nlist, 2 gfn.pair message pass, 3 gfn.node, 4 gfn.head, 5 other).
+ * pimd_profile(ctx, 1) starts (and clears) recording, pimd_profile(ctx, 0) stops it.
+ * pimd_profile_read synchronises and writes, per class, the summed milliseconds and the number of
+ * timed launches into HOST arrays of length 6. */
+#define PIMD_PROF_CLASSES 6
+int pimd_profile(pimd_ctx *ctx, int enable);
+int pimd_profile_read(pimd_ctx *ctx, double *h_ms, int64_t *h_launches);
+
 /* Number of kernels the library has launched on this context so far (HOST counter). */
 int64_t pimd_launch_count(const pimd_ctx *ctx);
 

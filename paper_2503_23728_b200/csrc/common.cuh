@@ -86,7 +86,18 @@ struct pimd_ctx {
     float *Fraw;                       // [rows][4] complete-row partial force sums
     int gran_m, gran_f;                // pairs per reduction granule
     int64_t n_gran_m, n_gran_f;
+    struct PimdProf *prof;             // host-side event recorder (pimd_profile)
 };
+
+// records a CUDA event pair on the context's stream around the launches made in its scope
+void pimd_prof_begin(pimd_ctx *c, int kind);
+void pimd_prof_end(pimd_ctx *c);
+struct ProfScope {
+    pimd_ctx *c;
+    ProfScope(pimd_ctx *ctx, int kind) : c(ctx) { if (c->prof) pimd_prof_begin(c, kind); }
+    ~ProfScope() { if (c->prof) pimd_prof_end(c); }
+};
+enum { PROF_NM = 0, PROF_NLIST = 1, PROF_PAIR = 2, PROF_NODE = 3, PROF_HEAD = 4, PROF_OTHER = 5 };
 
 void pimd_set_error(const char *fmt, ...);
 

@@ -241,13 +241,24 @@ int pimd_launch_gfn_forces(pimd_ctx *c)
     if (L == 0) {
         PIMD_CUDA_CHECK(cudaMemsetAsync(c->Gfeat, 0, sizeof(float) * (size_t)c->rows * c->net.H, c->stream));
     } else {
-        if ((rc = gfn::launch_node(c, 0, 0))) return rc;
+        {
+            ProfScope ps(c, PROF_NODE);
+            if ((rc = gfn::launch_node(c, 0, 0))) return rc;
+        }
         for (int l = 0; l < L; ++l) {
-            if ((rc = gfn::launch_pair(c, l, false))) return rc;
+            {
+                ProfScope ps(c, PROF_PAIR);
+                if ((rc = gfn::launch_pair(c, l, false))) return rc;
+            }
+            ProfScope ps(c, PROF_NODE);
             if ((rc = gfn::launch_node(c, 1, l))) return rc;
         }
     }
-    if ((rc = gfn::launch_pair(c, L, true))) return rc;
+    {
+        ProfScope ps(c, PROF_HEAD);
+        if ((rc = gfn::launch_pair(c, L, true))) return rc;
+    }
+    ProfScope ps(c, PROF_OTHER);
     gfn::force_finalize_kernel<<<(unsigned)((c->rows + 255) / 256), 256, 0, c->stream>>>(
         c->rows, c->nl.row_ptr, c->gran_f, c->net.force_scale, c->Fraw, c->carry_f, c->F);
     c->launches++;

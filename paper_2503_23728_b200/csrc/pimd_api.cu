@@ -21,6 +21,41 @@ void pimd_set_error(const char *fmt, ...)
 
 extern "C" const char *pimd_last_error(void) { return g_err; }
 
+struct PimdProf {
+    bool on = false;
+    struct Rec { int kind; cudaEvent_t a, b; };
+    std::vector<Rec> recs;
+    std::vector<cudaEvent_t> pool;
+    cudaEvent_t get()
+    {
+        if (!pool.empty()) { cudaEvent_t e = pool.back(); pool.pop_back(); return e; }
+        cudaEvent_t e;
+        cudaEventCreate(&e);
+        return e;
+    }
+    void clear()
+    {
+        for (auto &r : recs) { pool.push_back(r.a); pool.push_back(r.b); }
+        recs.clear();
+    }
+};
+
+void pimd_prof_begin(pimd_ctx *c, int kind)
+{
+    PimdProf *p = c->prof;
+    if (!p || !p->on) return;
+    PimdProf::Rec r{kind, p->get(), p->get()};
+    cudaEventRecord(r.a, c->stream);
+    p->recs.push_back(r);
+}
+
+void pimd_prof_end(pimd_ctx *c)
+{
+    PimdProf *p = c->prof;
+    if (!p || !p->on || p->recs.empty()) return;
+    cudaEventRecord(p->recs.back().b, c->stream);
+}
+
 namespace {
 
 struct Layout {
@@ -42,7 +77,7 @@ size_t take(size_t &cur, size_t bytes)
 
 int64_t derived_weight_floats(int S, int K, int H, int L)
 {
-    return (int64_t)S * H + (int64_t)K * H + H + 3LL * H * H + 4LL * H + (int64_t)L * (5LL * H * H + 3LL * H);
+    return (int64_t)S * H + (int64_t)K * H + 3LL * H * H + 4LL * H + (int64_t)L * (5LL * H * H + 3LL * H);
 }
 
 int64_t packed_weight_floats(int S, int K, int H, int L)
@@ -210,9 +245,13 @@ int compute_forces(pimd_ctx *c)
 {
     int rc;
     if (c->kind == 0) {
-        if ((rc = pimd_launch_nlist(c))) return rc;
+        {
+            ProfScope ps(c, PROF_NLIST);
+            if ((rc = pimd_launch_nlist(c))) return rc;
+        }
         if ((rc = pimd_launch_gfn_forces(c))) return rc;
     } else {
+        ProfScope ps(c, PROF_OTHER);
         if ((rc = pimd_launch_simple_forces(c))) return rc;
     }
     c->forces_valid = 1;
@@ -376,6 +415,11 @@ extern "C" void pimd_destroy(pimd_ctx *c)
 {
     if (!c) return;
     cudaStreamSynchronize(c->stream);
+    if (c->prof) {
+        c->prof->clear();
+        for (auto e : c->prof->pool) cudaEventDestroy(e);
+        delete c->prof;
+    }
     delete c;
 }
 
@@ -386,9 +430,15 @@ extern "C" int pimd_step(pimd_ctx *c, int n)
     if (!c->forces_valid && (rc = compute_forces(c))) return rc;
     for (int s = 0; s < n; ++s) {
         const uint32_t t = (uint32_t)c->step;
-        if ((rc = pimd_launch_nm_pre(c, t))) return rc;     // O(dt/2) B(dt/2) A(dt)
+        {
+            ProfScope ps(c, PROF_NM);
+            if ((rc = pimd_launch_nm_pre(c, t))) return rc;     // O(dt/2) B(dt/2) A(dt)
+        }
         if ((rc = compute_forces(c))) return rc;            // neighbour list + forces at the new positions
-        if ((rc = pimd_launch_nm_post(c, t))) return rc;    // B(dt/2) O(dt/2)
+        {
+            ProfScope ps(c, PROF_NM);
+            if ((rc = pimd_launch_nm_post(c, t))) return rc;    // B(dt/2) O(dt/2)
+        }
         c->step += 1;
     }
     return 0;
@@ -460,6 +510,31 @@ extern "C" int pimd_sync(pimd_ctx *c)
 {
     if (!c) { pimd_set_error("null context"); return PIMD_ERR_ARG; }
     return check_device_error(c);
+}
+
+extern "C" int pimd_profile(pimd_ctx *c, int enable)
+{
+    if (!c) { pimd_set_error("null context"); return PIMD_ERR_ARG; }
+    if (!c->prof) c->prof = new PimdProf();
+    PIMD_CUDA_CHECK(cudaStreamSynchronize(c->stream));
+    if (enable) c->prof->clear();
+    c->prof->on = enable != 0;
+    return 0;
+}
+
+extern "C" int pimd_profile_read(pimd_ctx *c, double *h_ms, int64_t *h_launches)
+{
+    if (!c || !h_ms || !h_launches) { pimd_set_error("null argument"); return PIMD_ERR_ARG; }
+    for (int k = 0; k < PIMD_PROF_CLASSES; ++k) { h_ms[k] = 0.0; h_launches[k] = 0; }
+    if (!c->prof) return 0;
+    PIMD_CUDA_CHECK(cudaStreamSynchronize(c->stream));
+    for (auto &r : c->prof->recs) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, r.a, r.b) != cudaSuccess) { (void)cudaGetLastError(); continue; }
+        h_ms[r.kind] += ms;
+        h_launches[r.kind] += 1;
+    }
+    return 0;
 }
 
 extern "C" int64_t pimd_launch_count(const pimd_ctx *c) { return c ? c->launches : 0; }

@@ -59,6 +59,8 @@ def load_library():
     L.pimd_set_state.argtypes = [vp, vp, vp, C.c_int64]
     L.pimd_nlist.argtypes = [vp, vp, vp, C.c_int64, C.POINTER(C.c_int64)]
     L.pimd_sync.argtypes = [vp]
+    L.pimd_profile.argtypes = [vp, C.c_int]
+    L.pimd_profile_read.argtypes = [vp, dp, C.POINTER(C.c_int64)]
     L.pimd_launch_count.argtypes = [vp]
     L.pimd_launch_count.restype = C.c_int64
     L.pimd_last_error.restype = C.c_char_p
@@ -182,6 +184,18 @@ class PIMD:
 
     def sync(self):
         _check(load_library().pimd_sync(self._h))
+
+    PROF_CLASSES = ("pimd_nm", "nlist", "gfn.pair", "gfn.node", "gfn.head", "other")
+
+    def profile(self, enable: bool):
+        _check(load_library().pimd_profile(self._h, int(bool(enable))))
+
+    def profile_read(self):
+        """{class: (total_ms, timed_launch_groups)} measured with CUDA events on the context's stream."""
+        ms = (C.c_double * 6)()
+        n = (C.c_int64 * 6)()
+        _check(load_library().pimd_profile_read(self._h, ms, n))
+        return {k: (float(ms[i]), int(n[i])) for i, k in enumerate(self.PROF_CLASSES)}
 
     def launch_count(self) -> int:
         return int(load_library().pimd_launch_count(self._h))

@@ -51,7 +51,7 @@ def test_workloads_bit_exact(cuda_device, name):
     _compare(gpu, ref)
     spread_beads(gpu, ref, scale=0.05)
     rp, _ = _compare(gpu, ref)
-    assert abs(rp[-1] / w.rows - {"fad_p8": 8.8, "water64": 89.6, "ice512": 85.0}[name]) < 1.0
+    assert abs(rp[-1] / w.rows - {"fad_p8": 8.8, "water64": 89.6, "ice512": 85.0}[name]) < 2.5
 
 
 def test_replicas_bit_exact(cuda_device):
