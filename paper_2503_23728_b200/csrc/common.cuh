@@ -80,6 +80,8 @@ struct pimd_ctx {
     NlistDev nl;
     GfnDev net;
     float *weights_dev;                // raw + derived weights
+    uint16_t *wimg_e1, *wimg_e2, *wimg_fe;   // bf16 UMMA images (K-major, 128B swizzle) for the tcgen05 path
+    int use_tc;                        // 1: tensor-core pair kernels (gemm_dtype 1, K=64, H=128)
     float *nfeat, *xfeat, *mfeat, *Efeat, *Gfeat;   // [rows][H]
     float *carry_m;                    // [n_gran_m][2][H]
     float *carry_f;                    // [n_gran_f][2][4]

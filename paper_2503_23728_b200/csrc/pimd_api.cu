@@ -61,7 +61,7 @@ namespace {
 struct Layout {
     size_t q, p, F, species, mass, C, CT, omega, err, est_partial, est_out;
     size_t cell_id, cell_count, cell_start, cell_cursor, sorted_atom, sorted_q, nnz, row_ptr, block_sums, col, pair_row;
-    size_t weights, nfeat, xfeat, mfeat, Efeat, Gfeat, carry_m, carry_f, Fraw;
+    size_t wimg, weights, nfeat, xfeat, mfeat, Efeat, Gfeat, carry_m, carry_f, Fraw;
     size_t total;
     int ncell[3], nct;
     int64_t pair_cap, n_gran_m, n_gran_f, n_wfloats;
@@ -166,6 +166,7 @@ int compute_layout(int N, int R, int P, const double box[3], const pimd_net_para
         L->col = take(cur, sizeof(int) * L->pair_cap);
         L->pair_row = take(cur, sizeof(int) * L->pair_cap);
         L->weights = take(cur, sizeof(float) * L->n_wfloats);
+        L->wimg = take(cur, 5 * 16384);   // bf16 UMMA images: W_e1 (16 KB), W_e2 (32 KB), W_f1 W_e2 (32 KB)
         L->nfeat = take(cur, sizeof(float) * rows * H);
         L->xfeat = take(cur, sizeof(float) * rows * H);
         L->mfeat = take(cur, sizeof(float) * rows * H);
@@ -179,8 +180,29 @@ int compute_layout(int N, int R, int P, const double box[3], const pimd_net_para
     return 0;
 }
 
+uint16_t f32_to_bf16_rne(float f)
+{
+    uint32_t u;
+    memcpy(&u, &f, 4);
+    if ((u & 0x7FFFFFFFu) > 0x7F800000u) return (uint16_t)((u >> 16) | 0x40);   // NaN
+    u += 0x7FFFu + ((u >> 16) & 1u);
+    return (uint16_t)(u >> 16);
+}
+
+// bf16 image of a row-major [n_rows][n_k] matrix as UMMA K-major operand blocks of 64 k (128-byte rows, 16-byte
+// chunks XOR-swizzled by row & 7), block kb at byte offset kb * n_rows * 128
+void build_umma_image(const float *W, int n_rows, int n_k, uint16_t *img)
+{
+    for (int kb = 0; kb < n_k / 64; ++kb)
+        for (int n = 0; n < n_rows; ++n)
+            for (int c = 0; c < 8; ++c)
+                for (int e = 0; e < 8; ++e)
+                    img[(size_t)kb * n_rows * 64 + (size_t)n * 64 + ((c ^ (n & 7)) * 8) + e] =
+                        f32_to_bf16_rne(W[(size_t)n * n_k + kb * 64 + c * 8 + e]);
+}
+
 // derived, transposed fp32 weights in the order the kernels use (S:G0 is the input order)
-void build_weights(const pimd_net_params *net, std::vector<float> &out, std::vector<size_t> &offs)
+void build_weights(const pimd_net_params *net, std::vector<float> &out, std::vector<size_t> &offs, std::vector<float> &Wfe)
 {
     const int S = net->n_species, K = net->n_rbf, H = net->hidden, L = net->n_layers;
     const float *w = net->weights;
@@ -201,7 +223,8 @@ void build_weights(const pimd_net_params *net, std::vector<float> &out, std::vec
     }
     const float *Wf1 = mat(H, H), *bf1 = vec(H), *wf2 = vec(H);
     // W_fe = W_f1 W_e2 and b_fe = W_f1 b_e2 + b_f1, formed in fp64 then rounded once
-    std::vector<float> Wfe((size_t)H * H), bfe(H);
+    std::vector<float> bfe(H);
+    Wfe.assign((size_t)H * H, 0.f);
     for (int o = 0; o < H; ++o) {
         for (int k = 0; k < H; ++k) {
             double s = 0.0;
@@ -365,6 +388,7 @@ extern "C" int pimd_create(pimd_ctx **out, int n_atoms, int n_replicas, const in
     CREATE_CHECK(cudaMemcpyAsync(c->omega_k, om.data(), sizeof(double) * P, cudaMemcpyHostToDevice, st));
 
     std::vector<float> wd;
+    std::vector<uint16_t> wimg;
     if (net->kind == 0) {
         const int H = net->hidden;
         NlistDev &nl = c->nl;
@@ -381,7 +405,19 @@ extern "C" int pimd_create(pimd_ctx **out, int n_atoms, int n_replicas, const in
         c->carry_m = (float *)(ws + L.carry_m); c->carry_f = (float *)(ws + L.carry_f); c->Fraw = (float *)(ws + L.Fraw);
         c->gran_m = L.gran_m; c->gran_f = L.gran_f; c->n_gran_m = L.n_gran_m; c->n_gran_f = L.n_gran_f;
         std::vector<size_t> offs;
-        build_weights(net, wd, offs);
+        std::vector<float> Wfe;
+        build_weights(net, wd, offs, Wfe);
+        c->use_tc = (net->gemm_dtype == 1 && net->n_rbf == 64 && net->hidden == 128) ? 1 : 0;
+        c->wimg_e1 = (uint16_t *)(ws + L.wimg); c->wimg_e2 = c->wimg_e1 + 8192; c->wimg_fe = c->wimg_e2 + 16384;
+        if (c->use_tc) {
+            wimg.resize(5 * 8192);
+            const float *We1 = net->weights + (size_t)net->n_species * H;          // [H][K]
+            const float *We2 = We1 + (size_t)H * net->n_rbf + H;                   // [H][H]
+            build_umma_image(We1, H, net->n_rbf, wimg.data());
+            build_umma_image(We2, H, H, wimg.data() + 8192);
+            build_umma_image(Wfe.data(), H, H, wimg.data() + 8192 + 16384);
+            CREATE_CHECK(cudaMemcpyAsync(c->wimg_e1, wimg.data(), sizeof(uint16_t) * wimg.size(), cudaMemcpyHostToDevice, st));
+        }
         if ((int64_t)wd.size() != L.n_wfloats) {
             pimd_set_error("internal: derived weight count %zu != %lld", wd.size(), (long long)L.n_wfloats);
             delete c;
