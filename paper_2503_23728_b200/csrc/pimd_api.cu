@@ -191,14 +191,14 @@ uint16_t f32_to_bf16_rne(float f)
 
 // bf16 image of a row-major [n_rows][n_k] matrix as UMMA K-major operand blocks of 64 k (128-byte rows, 16-byte
 // chunks XOR-swizzled by row & 7), block kb at byte offset kb * n_rows * 128
-void build_umma_image(const float *W, int n_rows, int n_k, uint16_t *img)
+void build_umma_image(const float *W, int n_rows, int n_k, float scale, uint16_t *img)
 {
     for (int kb = 0; kb < n_k / 64; ++kb)
         for (int n = 0; n < n_rows; ++n)
             for (int c = 0; c < 8; ++c)
                 for (int e = 0; e < 8; ++e)
                     img[(size_t)kb * n_rows * 64 + (size_t)n * 64 + ((c ^ (n & 7)) * 8) + e] =
-                        f32_to_bf16_rne(W[(size_t)n * n_k + kb * 64 + c * 8 + e]);
+                        f32_to_bf16_rne(scale * W[(size_t)n * n_k + kb * 64 + c * 8 + e]);
 }
 
 // derived, transposed fp32 weights in the order the kernels use (S:G0 is the input order)
@@ -413,9 +413,9 @@ extern "C" int pimd_create(pimd_ctx **out, int n_atoms, int n_replicas, const in
             wimg.resize(5 * 8192);
             const float *We1 = net->weights + (size_t)net->n_species * H;          // [H][K]
             const float *We2 = We1 + (size_t)H * net->n_rbf + H;                   // [H][H]
-            build_umma_image(We1, H, net->n_rbf, wimg.data());
-            build_umma_image(We2, H, H, wimg.data() + 8192);
-            build_umma_image(Wfe.data(), H, H, wimg.data() + 8192 + 16384);
+            build_umma_image(We1, H, net->n_rbf, 0.5f, wimg.data());   // SiLU(x) = h tanh(h) + h, h = x/2
+            build_umma_image(We2, H, H, 1.0f, wimg.data() + 8192);
+            build_umma_image(Wfe.data(), H, H, 0.5f, wimg.data() + 8192 + 16384);
             CREATE_CHECK(cudaMemcpyAsync(c->wimg_e1, wimg.data(), sizeof(uint16_t) * wimg.size(), cudaMemcpyHostToDevice, st));
         }
         if ((int64_t)wd.size() != L.n_wfloats) {
