@@ -47,6 +47,8 @@ struct NlistDev {
     int *sorted_atom;                  // [rows] local atom index in cell order
     double *sorted_q;                  // [rows][3]
     int *nnz;                          // [rows]
+    int *hits;                         // [rows][hit_stride] unsorted neighbour indices of each row
+    int hit_stride;
     int *row_ptr;                      // [rows+1]
     int *block_sums;                   // [ceil(rows/1024)+1]
     int *col;                          // [pair_cap] local atom index j

@@ -1,8 +1,9 @@
 // nlist_kernels.cu -- per-bead-system periodic cell list -> CSR pair list (rows a1-a3 of SURVEY 8(a)).
 //
 // bin (wrapped fraction -> cell) -> counting sort (histogram, per-system exclusive scan, scatter of
-// atom index + fp64 position into cell order) -> warp-per-row stencil scan, twice: count, then fill
-// with an in-shared-memory rank sort so that every CSR row lists j ascending.  The inclusion test is
+// atom index + fp64 position into cell order) -> warp-per-row stencil scan that counts the hits and
+// parks them in a fixed-stride scratch row -> row_ptr scan -> fill with an in-shared-memory rank sort
+// so that every CSR row lists j ascending.  The inclusion test is
 // the fp64 sequence of S:L3 written with explicit round-to-nearest intrinsics (no FMA contraction), so
 // the list is bit-identical to the oracle's.  Integer atomics only order the scatter inside a cell;
 // the sorted rows make the CSR deterministic.
@@ -15,7 +16,9 @@ struct NlArgs {
     int64_t rows;
     double box[3];
     double rc2;
-    int nc[3], nct;
+    float rc2_lo, rc2_hi;          // fp32 pre-filter band around r_c^2 (exact fp64 test inside the band)
+    float boxf[3], inv_boxf[3];
+    int nc[3], nct, hit_stride;
     const double *q;
     NlistDev d;
     int *err;
@@ -121,10 +124,28 @@ __device__ __forceinline__ bool within_cutoff(const double qi[3], const double *
     return d2 < a.rc2;
 }
 
+// Same decision as within_cutoff, but most candidates are settled by an fp32 estimate of d^2: it differs from the
+// exact value by a relative error far below the 1e-3 band (fp64 difference rounded once to fp32; the image shift may
+// differ from the exact one only when |dx| ~ L/2 >= r_c, which lands outside the band or inside it, never on the
+// wrong side).  Only candidates inside the band evaluate the exact S:L3 sequence, so the list stays bit-exact.
+__device__ __forceinline__ bool within_cutoff_fast(const double qi[3], const double *__restrict__ qj, const NlArgs &a)
+{
+    float d2 = 0.f;
+#pragma unroll
+    for (int ax = 0; ax < 3; ++ax) {
+        float dx = (float)(qj[ax] - qi[ax]);
+        if (a.periodic) dx = fmaf(-a.boxf[ax], rintf(dx * a.inv_boxf[ax]), dx);
+        d2 = fmaf(dx, dx, d2);
+    }
+    if (d2 > a.rc2_hi) return false;
+    if (d2 < a.rc2_lo) return true;
+    return within_cutoff(qi, qj, a);
+}
+
 // Walks the de-duplicated 3x3x3 stencil of `row` with one warp.  FILL = false: returns the hit count.
 // FILL = true: also stores the hit atom indices in buf (capacity PIMD_MAX_NBR), unsorted.
 template <bool FILL>
-__device__ __forceinline__ int stencil_scan(const NlArgs &a, int64_t row, int *buf)
+__device__ __forceinline__ int stencil_scan(const NlArgs &a, int64_t row, int *buf, int cap)
 {
     const int lane = threadIdx.x & 31;
     const int sys = (int)(row / a.N), i = (int)(row - (int64_t)sys * a.N);
@@ -158,12 +179,12 @@ __device__ __forceinline__ int stencil_scan(const NlArgs &a, int64_t row, int *b
                     int j = -1;
                     if (s < s1) {
                         j = a.d.sorted_atom[sbase + s];
-                        hit = (j != i) && within_cutoff(qi, a.d.sorted_q + (sbase + s) * 3, a);
+                        hit = (j != i) && within_cutoff_fast(qi, a.d.sorted_q + (sbase + s) * 3, a);
                     }
                     unsigned m = __ballot_sync(0xffffffffu, hit);
                     if (FILL && hit) {
                         int idx = total + __popc(m & ((1u << lane) - 1u));
-                        if (idx < PIMD_MAX_NBR) buf[idx] = j;
+                        if (idx < cap) buf[idx] = j;
                     }
                     total += __popc(m);
                 }
@@ -175,8 +196,11 @@ __global__ void __launch_bounds__(256) count_kernel(NlArgs a)
 {
     int64_t row = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
     if (row >= a.rows) return;
-    int n = stencil_scan<false>(a, row, nullptr);
-    if ((threadIdx.x & 31) == 0) a.d.nnz[row] = n;
+    int n = stencil_scan<true>(a, row, a.d.hits + row * a.hit_stride, a.hit_stride);
+    if ((threadIdx.x & 31) == 0) {
+        if (n > a.hit_stride) { atomicOr(a.err, PIMD_FLAG_PAIRS); n = a.hit_stride; }
+        a.d.nnz[row] = n;
+    }
 }
 
 // row_ptr: three-kernel exclusive scan over rows (1024 rows per block)
@@ -225,12 +249,10 @@ __global__ void __launch_bounds__(256) fill_kernel(NlArgs a)
     if (row >= a.rows) return;
     if (a.d.row_ptr[a.rows] == 0) return;   // empty or overflowed list
     int *buf = sbuf[w];
-    int n = stencil_scan<true>(a, row, buf);
+    const int n = a.d.nnz[row];
+    const int *hits = a.d.hits + row * a.hit_stride;
+    for (int e = lane; e < n; e += 32) buf[e] = hits[e];
     __syncwarp();
-    if (n > PIMD_MAX_NBR) {
-        if (lane == 0) atomicOr(a.err, PIMD_FLAG_PAIRS);
-        n = PIMD_MAX_NBR;
-    }
     const int64_t base = a.d.row_ptr[row];
     for (int e = lane; e < n; e += 32) {   // rank sort: j values in a row are distinct (box >= 2 r_c)
         int v = buf[e], rank = 0;
@@ -249,6 +271,9 @@ int pimd_launch_nlist(pimd_ctx *c)
     for (int k = 0; k < 3; ++k) { a.box[k] = c->box[k]; a.nc[k] = c->nl.ncell[k]; }
     a.rc2 = (double)c->net.r_cut * (double)c->net.r_cut;
     a.nct = c->nl.ncell_tot; a.q = c->q; a.d = c->nl; a.err = c->err;
+    a.rc2_lo = (float)(a.rc2 * (1.0 - 1e-3)); a.rc2_hi = (float)(a.rc2 * (1.0 + 1e-3));
+    for (int k = 0; k < 3; ++k) { a.boxf[k] = (float)c->box[k]; a.inv_boxf[k] = c->periodic ? (float)(1.0 / c->box[k]) : 0.f; }
+    a.hit_stride = c->nl.hit_stride;
     const int64_t rows = c->rows;
     const unsigned gthr = (unsigned)((rows + 255) / 256), gwarp = (unsigned)((rows + 7) / 8);
     const int nblk = (int)((rows + 1023) / 1024);

@@ -60,12 +60,12 @@ namespace {
 
 struct Layout {
     size_t q, p, F, species, mass, C, CT, omega, err, est_partial, est_out;
-    size_t cell_id, cell_count, cell_start, cell_cursor, sorted_atom, sorted_q, nnz, row_ptr, block_sums, col, pair_row;
+    size_t cell_id, cell_count, cell_start, cell_cursor, sorted_atom, sorted_q, nnz, hits, row_ptr, block_sums, col, pair_row;
     size_t wimg, weights, nfeat, xfeat, mfeat, Efeat, Gfeat, carry_m, carry_f, Fraw;
     size_t total;
     int ncell[3], nct;
     int64_t pair_cap, n_gran_m, n_gran_f, n_wfloats;
-    int gran_m, gran_f;
+    int gran_m, gran_f, hit_stride;
 };
 
 size_t take(size_t &cur, size_t bytes)
@@ -161,6 +161,8 @@ int compute_layout(int N, int R, int P, const double box[3], const pimd_net_para
         L->sorted_atom = take(cur, sizeof(int) * rows);
         L->sorted_q = take(cur, sizeof(double) * rows * 3);
         L->nnz = take(cur, sizeof(int) * rows);
+        L->hit_stride = (N - 1 < PIMD_MAX_NBR) ? (N > 1 ? N - 1 : 1) : PIMD_MAX_NBR;
+        L->hits = take(cur, sizeof(int) * rows * L->hit_stride);
         L->row_ptr = take(cur, sizeof(int) * (rows + 1));
         L->block_sums = take(cur, sizeof(int) * ((rows + 1023) / 1024 + 1));
         L->col = take(cur, sizeof(int) * L->pair_cap);
@@ -397,7 +399,7 @@ extern "C" int pimd_create(pimd_ctx **out, int n_atoms, int n_replicas, const in
         nl.cell_id = (int *)(ws + L.cell_id); nl.cell_count = (int *)(ws + L.cell_count);
         nl.cell_start = (int *)(ws + L.cell_start); nl.cell_cursor = (int *)(ws + L.cell_cursor);
         nl.sorted_atom = (int *)(ws + L.sorted_atom); nl.sorted_q = (double *)(ws + L.sorted_q);
-        nl.nnz = (int *)(ws + L.nnz); nl.row_ptr = (int *)(ws + L.row_ptr); nl.block_sums = (int *)(ws + L.block_sums);
+        nl.nnz = (int *)(ws + L.nnz); nl.hits = (int *)(ws + L.hits); nl.hit_stride = L.hit_stride; nl.row_ptr = (int *)(ws + L.row_ptr); nl.block_sums = (int *)(ws + L.block_sums);
         nl.col = (int *)(ws + L.col); nl.pair_row = (int *)(ws + L.pair_row); nl.pair_cap = L.pair_cap;
         c->weights_dev = (float *)(ws + L.weights);
         c->nfeat = (float *)(ws + L.nfeat); c->xfeat = (float *)(ws + L.xfeat); c->mfeat = (float *)(ws + L.mfeat);

@@ -40,6 +40,28 @@ def test_small_systems_with_biases(cuda_device, K, H, L):
         assert np.abs(Fg.sum(axis=2)).max() < 1e-4  # momentum conservation per bead-system
 
 
+@pytest.mark.parametrize("L", [0, 1, 3])
+def test_small_systems_tensor_core_path(cuda_device, L):
+    """gemm_dtype = 1 (bf16 operands on tcgen05, fp32 accumulate): ragged tiles, biases, empty rows; 2e-2."""
+    rng = np.random.default_rng(10 + L)
+    for box, n_at, P in [(np.zeros(3), 23, 3), (np.array([6.5, 7.0, 9.2]), 77, 2), (np.array([12.5, 13.0, 12.2]), 700, 1)]:
+        x = rng.uniform(0, 1, (2, n_at, 3)) * (box if box[0] > 0 else 4.5)
+        if box[0] == 0:
+            x[:, 5] += 100.0  # an atom with no neighbours
+        sp = rng.integers(0, 3, n_at).astype(np.int32)
+        spec = _biased_spec(64, 128, L, 3.0, 1.0 / 12.0, 0.2)
+        spec.gemm_dtype = 1
+        gpu, ref = make_pair(sp, x, box, P, 300.0, 0.25, 1.0, 0, spec)
+        spread_beads(gpu, ref, scale=0.05)
+        Fg, Fr = _forces_pair(gpu, ref)
+        scale = np.sqrt((Fr ** 2).sum(-1).mean())
+        err = np.abs(Fg - Fr).max()
+        assert err <= RTOL16 * max(scale, np.abs(Fr).max()), (L, n_at, err, scale)
+        assert np.sqrt(((Fg - Fr) ** 2).sum(-1).mean()) <= 0.5 * RTOL16 * scale  # rms error well inside the bound
+        if box[0] == 0:
+            assert np.all(Fg[:, :, 5] == 0.0)
+
+
 @pytest.mark.parametrize("name", ["fad_p8", "fad_x64_p32", "water64"])
 def test_fp32_workload_forces(cuda_device, name):
     w = pi.make_workload(name)
