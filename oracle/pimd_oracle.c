@@ -70,6 +70,7 @@ typedef struct {
     double **Ws, **Wvn, **Wvm, **bv1, **Wv2, **bv2, **Wa, **ba;
     double *Wf1, *bf1, *wf2, bf2;
     double *q, *p, *F; /* [R][P][N][3] */
+    double *Fgross;    /* [R][P][N] diagnostic: sum of the magnitudes of the terms of F_i */
     double *C;         /* [P][P], C[j*P+k], bead j, mode k */
     double *omega_k;   /* [P] */
     int forces_valid;
@@ -264,7 +265,11 @@ static void affine(const double *Wt, const double *b, const double *x, int n_in,
 static int g_inner_parallel = 0;
 
 /* forces on one bead-system from its pair list; F[N][3] in eV/A */
-static void gfn_forces_system(const ref_ctx *c, const double *q, const int32_t *row_ptr, const int32_t *col, double *F)
+/* gross (may be NULL): per atom, force_scale * sum_j c_ij (sum_o |w_f2[o] SiLU(t_o)| + |b_f2|): the sum of the magnitudes
+ * of every term that is added up into F_i (readout channels, then neighbours).  A diagnostic only -- the scale a
+ * forward error bound of those sums is stated against; F does not depend on it. */
+static void gfn_forces_system(const ref_ctx *c, const double *q, const int32_t *row_ptr, const int32_t *col, double *F,
+                              double *gross)
 {
     const int N = c->N, H = c->net.hidden, K = c->net.n_rbf, L = c->net.n_layers;
     const double rc = c->net.r_cut;
@@ -341,15 +346,21 @@ static void gfn_forces_system(const ref_ctx *c, const double *q, const int32_t *
     /* G4: F_ij = c_ij * d_ij * phi_f(e_ij), F_i = force_scale * sum_j F_ij */
 #pragma omp parallel for schedule(static) if (g_inner_parallel)
     for (int i = 0; i < N; ++i) {
-        double f[3] = {0.0, 0.0, 0.0}, t[512];
+        double f[3] = {0.0, 0.0, 0.0}, t[512], fg = 0.0;
         for (int p = row_ptr[i]; p < row_ptr[i + 1]; ++p) {
             affine(c->Wf1, c->bf1, e + (size_t)p * H, H, H, t);
-            double s = 0.0;
-            for (int o = 0; o < H; ++o) s += c->wf2[o] * silu(t[o]);
+            double s = 0.0, sa = 0.0;
+            for (int o = 0; o < H; ++o) {
+                double term = c->wf2[o] * silu(t[o]);
+                s += term;
+                sa += fabs(term);
+            }
             s += c->bf2;
             for (int ax = 0; ax < 3; ++ax) f[ax] += cw[p] * s * uv[3 * p + ax];
+            fg += cw[p] * (sa + fabs(c->bf2));
         }
         for (int ax = 0; ax < 3; ++ax) F[3 * i + ax] = c->net.force_scale * f[ax];
+        if (gross) gross[i] = fabs(c->net.force_scale) * fg;
     }
     free(n); free(x); free(m); free(a); free(e); free(cw); free(uv); free(pi_row);
 }
@@ -395,7 +406,7 @@ static int compute_forces(ref_ctx *c)
 #pragma omp atomic write
                 overflow = 1;
             } else {
-                gfn_forces_system(c, qs, rp, cl, c->F + (size_t)s * N * 3);
+                gfn_forces_system(c, qs, rp, cl, c->F + (size_t)s * N * 3, c->Fgross ? c->Fgross + (size_t)s * N : NULL);
             }
             free(rp); free(cl);
         }
@@ -590,6 +601,7 @@ int ref_create(ref_ctx **out, int n_atoms, int n_replicas, const int32_t *specie
     c->q = (double *)malloc(sizeof(double) * n);
     c->p = (double *)malloc(sizeof(double) * n);
     c->F = (double *)calloc(n, sizeof(double));
+    c->Fgross = (double *)calloc(n / 3 + 1, sizeof(double));
     c->C = (double *)malloc(sizeof(double) * (size_t)P * P);
     c->omega_k = (double *)malloc(sizeof(double) * P);
     ref_nm_matrix(P, c->C);
@@ -620,7 +632,7 @@ int ref_create(ref_ctx **out, int n_atoms, int n_replicas, const int32_t *specie
 void ref_destroy(ref_ctx *c)
 {
     if (!c) return;
-    free(c->species); free(c->mass); free(c->q); free(c->p); free(c->F); free(c->C); free(c->omega_k);
+    free(c->species); free(c->mass); free(c->q); free(c->p); free(c->F); free(c->Fgross); free(c->C); free(c->omega_k);
     if (c->net.kind == 0) {
         free(c->Emb); free(c->We1); free(c->be1); free(c->We2); free(c->be2);
         for (int l = 0; l < c->net.n_layers; ++l) {
@@ -639,6 +651,15 @@ int ref_forces(ref_ctx *c, double *out)
     int rc = compute_forces(c);
     if (rc) return rc;
     memcpy(out, c->F, sizeof(double) * (size_t)c->R * c->P * c->N * 3);
+    return 0;
+}
+
+int ref_force_gross(ref_ctx *c, double *out)
+{ /* [R][P][N]: sum of the magnitudes of the terms of F_i at the current q (diagnostic scale for error bounds; kind 0) */
+    if (!c || !out || c->net.kind != 0) return -1;
+    int rc = compute_forces(c);
+    if (rc) return rc;
+    memcpy(out, c->Fgross, sizeof(double) * (size_t)c->R * c->P * c->N);
     return 0;
 }
 

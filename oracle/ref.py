@@ -53,6 +53,7 @@ def lib():
         L.ref_destroy.restype = None
         L.ref_step.argtypes = [C.c_void_p, C.c_int]
         L.ref_forces.argtypes = [C.c_void_p, dp]
+        L.ref_force_gross.argtypes = [C.c_void_p, dp]
         L.ref_get_state.argtypes = [C.c_void_p, dp, dp, C.POINTER(C.c_int64)]
         L.ref_set_state.argtypes = [C.c_void_p, dp, dp, C.c_int64]
         L.ref_nlist.argtypes = [C.c_void_p, ip, ip, C.c_int64, C.POINTER(C.c_int64), C.c_int]
@@ -191,6 +192,15 @@ class RefPIMD:
         rc = lib().ref_forces(self._h, _dp(out))
         if rc != 0:
             raise RuntimeError(f"ref_forces failed: {rc}")
+        return out
+
+    def force_gross(self):
+        """[R][P][N]: force_scale * sum_j c_ij (sum_o |w_f2[o] SiLU(t_o)| + |b_f2|), the sum of the magnitudes of all
+        terms added up into F_i -- the scale forward error bounds of F_i are stated against."""
+        out = np.zeros(self.shape[:3])
+        rc = lib().ref_force_gross(self._h, _dp(out))
+        if rc != 0:
+            raise RuntimeError(f"ref_force_gross failed: {rc}")
         return out
 
     def get_state(self):

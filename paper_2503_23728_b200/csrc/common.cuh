@@ -83,7 +83,10 @@ struct pimd_ctx {
     GfnDev net;
     float *weights_dev;                // raw + derived weights
     uint16_t *wimg_e1, *wimg_e2, *wimg_fe;   // bf16 UMMA images (K-major, 128B swizzle) for the tcgen05 path
-    int use_tc;                        // 1: tensor-core pair kernels (gemm_dtype 1, K=64, H=128)
+    int use_tc;                        // 1: tensor-core pair and node kernels (gemm_dtype 1, K=64, H=128)
+    uint16_t *wimg_node;               // [L][5] bf16 UMMA images: W_vn/2, W_vm/2, W_v2, W_a, W_s^{l+1} (or W_f1)
+    float *xs0;                        // [S][H] W_s^0 Emb[s]
+    uint32_t *XE;                      // [rows][H] packed bf16 (x | E << 16) gathered by the pair kernels (aliases xfeat)
     float *nfeat, *xfeat, *mfeat, *Efeat, *Gfeat;   // [rows][H]
     float *carry_m;                    // [n_gran_m][2][H]
     float *carry_f;                    // [n_gran_f][2][4]

@@ -205,8 +205,13 @@ int launch_node_t(pimd_ctx *c, const NodeArgs &a)
     return 0;
 }
 
+}  // namespace gfn
+namespace node_tc { int launch_node_tc(pimd_ctx *c, int mode, int layer); }
+namespace gfn {
+
 int launch_node(pimd_ctx *c, int mode, int layer)
 {
+    if (c->use_tc) return node_tc::launch_node_tc(c, mode, layer);
     const GfnDev &n = c->net;
     NodeArgs a;
     a.N = c->N; a.mode = mode; a.rows = c->rows; a.species = c->species; a.row_ptr = c->nl.row_ptr;

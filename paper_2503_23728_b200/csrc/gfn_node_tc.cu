@@ -1,0 +1,318 @@
+// gfn_node_tc.cu -- atom-wise dense layers of the GFN force net on the 5th-gen tensor cores
+// (rows a4, a6 of SURVEY 8(a); P:L74 phi_v and the node->edge MLP of P:L76), bf16 operands with fp32
+// accumulation in TMEM.  Used when gemm_dtype == 1 and H == 128 (BASELINE configs[3..4]).
+//
+// One persistent CTA per SM keeps the five H x H weight matrices of the layer resident in shared memory
+// as pre-swizzled bf16 UMMA operands (5 x 32 KB, one TMA bulk copy each) and walks 128-row tiles:
+//   h   = SiLU(W_vn n + W_vm m + b_v1)      one K = 256 accumulation chain, m assembled from the carry slots
+//   n  += W_v2 h + b_v2                     fp32 residual stream in HBM, bf16 copy as the next operand
+//   E  += W_a n + b_a                       running sum of the edge updates (S:G5), fp32 master in HBM
+//   x   = W_s^{l+1} n                       or, after the last layer,  G = W_f1 E
+// The pair kernels gather x_j, E_j per directed pair in the message passes: that copy is written as packed bf16
+// (XE[row][c] = x | E << 16) so that one 32-bit load serves both and the L2 gather traffic halves.  G stays fp32:
+// G_i + G_j enters the force readout directly, with no averaging over neighbours behind it.
+// SiLU(x) = h tanh(h) + h with h = x/2: the 1/2 is folded (exactly) into the W_vn, W_vm images and b_v1.
+#include "common.cuh"
+#include "tc_ptx.cuh"
+
+namespace node_tc {
+
+constexpr int TR = 128;            // rows per tile
+constexpr int H = 128;
+constexpr int NTH = 512;
+constexpr int OPB = TR * H * 2;    // bytes of one bf16 operand tile / weight image
+constexpr int NW = 5;              // resident weight images: W_vn/2, W_vm/2, W_v2, W_a, W_next
+
+struct Args {
+    int64_t rows;
+    int N, last, gran_m, n_tiles;
+    const int *row_ptr;
+    const uint16_t *Wimg;
+    const float *bv1, *bv2, *ba;
+    float *n, *E;
+    const float *m, *carry_m;
+    uint32_t *XE;
+    float *G;
+};
+
+constexpr int OFF_W = 0, OFF_A0 = NW * OPB, OFF_A1 = OFF_A0 + OPB, OFF_B = OFF_A1 + OPB, OFF_BAR = OFF_B + 3 * H * 4,
+              SMEM_BYTES = OFF_BAR + 32;
+
+// byte offset of element (row r, k) in a K-major [128][128] bf16 operand: two k-blocks of [128][64] (128-byte rows),
+// 16-byte chunks XOR-swizzled by r & 7
+__device__ __forceinline__ int op_off(int r, int k)
+{
+    return (k >> 6) * (TR * 128) + r * 128 + ((((k & 63) >> 3) ^ (r & 7)) << 4) + (k & 7) * 2;
+}
+
+__device__ __forceinline__ float4 assemble_m(const Args &a, int64_t row, int c0, int n_pairs)
+{
+    const int rs = a.row_ptr[row], re = a.row_ptr[row + 1];
+    float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (re <= rs || n_pairs == 0) return v;
+    const int g0 = rs / a.gran_m, g1 = (re - 1) / a.gran_m;
+    if (g0 == g1) return __ldg((const float4 *)(a.m + (size_t)row * H + c0));
+    v = __ldg((const float4 *)(a.carry_m + ((size_t)g0 * 2 + 1) * H + c0));
+    for (int g = g0 + 1; g <= g1; ++g) {
+        float4 t = __ldg((const float4 *)(a.carry_m + ((size_t)g * 2 + 0) * H + c0));
+        v.x += t.x; v.y += t.y; v.z += t.z; v.w += t.w;
+    }
+    return v;
+}
+
+// D (+)= A . B^T over K = 128 (8 x UMMA 128x128x16); one thread
+__device__ __forceinline__ void issue_gemm(uint32_t tmem_d, uint32_t sA, uint32_t sB, uint32_t idesc, bool accumulate)
+{
+#pragma unroll
+    for (int kk = 0; kk < H / 16; ++kk) {
+        const uint32_t off = (kk >> 2) * (TR * 128) + (kk & 3) * 32;
+        tc::mma_bf16_ss(tmem_d, tc::make_desc_sw128(sA + off), tc::make_desc_sw128(sB + off), idesc, (accumulate || kk > 0) ? 1u : 0u);
+    }
+}
+
+// 16 fp32 values of row r, columns [c0, c0 + 16) -> bf16 -> two swizzled 16-byte chunks of operand `A`
+__device__ __forceinline__ void store_operand16(unsigned char *A, int r, int c0, const float (&v)[16])
+{
+    uint32_t pk[8];
+#pragma unroll
+    for (int e = 0; e < 8; ++e) pk[e] = tc::pack_bf16(v[2 * e], v[2 * e + 1]);
+    unsigned char *base = A + (c0 >> 6) * (TR * 128) + r * 128;
+    const int ch = (c0 & 63) >> 3;
+    *(uint4 *)(base + ((ch ^ (r & 7)) << 4)) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+    *(uint4 *)(base + (((ch + 1) ^ (r & 7)) << 4)) = make_uint4(pk[4], pk[5], pk[6], pk[7]);
+}
+
+__global__ void __launch_bounds__(NTH, 1) node_tc_kernel(const __grid_constant__ Args a)
+{
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    unsigned char *S = smem_raw + ((1024u - (tc::smem_u32(smem_raw) & 1023u)) & 1023u);
+    unsigned char *Wm = S + OFF_W, *A0 = S + OFF_A0, *A1 = S + OFF_A1;
+    float *sb = (float *)(S + OFF_B);
+    uint64_t *mbar_w = (uint64_t *)(S + OFF_BAR), *mbar_mma = mbar_w + 1;
+    uint32_t *tmem_slot = (uint32_t *)(mbar_w + 2);
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int n_pairs = a.row_ptr[a.rows];
+
+    if (tid == 0) { tc::mbar_init(mbar_w, 1); tc::mbar_init(mbar_mma, 1); tc::fence_mbar_init(); }
+    if (warp == 1) tc::tmem_alloc(tmem_slot, 256);
+    for (int i = tid; i < H; i += NTH) { sb[i] = 0.5f * a.bv1[i]; sb[H + i] = a.bv2[i]; sb[2 * H + i] = a.ba[i]; }
+    tc::tc_fence_before_sync();
+    __syncthreads();
+    tc::tc_fence_after_sync();
+    if (tid == 0) {
+        tc::mbar_arrive_expect_tx(mbar_w, NW * OPB);
+        for (int w = 0; w < NW; ++w) tc::bulk_g2s(Wm + w * OPB, a.Wimg + (size_t)w * (OPB / 2), OPB, mbar_w);
+    }
+    const uint32_t tmem_d0 = *tmem_slot, tmem_d1 = tmem_d0 + 128;
+    const int q = warp & 3, g = warp >> 2;                 // TMEM lane quadrant; 32-column group
+    const int r = q * 32 + lane;                           // row of the tile = TMEM lane
+    const uint32_t lane_field = (uint32_t)(q * 32) << 16;
+    const uint32_t idesc = tc::make_idesc_bf16(TR, H);
+    const uint32_t sW = tc::smem_u32(Wm), sA0 = tc::smem_u32(A0), sA1 = tc::smem_u32(A1);
+    uint32_t par = 0;
+    bool w_ready = false;
+
+    for (int tile = blockIdx.x; tile < a.n_tiles; tile += gridDim.x) {
+        const int64_t row0 = (int64_t)tile * TR;
+        // ---- operands n, m (fp32 in HBM) -> bf16 swizzled tiles; one warp per row: coalesced 512-byte reads
+#pragma unroll 2
+        for (int it = 0; it < TR * H / 4 / NTH; ++it) {
+            const int idx = tid + it * NTH, rr = idx >> 5, k = (idx & 31) * 4;
+            const int64_t row = row0 + rr;
+            float4 nv = make_float4(0.f, 0.f, 0.f, 0.f), mv = nv;
+            if (row < a.rows) {
+                nv = *(const float4 *)(a.n + (size_t)row * H + k);
+                mv = assemble_m(a, row, k, n_pairs);
+            }
+            const int off = op_off(rr, k);
+            *(uint2 *)(A0 + off) = make_uint2(tc::pack_bf16(nv.x, nv.y), tc::pack_bf16(nv.z, nv.w));
+            *(uint2 *)(A1 + off) = make_uint2(tc::pack_bf16(mv.x, mv.y), tc::pack_bf16(mv.z, mv.w));
+        }
+        tc::fence_proxy_async_smem();
+        __syncthreads();
+        // ---- D0 = n (W_vn/2)^T + m (W_vm/2)^T
+        if (tid == 0) {
+            if (!w_ready) tc::mbar_wait(mbar_w, 0);
+            tc::tc_fence_after_sync();
+            issue_gemm(tmem_d0, sA0, sW + 0 * OPB, idesc, false);
+            issue_gemm(tmem_d0, sA1, sW + 1 * OPB, idesc, true);
+            tc::mma_commit(mbar_mma);
+        }
+        w_ready = true;
+        tc::mbar_wait(mbar_mma, par);
+        par ^= 1;
+        tc::tc_fence_after_sync();
+        // ---- h = SiLU(2 (D0 + b_v1/2)) -> A1
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+            const int c0 = g * 32 + j * 16;
+            float v[16];
+            tc::tmem_ld16(tmem_d0 + lane_field + c0, v);
+#pragma unroll
+            for (int e = 0; e < 16; ++e) {
+                const float hh = v[e] + sb[c0 + e];
+                v[e] = fmaf(hh, tc::tanh_approx(hh), hh);
+            }
+            store_operand16(A1, r, c0, v);
+        }
+        tc::tc_fence_before_sync();
+        tc::fence_proxy_async_smem();
+        __syncthreads();
+        // ---- D0 = h W_v2^T
+        if (tid == 0) {
+            tc::tc_fence_after_sync();
+            issue_gemm(tmem_d0, sA1, sW + 2 * OPB, idesc, false);
+            tc::mma_commit(mbar_mma);
+        }
+        tc::mbar_wait(mbar_mma, par);
+        par ^= 1;
+        tc::tc_fence_after_sync();
+        // ---- n <- n + D0 + b_v2  (fp32 master in HBM; bf16 copy -> A0)
+        const int64_t row = row0 + r;
+        const bool valid = row < a.rows;
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+            const int c0 = g * 32 + j * 16;
+            float v[16], nn[16];
+            tc::tmem_ld16(tmem_d0 + lane_field + c0, v);
+#pragma unroll
+            for (int e4 = 0; e4 < 4; ++e4) {
+                float4 t = valid ? *(const float4 *)(a.n + (size_t)row * H + c0 + e4 * 4) : make_float4(0.f, 0.f, 0.f, 0.f);
+                nn[e4 * 4 + 0] = t.x; nn[e4 * 4 + 1] = t.y; nn[e4 * 4 + 2] = t.z; nn[e4 * 4 + 3] = t.w;
+            }
+#pragma unroll
+            for (int e = 0; e < 16; ++e) nn[e] = nn[e] + (v[e] + sb[H + c0 + e]);
+            if (valid)
+#pragma unroll
+                for (int e4 = 0; e4 < 4; ++e4)
+                    *(float4 *)(a.n + (size_t)row * H + c0 + e4 * 4) =
+                        make_float4(nn[e4 * 4], nn[e4 * 4 + 1], nn[e4 * 4 + 2], nn[e4 * 4 + 3]);
+            store_operand16(A0, r, c0, nn);
+        }
+        tc::tc_fence_before_sync();
+        tc::fence_proxy_async_smem();
+        __syncthreads();
+        // ---- D0 = n W_a^T ;  D1 = n W_next^T (x of the next layer)
+        if (tid == 0) {
+            tc::tc_fence_after_sync();
+            issue_gemm(tmem_d0, sA0, sW + 3 * OPB, idesc, false);
+            if (!a.last) issue_gemm(tmem_d1, sA0, sW + 4 * OPB, idesc, false);
+            tc::mma_commit(mbar_mma);
+        }
+        tc::mbar_wait(mbar_mma, par);
+        par ^= 1;
+        tc::tc_fence_after_sync();
+        // ---- E <- E + D0 + b_a ; XE = (x, E) packed bf16, or E -> A1 for G = W_f1 E
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+            const int c0 = g * 32 + j * 16;
+            float v[16], ee[16];
+            tc::tmem_ld16(tmem_d0 + lane_field + c0, v);
+#pragma unroll
+            for (int e4 = 0; e4 < 4; ++e4) {
+                float4 t = valid ? *(const float4 *)(a.E + (size_t)row * H + c0 + e4 * 4) : make_float4(0.f, 0.f, 0.f, 0.f);
+                ee[e4 * 4 + 0] = t.x; ee[e4 * 4 + 1] = t.y; ee[e4 * 4 + 2] = t.z; ee[e4 * 4 + 3] = t.w;
+            }
+#pragma unroll
+            for (int e = 0; e < 16; ++e) ee[e] = ee[e] + (v[e] + sb[2 * H + c0 + e]);
+            if (valid)
+#pragma unroll
+                for (int e4 = 0; e4 < 4; ++e4)
+                    *(float4 *)(a.E + (size_t)row * H + c0 + e4 * 4) =
+                        make_float4(ee[e4 * 4], ee[e4 * 4 + 1], ee[e4 * 4 + 2], ee[e4 * 4 + 3]);
+            if (!a.last) {
+                tc::tmem_ld16(tmem_d1 + lane_field + c0, v);
+                if (valid)
+#pragma unroll
+                    for (int e4 = 0; e4 < 4; ++e4)
+                        *(uint4 *)(a.XE + (size_t)row * H + c0 + e4 * 4) =
+                            make_uint4(tc::pack_bf16(v[e4 * 4], ee[e4 * 4]), tc::pack_bf16(v[e4 * 4 + 1], ee[e4 * 4 + 1]),
+                                       tc::pack_bf16(v[e4 * 4 + 2], ee[e4 * 4 + 2]), tc::pack_bf16(v[e4 * 4 + 3], ee[e4 * 4 + 3]));
+            } else {
+                store_operand16(A1, r, c0, ee);
+            }
+        }
+        if (a.last) {
+            tc::tc_fence_before_sync();
+            tc::fence_proxy_async_smem();
+            __syncthreads();
+            if (tid == 0) {
+                tc::tc_fence_after_sync();
+                issue_gemm(tmem_d1, sA1, sW + 4 * OPB, idesc, false);
+                tc::mma_commit(mbar_mma);
+            }
+            tc::mbar_wait(mbar_mma, par);
+            par ^= 1;
+            tc::tc_fence_after_sync();
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+                const int c0 = g * 32 + j * 16;
+                float v[16];
+                tc::tmem_ld16(tmem_d1 + lane_field + c0, v);
+                if (valid)
+#pragma unroll
+                    for (int e4 = 0; e4 < 4; ++e4)
+                        *(float4 *)(a.G + (size_t)row * H + c0 + e4 * 4) =
+                            make_float4(v[e4 * 4], v[e4 * 4 + 1], v[e4 * 4 + 2], v[e4 * 4 + 3]);
+            }
+        }
+        tc::tc_fence_before_sync();
+        __syncthreads();   // TMEM and operand tiles free for the next tile
+    }
+    if (!w_ready && tid == 0) tc::mbar_wait(mbar_w, 0);   // never leave with bulk copies in flight
+    __syncthreads();
+    if (warp == 1) tc::tmem_dealloc(tmem_d0, 256);
+}
+
+// layer-0 inputs: n = Emb[species], E = 0, x = W_s^0 n (one vector per species, formed on the host) -> XE
+__global__ void node_init_tc_kernel(int64_t rows, int N, const int *__restrict__ species, const float *__restrict__ Emb,
+                                    const float *__restrict__ xs0, float *__restrict__ n, float *__restrict__ E,
+                                    uint32_t *__restrict__ XE)
+{
+    const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= rows * (H / 4)) return;
+    const int64_t row = idx >> 5;
+    const int c0 = (int)(idx & 31) * 4;
+    const int s = species[row % N];
+    const float4 nv = __ldg((const float4 *)(Emb + (size_t)s * H + c0));
+    const float4 xv = __ldg((const float4 *)(xs0 + (size_t)s * H + c0));
+    *(float4 *)(n + (size_t)row * H + c0) = nv;
+    *(float4 *)(E + (size_t)row * H + c0) = make_float4(0.f, 0.f, 0.f, 0.f);
+    *(uint4 *)(XE + (size_t)row * H + c0) =
+        make_uint4(tc::pack_bf16(xv.x, 0.f), tc::pack_bf16(xv.y, 0.f), tc::pack_bf16(xv.z, 0.f), tc::pack_bf16(xv.w, 0.f));
+}
+
+int launch_node_tc(pimd_ctx *c, int mode, int layer)
+{
+    const GfnDev &n = c->net;
+    if (mode == 0) {
+        const int64_t work = c->rows * (H / 4);
+        node_init_tc_kernel<<<(unsigned)((work + 255) / 256), 256, 0, c->stream>>>(c->rows, c->N, c->species, n.Emb, c->xs0,
+                                                                                 c->nfeat, c->Efeat, c->XE);
+        c->launches++;
+        PIMD_CUDA_CHECK(cudaGetLastError());
+        return 0;
+    }
+    const GfnLayerW &w = n.layer[layer];
+    Args a;
+    a.rows = c->rows; a.N = c->N; a.last = (layer == n.L - 1); a.gran_m = c->gran_m;
+    a.n_tiles = (int)((c->rows + TR - 1) / TR);
+    a.row_ptr = c->nl.row_ptr;
+    a.Wimg = c->wimg_node + (size_t)layer * NW * (OPB / 2);
+    a.bv1 = w.bv1; a.bv2 = w.bv2; a.ba = w.ba;
+    a.n = c->nfeat; a.E = c->Efeat; a.m = c->mfeat; a.carry_m = c->carry_m;
+    a.XE = c->XE; a.G = c->Gfeat;
+    const size_t smem = SMEM_BYTES + 1024;
+    static bool attr = false;
+    if (!attr) {
+        PIMD_CUDA_CHECK(cudaFuncSetAttribute(node_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr = true;
+    }
+    const int grid = a.n_tiles < c->num_sms ? a.n_tiles : c->num_sms;
+    node_tc_kernel<<<grid, NTH, smem, c->stream>>>(a);
+    c->launches++;
+    PIMD_CUDA_CHECK(cudaGetLastError());
+    return 0;
+}
+
+}  // namespace node_tc

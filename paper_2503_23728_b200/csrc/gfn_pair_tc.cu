@@ -34,7 +34,8 @@ struct PairArgs {
     const double *q;
     const uint16_t *W1img, *W2img;        // bf16 UMMA images: 0.5 W_e1 [128][64]; W_e2 (message) or 0.5 W_f1 W_e2 (head), 2 x [128][64]
     const float *b1, *b2;
-    const float *Ea, *xa;                 // message: E, x ; head: G, unused
+    const uint32_t *XE;                   // message: packed bf16 (x | E << 16) per (row, channel)
+    const float *Gf;                      // head: fp32 G = W_f1 E
     const float *wf2; float bf2;
     float *m_out, *carry_m, *Fraw, *carry_f;
 };
@@ -79,8 +80,8 @@ __device__ __forceinline__ void flush_m(const PairArgs &a, const GroupSmem &G, i
 // D2 is TRANSPOSED: TMEM lane = channel c, column = pair.  Thread (c, half) walks the 64 pairs of its granule in
 // CSR order, 16 at a time (one tcgen05.ld).  Chunks without a row boundary (fmask == 0) take a branch-free path.
 template <bool HEAD>
-__device__ __forceinline__ void epilogue(const PairArgs &a, Smem &S, GroupSmem &G, const float *__restrict__ Ea,
-                                         const float *__restrict__ xa, uint32_t tmem_lane, int c, int half, int lane,
+__device__ __forceinline__ void epilogue(const PairArgs &a, Smem &S, GroupSmem &G, const uint32_t *__restrict__ XE,
+                                         const float *__restrict__ Gf, uint32_t tmem_lane, int c, int half, int lane,
                                          int gtid, int64_t tile0, int bar_id)
 {
     constexpr int GP = 64;
@@ -92,30 +93,31 @@ __device__ __forceinline__ void epilogue(const PairArgs &a, Smem &S, GroupSmem &
 #pragma unroll 1
         for (int cc = 0; cc < 4; ++cc) {
             const int q0 = half * GP + cc * 16;
-            float v[16], xj[16], Ej[16], w[16];
+            float v[16], w[16];
+            uint32_t xe[16];
 #pragma unroll
             for (int e4 = 0; e4 < 4; ++e4) {
                 const int4 o = *(const int4 *)&G.joff[q0 + e4 * 4];
-                xj[e4 * 4 + 0] = __ldg(xa + o.x + c); Ej[e4 * 4 + 0] = __ldg(Ea + o.x + c);
-                xj[e4 * 4 + 1] = __ldg(xa + o.y + c); Ej[e4 * 4 + 1] = __ldg(Ea + o.y + c);
-                xj[e4 * 4 + 2] = __ldg(xa + o.z + c); Ej[e4 * 4 + 2] = __ldg(Ea + o.z + c);
-                xj[e4 * 4 + 3] = __ldg(xa + o.w + c); Ej[e4 * 4 + 3] = __ldg(Ea + o.w + c);
+                xe[e4 * 4 + 0] = __ldg(XE + o.x + c); xe[e4 * 4 + 1] = __ldg(XE + o.y + c);
+                xe[e4 * 4 + 2] = __ldg(XE + o.z + c); xe[e4 * 4 + 3] = __ldg(XE + o.w + c);
                 *(float4 *)&w[e4 * 4] = *(const float4 *)&G.w[q0 + e4 * 4];
             }
             const unsigned mask = G.fmask[half * 4 + cc];
             tc::tmem_ld16(tmem_lane + q0, v);
             if (mask == 0u) {
 #pragma unroll
-                for (int e = 0; e < 16; ++e) sum = fmaf((v[e] + be) + Ej[e], w[e] * xj[e], sum);
+                for (int e = 0; e < 16; ++e)
+                    sum = fmaf((v[e] + be) + tc::bf16hi_to_f32(xe[e]), w[e] * tc::bf16lo_to_f32(xe[e]), sum);
             } else {
 #pragma unroll
                 for (int e = 0; e < 16; ++e) {
                     if ((mask >> e) & 1u) {   // warp-uniform
                         flush_m(a, G, cur, pfirst, g0, g1, gidx, c, sum);
                         cur = G.row[q0 + e]; pfirst = q0 + e; sum = 0.f;
-                        be = b2c + ((cur >= 0) ? __ldg(Ea + (size_t)cur * H + c) : 0.f);
+                        be = b2c + ((cur >= 0) ? tc::bf16hi_to_f32(__ldg(XE + (size_t)cur * H + c)) : 0.f);
                     }
-                    sum = fmaf((v[e] + be) + Ej[e], w[e] * xj[e], sum);   // w = 0 for pairs past the end of the list
+                    // w = 0 for pairs past the end of the list
+                    sum = fmaf((v[e] + be) + tc::bf16hi_to_f32(xe[e]), w[e] * tc::bf16lo_to_f32(xe[e]), sum);
                 }
             }
         }
@@ -134,8 +136,8 @@ __device__ __forceinline__ void epilogue(const PairArgs &a, Smem &S, GroupSmem &
 #pragma unroll
             for (int e4 = 0; e4 < 4; ++e4) {
                 const int4 o = *(const int4 *)&G.joff[q0 + e4 * 4];
-                Gj[e4 * 4 + 0] = __ldg(Ea + o.x + c); Gj[e4 * 4 + 1] = __ldg(Ea + o.y + c);
-                Gj[e4 * 4 + 2] = __ldg(Ea + o.z + c); Gj[e4 * 4 + 3] = __ldg(Ea + o.w + c);
+                Gj[e4 * 4 + 0] = __ldg(Gf + o.x + c); Gj[e4 * 4 + 1] = __ldg(Gf + o.y + c);
+                Gj[e4 * 4 + 2] = __ldg(Gf + o.z + c); Gj[e4 * 4 + 3] = __ldg(Gf + o.w + c);
             }
             const unsigned mask = G.fmask[half * 4 + cc];
             tc::tmem_ld16(tmem_lane + q0, v);
@@ -150,7 +152,7 @@ __device__ __forceinline__ void epilogue(const PairArgs &a, Smem &S, GroupSmem &
                 for (int e = 0; e < 16; ++e) {
                     if ((mask >> e) & 1u) {
                         const int r = G.row[q0 + e];
-                        be = b2c + ((r >= 0) ? 0.5f * __ldg(Ea + (size_t)r * H + c) : 0.f);
+                        be = b2c + ((r >= 0) ? 0.5f * __ldg(Gf + (size_t)r * H + c) : 0.f);
                     }
                     const float h = fmaf(0.5f, Gj[e], v[e] + be);
                     v[e] = wc * fmaf(h, tc::tanh_approx(h), h);
@@ -219,8 +221,8 @@ __global__ void __launch_bounds__(GT * NG, 1) pair_tc_kernel(const __grid_consta
     const int64_t n_pairs = a.row_ptr[a.rows];
     if ((int64_t)blockIdx.x * (NG * TP) >= n_pairs) return;   // uniform per CTA
     GroupSmem &G = S.g[grp];
-    const float *__restrict__ Ea = a.Ea;
-    const float *__restrict__ xa = a.xa;
+    const uint32_t *__restrict__ XE = a.XE;
+    const float *__restrict__ Gf = a.Gf;
 
     // ---- one-time setup: weights (generic proxy) -> smem, mbarriers, TMEM
     {
@@ -348,7 +350,7 @@ __global__ void __launch_bounds__(GT * NG, 1) pair_tc_kernel(const __grid_consta
         parity ^= 1;
         tc::tc_fence_after_sync();
         // EPILOGUE (see part 2)
-        epilogue<HEAD>(a, S, G, Ea, xa, tmem_d2 + lane_field, p, half, lane, gtid, tile0, bar_id);
+        epilogue<HEAD>(a, S, G, XE, Gf, tmem_d2 + lane_field, p, half, lane, gtid, tile0, bar_id);
         tc::named_bar_sync(bar_id, GT);   // tile buffers free for the next iteration
     }
     // ---- teardown
@@ -367,7 +369,7 @@ int launch_pair_tc(pimd_ctx *c, bool head)
     a.row_ptr = c->nl.row_ptr; a.col = c->nl.col; a.pair_row = c->nl.pair_row; a.rows = c->rows; a.q = c->q;
     a.W1img = c->wimg_e1; a.W2img = head ? c->wimg_fe : c->wimg_e2;
     a.b1 = c->net.be1; a.b2 = head ? c->net.bfe : c->net.be2;
-    a.Ea = head ? c->Gfeat : c->Efeat; a.xa = c->xfeat;
+    a.XE = c->XE; a.Gf = c->Gfeat;
     a.wf2 = c->net.wf2; a.bf2 = c->net.bf2;
     a.m_out = c->mfeat; a.carry_m = c->carry_m; a.Fraw = c->Fraw; a.carry_f = c->carry_f;
     const size_t smem = sizeof(Smem) + 1024;

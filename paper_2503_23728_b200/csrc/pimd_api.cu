@@ -61,7 +61,7 @@ namespace {
 struct Layout {
     size_t q, p, F, species, mass, C, CT, omega, err, est_partial, est_out;
     size_t cell_id, cell_count, cell_start, cell_cursor, sorted_atom, sorted_q, nnz, hits, row_ptr, block_sums, col, pair_row;
-    size_t wimg, weights, nfeat, xfeat, mfeat, Efeat, Gfeat, carry_m, carry_f, Fraw;
+    size_t wimg, wimg_node, xs0, weights, nfeat, xfeat, mfeat, Efeat, Gfeat, carry_m, carry_f, Fraw;
     size_t total;
     int ncell[3], nct;
     int64_t pair_cap, n_gran_m, n_gran_f, n_wfloats;
@@ -169,6 +169,8 @@ int compute_layout(int N, int R, int P, const double box[3], const pimd_net_para
         L->pair_row = take(cur, sizeof(int) * L->pair_cap);
         L->weights = take(cur, sizeof(float) * L->n_wfloats);
         L->wimg = take(cur, 5 * 16384);   // bf16 UMMA images: W_e1 (16 KB), W_e2 (32 KB), W_f1 W_e2 (32 KB)
+        L->wimg_node = take(cur, (size_t)(net->n_layers > 0 ? net->n_layers : 1) * 5 * 32768);
+        L->xs0 = take(cur, sizeof(float) * (size_t)net->n_species * H);
         L->nfeat = take(cur, sizeof(float) * rows * H);
         L->xfeat = take(cur, sizeof(float) * rows * H);
         L->mfeat = take(cur, sizeof(float) * rows * H);
@@ -204,7 +206,11 @@ void build_umma_image(const float *W, int n_rows, int n_k, float scale, uint16_t
 }
 
 // derived, transposed fp32 weights in the order the kernels use (S:G0 is the input order)
-void build_weights(const pimd_net_params *net, std::vector<float> &out, std::vector<size_t> &offs, std::vector<float> &Wfe)
+struct RawLayer { const float *Ws, *Wvn, *Wvm, *bv1, *Wv2, *bv2, *Wa, *ba; };
+struct RawNet { const float *Emb, *We1, *be1, *We2, *be2, *Wf1, *bf1, *wf2; std::vector<RawLayer> layer; };
+
+void build_weights(const pimd_net_params *net, std::vector<float> &out, std::vector<size_t> &offs, std::vector<float> &Wfe,
+                   RawNet &raw)
 {
     const int S = net->n_species, K = net->n_rbf, H = net->hidden, L = net->n_layers;
     const float *w = net->weights;
@@ -217,13 +223,14 @@ void build_weights(const pimd_net_params *net, std::vector<float> &out, std::vec
     };
     auto pushV = [&](const float *v, int n) { offs.push_back(out.size()); out.insert(out.end(), v, v + n); };
     const float *Emb = mat(S, H), *We1 = mat(H, K), *be1 = vec(H), *We2 = mat(H, H), *be2 = vec(H);
-    struct Lw { const float *Ws, *Wvn, *Wvm, *bv1, *Wv2, *bv2, *Wa, *ba; };
-    std::vector<Lw> lw(L);
+    std::vector<RawLayer> lw(L);
     for (int l = 0; l < L; ++l) {
         lw[l].Ws = mat(H, H); lw[l].Wvn = mat(H, H); lw[l].Wvm = mat(H, H); lw[l].bv1 = vec(H);
         lw[l].Wv2 = mat(H, H); lw[l].bv2 = vec(H); lw[l].Wa = mat(H, H); lw[l].ba = vec(H);
     }
     const float *Wf1 = mat(H, H), *bf1 = vec(H), *wf2 = vec(H);
+    raw.Emb = Emb; raw.We1 = We1; raw.be1 = be1; raw.We2 = We2; raw.be2 = be2; raw.Wf1 = Wf1; raw.bf1 = bf1; raw.wf2 = wf2;
+    raw.layer = lw;
     // W_fe = W_f1 W_e2 and b_fe = W_f1 b_e2 + b_f1, formed in fp64 then rounded once
     std::vector<float> bfe(H);
     Wfe.assign((size_t)H * H, 0.f);
@@ -389,8 +396,8 @@ extern "C" int pimd_create(pimd_ctx **out, int n_atoms, int n_replicas, const in
     CREATE_CHECK(cudaMemcpyAsync(c->CmatT, CT.data(), sizeof(double) * P * P, cudaMemcpyHostToDevice, st));
     CREATE_CHECK(cudaMemcpyAsync(c->omega_k, om.data(), sizeof(double) * P, cudaMemcpyHostToDevice, st));
 
-    std::vector<float> wd;
-    std::vector<uint16_t> wimg;
+    std::vector<float> wd, xs0;
+    std::vector<uint16_t> wimg, wimg_node;
     if (net->kind == 0) {
         const int H = net->hidden;
         NlistDev &nl = c->nl;
@@ -408,7 +415,8 @@ extern "C" int pimd_create(pimd_ctx **out, int n_atoms, int n_replicas, const in
         c->gran_m = L.gran_m; c->gran_f = L.gran_f; c->n_gran_m = L.n_gran_m; c->n_gran_f = L.n_gran_f;
         std::vector<size_t> offs;
         std::vector<float> Wfe;
-        build_weights(net, wd, offs, Wfe);
+        RawNet raw;
+        build_weights(net, wd, offs, Wfe, raw);
         c->use_tc = (net->gemm_dtype == 1 && net->n_rbf == 64 && net->hidden == 128) ? 1 : 0;
         c->wimg_e1 = (uint16_t *)(ws + L.wimg); c->wimg_e2 = c->wimg_e1 + 8192; c->wimg_fe = c->wimg_e2 + 16384;
         if (c->use_tc) {
@@ -419,6 +427,29 @@ extern "C" int pimd_create(pimd_ctx **out, int n_atoms, int n_replicas, const in
             build_umma_image(We2, H, H, 1.0f, wimg.data() + 8192);
             build_umma_image(Wfe.data(), H, H, 0.5f, wimg.data() + 8192 + 16384);
             CREATE_CHECK(cudaMemcpyAsync(c->wimg_e1, wimg.data(), sizeof(uint16_t) * wimg.size(), cudaMemcpyHostToDevice, st));
+            // atom-wise layers: five images per layer; SiLU's 1/2 folded into W_vn, W_vm
+            c->wimg_node = (uint16_t *)(ws + L.wimg_node); c->xs0 = (float *)(ws + L.xs0);
+            c->XE = (uint32_t *)c->xfeat;
+            const int Ln = net->n_layers;
+            wimg_node.resize((size_t)(Ln > 0 ? Ln : 1) * 5 * 16384);
+            for (int l = 0; l < Ln; ++l) {
+                uint16_t *img = wimg_node.data() + (size_t)l * 5 * 16384;
+                build_umma_image(raw.layer[l].Wvn, H, H, 0.5f, img);
+                build_umma_image(raw.layer[l].Wvm, H, H, 0.5f, img + 16384);
+                build_umma_image(raw.layer[l].Wv2, H, H, 1.0f, img + 2 * 16384);
+                build_umma_image(raw.layer[l].Wa, H, H, 1.0f, img + 3 * 16384);
+                build_umma_image(l + 1 < Ln ? raw.layer[l + 1].Ws : raw.Wf1, H, H, 1.0f, img + 4 * 16384);
+            }
+            xs0.assign((size_t)net->n_species * H, 0.f);
+            if (Ln > 0)
+                for (int s = 0; s < net->n_species; ++s)
+                    for (int o = 0; o < H; ++o) {
+                        double acc = 0.0;
+                        for (int k = 0; k < H; ++k) acc += (double)raw.layer[0].Ws[(size_t)o * H + k] * (double)raw.Emb[(size_t)s * H + k];
+                        xs0[(size_t)s * H + o] = (float)acc;
+                    }
+            CREATE_CHECK(cudaMemcpyAsync(c->wimg_node, wimg_node.data(), sizeof(uint16_t) * wimg_node.size(), cudaMemcpyHostToDevice, st));
+            CREATE_CHECK(cudaMemcpyAsync(c->xs0, xs0.data(), sizeof(float) * xs0.size(), cudaMemcpyHostToDevice, st));
         }
         if ((int64_t)wd.size() != L.n_wfloats) {
             pimd_set_error("internal: derived weight count %zu != %lld", wd.size(), (long long)L.n_wfloats);

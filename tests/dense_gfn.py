@@ -31,8 +31,9 @@ def silu(x):
     return x / (1.0 + np.exp(-x))
 
 
-def dense_forces(species, x, box, w, S, K, H, L, r_cut, agg_norm, force_scale):
-    """x [N,3]; box [3] (zeros = open).  Returns F [N,3]."""
+def dense_forces(species, x, box, w, S, K, H, L, r_cut, agg_norm, force_scale, gross=False):
+    """x [N,3]; box [3] (zeros = open).  Returns F [N,3]; with gross=True also the sum of the
+    magnitudes of all terms of F_i, force_scale * sum_j c_ij (sum_o |w_f2[o] SiLU(t_o)| + |b_f2|)  [N]."""
     p = unpack(w, S, K, H, L)
     N = x.shape[0]
     delta = x[None, :, :] - x[:, None, :]  # delta[i, j] = x_j - x_i
@@ -56,5 +57,9 @@ def dense_forces(species, x, box, w, S, K, H, L, r_cut, agg_norm, force_scale):
         n = n + silu(n @ lay["W_vn"].T + m @ lay["W_vm"].T + lay["b_v1"]) @ lay["W_v2"].T + lay["b_v2"]
         E = E + n @ lay["W_a"].T + lay["b_a"]
     e = e0 + E[:, None, :] + E[None, :, :]
-    s = silu(e @ p["W_f1"].T + p["b_f1"]) @ p["w_f2"] + p["b_f2"]  # [N,N]
-    return force_scale * np.einsum("ij,ij,ija->ia", c, s, u)
+    act = silu(e @ p["W_f1"].T + p["b_f1"])
+    s = act @ p["w_f2"] + p["b_f2"]  # [N,N]
+    F = force_scale * np.einsum("ij,ij,ija->ia", c, s, u)
+    if gross:
+        return F, abs(force_scale) * (c * (np.abs(act) @ np.abs(p["w_f2"]) + abs(p["b_f2"]))).sum(axis=1)
+    return F

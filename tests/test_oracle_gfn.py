@@ -85,6 +85,19 @@ def test_matches_independent_dense_numpy(cluster):
         assert np.abs(F - Fd).max() < 1e-12 * max(1.0, np.abs(F).max()), (K, H, L)
 
 
+def test_gross_pair_term_scale_matches_dense_numpy(cluster):
+    """The diagnostic the bf16 parity bound is stated against: the sum of the magnitudes of all terms of F_i (>= |F_i|)."""
+    sp, x = cluster
+    for (K, H, L, rc, box) in [(8, 16, 2, 3.0, np.zeros(3)), (6, 8, 3, 2.5, np.array([5.5, 6.0, 5.1]))]:
+        net = make_net(K, H, L, rc, seed=4)
+        xx = x if box[0] == 0 else x * 1.2
+        sim = RefPIMD(sp, MASSES, xx[None], box, 1, 300.0, 0.25, -1.0, 0, net)
+        F, g = sim.forces()[0, 0], sim.force_gross()[0, 0]
+        Fd, gd = dense_forces(sp, xx, box, net.weights, 3, K, H, L, net.r_cut, net.agg_norm, net.force_scale, gross=True)
+        assert np.abs(g - gd).max() < 1e-12 * max(1.0, gd.max())
+        assert np.all(np.linalg.norm(F, axis=1) <= g + 1e-12) and g.max() > 0
+
+
 def test_two_atoms_L0_by_hand():
     K, H, rc = 6, 8, 4.0
     net = make_net(K, H, 0, rc, seed=5)
