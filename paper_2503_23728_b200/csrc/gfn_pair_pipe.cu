@@ -1,0 +1,586 @@
+// gfn_pair_pipe.cu -- fused per-pair kernels of the GFN force net on the 5th-gen tensor cores, as a
+// warp-specialised pipeline (rows a5, a7 of SURVEY 8(a)).  bf16 operands, fp32 accumulation
+// in TMEM.  Used when gemm_dtype == 1 and (K, H) == (64, 128)  (BASELINE configs[3..4]; tolerance 2e-2).
+//
+// One persistent CTA per SM walks 128-pair tiles of the flat CSR pair list.  Five roles run concurrently on
+// different tiles and hand buffers to each other through mbarriers only (no CTA-wide barrier in the loop):
+//   P   4 warps, thread = pair : indices, fp64 minimum image -> distance, cutoff weight, row-segment flags (meta ring);
+//                                Gaussian RBF tile -> A1 (bf16, K-major, 128-byte swizzle)
+//   MMA 1 thread               : D1 = A1 (W_e1/2)^T  (4 x UMMA 128x128x16);  D2^T = W2 A2^T  (8 x UMMA), W2 = W_e2 or W_f1 W_e2/2
+//   H   4 warps, thread = pair : D1 (TMEM) + b -> SiLU -> A2 (bf16 operand of the second product)
+//   G   4 warps                : TMA bulk copies of the gathered rows (x_j|E_j packed bf16, or G_j fp32; 512 B per pair)
+//                                into a 4-slot shared-memory ring, 32 pairs per slot
+//   E   8 warps, thread = (channel, half tile): D2^T (TMEM lane = channel) -> e_ij = e0_ij + E_i + E_j (S:G5) ->
+//                                message: private running sums over CSR row segments, flushed at row boundaries;
+//                                head:    w_f2 . SiLU(.) reduced over channels by a fixed shuffle tree, then a
+//                                         segmented warp scan of c_ij s_ij u_ij over 32-pair granules.
+// Row segments that straddle a reduction granule go through carry slots that the consumer adds in a fixed
+// order: no floating-point atomics, bitwise reproducible.
+// SiLU(x) = h tanh(h) + h with h = x/2: the factor 1/2 is folded (exactly) into the bf16 weight images.
+#include "common.cuh"
+#include "tc_ptx.cuh"
+
+namespace gfn_pipe {
+
+constexpr int TP = 128;      // pairs per tile
+constexpr int H = 128;       // channels
+constexpr int K = 64;        // radial basis functions
+constexpr int NM = 4;        // meta ring depth (tiles)
+constexpr int NSLOT = 4;     // gather ring slots per tile (32 pairs each)
+constexpr int NTHREADS = 21 * 32;   // 4 P + 4 H + 8 E + 1 MMA + 4 G warps
+
+struct PairArgs {
+    int N, periodic;
+    double box[3], inv_box[3];
+    float r_cut, wscale;
+    const int *row_ptr, *col, *pair_row;
+    int64_t rows;
+    const double *q;
+    const uint16_t *W1img, *W2img;        // bf16 UMMA images: 0.5 W_e1 [128][64]; W_e2 (message) or 0.5 W_f1 W_e2 (head), 2 x [128][64]
+    const float *b1, *b2;
+    const void *gsrc;                     // message: XE packed bf16 (x | E << 16) [rows][128] u32; head: G fp32 [rows][128]
+    const float *wf2; float bf2;
+    float *m_out, *carry_m, *Fraw, *carry_f;
+};
+
+struct Meta {
+    float w[TP];                 // cutoff weight x wscale (0 for pairs past the end of the list)
+    int jrow[TP];                // global row of atom j
+    int rowk[TP];                // global row of atom i | kind << 29;  -1 past the end of the list
+    float u[3][TP];              // unit vector (r_i - r_j)/d  (head)
+    unsigned fmask[8];           // per 16-pair chunk: bit e set = pair starts a new row segment
+};
+
+// shared-memory carve (offsets from a 1024-aligned base)
+constexpr int OFF_W1 = 0;                          // 16 KB
+constexpr int OFF_W2 = OFF_W1 + 16384;             // 32 KB
+constexpr int OFF_A1 = OFF_W2 + 32768;             // 2 x 16 KB
+constexpr int OFF_A2 = OFF_A1 + 2 * 16384;         // 2 x 32 KB
+constexpr int OFF_RING = OFF_A2 + 2 * 32768;       // 4 x 16 KB
+constexpr int OFF_META = OFF_RING + NSLOT * 16384; // NM x sizeof(Meta)
+constexpr int OFF_BIAS = OFF_META + NM * (int)sizeof(Meta);   // b1, b2, wf2
+constexpr int OFF_S4 = OFF_BIAS + 3 * H * 4;       // head: s4[4][TP]
+constexpr int OFF_BAR = OFF_S4 + 4 * TP * 4;
+constexpr int N_BAR = 40;
+constexpr int OFF_TMEM = OFF_BAR + N_BAR * 8;
+constexpr int SMEM_BYTES = OFF_TMEM + 16;
+
+// mbarrier indices
+enum { A1_FULL = 0, A1_EMPTY = 2, D1_FULL = 4, D1_EMPTY = 6, A2_FULL = 8, A2_EMPTY = 10, D2_FULL = 12, D2_EMPTY = 14,
+       XE_FULL = 16, XE_EMPTY = 20, META_FULL = 24, META_EMPTY = 28, W_FULL = 32 };
+
+__device__ __forceinline__ float ex2_approx(float x)
+{
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+__device__ __forceinline__ int n_my_tiles(int64_t n_pairs)
+{
+    const int64_t n_tiles = (n_pairs + TP - 1) / TP;
+    if ((int64_t)blockIdx.x >= n_tiles) return 0;
+    return (int)((n_tiles - 1 - blockIdx.x) / gridDim.x) + 1;
+}
+
+// kind of the segment of row [rs, re) inside the granule [g0, g0 + GP): 0 whole row here (direct store),
+// 1 row began in an earlier granule (carry slot 0), 2 row continues into a later granule (carry slot 1)
+__device__ __forceinline__ int seg_kind(int rs, int re, int64_t g0, int GP)
+{
+    if (rs >= g0 && re <= g0 + GP) return 0;
+    return (rs < g0) ? 1 : 2;
+}
+
+__device__ __forceinline__ Meta &meta_of(unsigned char *S, int it) { return *(Meta *)(S + OFF_META + (it & (NM - 1)) * (int)sizeof(Meta)); }
+
+constexpr float RBF_C = 0.84932180028801904f;   // sqrt(0.5 log2 e): exp(-t^2/2) = 2^-(C t)^2
+constexpr unsigned FULL = 0xffffffffu;
+
+// ---- role P: per-pair geometry (S:G1) + Gaussian RBF tile.  Thread p owns pair p of every tile of this CTA.
+template <bool HEAD>
+__device__ __forceinline__ void role_P(const PairArgs &a, unsigned char *S, uint64_t *bar, int n_my, int64_t n_pairs, int p,
+                                       int lane)
+{
+    constexpr int GP = HEAD ? 32 : 64;            // pairs per reduction granule of the consumer
+    const float inv_rc = 1.0f / a.r_cut;
+    const float uc_scale = (float)(K - 1) / a.r_cut * RBF_C;
+    const int64_t stride = (int64_t)gridDim.x * TP;
+    int64_t pg = (int64_t)blockIdx.x * TP + p;
+    int row_n = -1, col_n = 0;
+    if (n_my > 0 && pg < n_pairs) { row_n = __ldg(a.pair_row + pg); col_n = __ldg(a.col + pg); }
+    for (int it = 0; it < n_my; ++it, pg += stride) {
+        const int row = row_n, cj = col_n;
+        if (it + 1 < n_my) {                      // indices of the next tile: in flight during this tile's arithmetic
+            const int64_t pn = pg + stride;
+            row_n = -1; col_n = 0;
+            if (pn < n_pairs) { row_n = __ldg(a.pair_row + pn); col_n = __ldg(a.col + pn); }
+        }
+        int jrow = 0, kind = 0;
+        float w = 0.f, ux = 0.f, uy = 0.f, uz = 0.f, dist = 0.f;
+        int prev_row = -1;
+        if (lane == 0 && (p & (GP - 1)) != 0 && pg - 1 < n_pairs) prev_row = __ldg(a.pair_row + pg - 1);
+        if (row >= 0) {
+            const int sys = row / a.N;
+            jrow = sys * a.N + cj;
+            const int rs = __ldg(a.row_ptr + row), re = __ldg(a.row_ptr + row + 1);
+            float f[3];
+#pragma unroll
+            for (int ax = 0; ax < 3; ++ax) {      // fp64 difference and minimum image, fp32 from there on
+                double dx = a.q[(size_t)jrow * 3 + ax] - a.q[(size_t)row * 3 + ax];
+                if (a.periodic) dx = dx - a.box[ax] * rint(dx * a.inv_box[ax]);
+                f[ax] = (float)dx;
+            }
+            const float d2 = fmaf(f[0], f[0], fmaf(f[1], f[1], f[2] * f[2]));
+            const float inv = rsqrtf(fmaxf(d2, 1e-24f));
+            dist = d2 * inv;
+            ux = -f[0] * inv; uy = -f[1] * inv; uz = -f[2] * inv;
+            w = a.wscale * 0.5f * (cospif(dist * inv_rc) + 1.0f);
+            kind = seg_kind(rs, re, pg & ~(int64_t)(GP - 1), GP);
+        }
+        int prev = __shfl_up_sync(FULL, row, 1);
+        if (lane == 0) prev = ((p & (GP - 1)) == 0) ? -2 : prev_row;
+        const unsigned fm = __ballot_sync(FULL, row != prev);
+        // ---- meta slot
+        tc::mbar_wait(&bar[META_EMPTY + (it & (NM - 1))], ((it / NM) & 1) ^ 1);
+        Meta &M = meta_of(S, it);
+        if (lane == 0) { M.fmask[2 * (p >> 5)] = fm & 0xFFFFu; M.fmask[2 * (p >> 5) + 1] = fm >> 16; }
+        M.w[p] = w; M.jrow[p] = jrow; M.rowk[p] = (row < 0) ? -1 : (row | (kind << 29));
+        if (HEAD) { M.u[0][p] = ux; M.u[1][p] = uy; M.u[2][p] = uz; }
+        __syncwarp();
+        if (lane == 0) tc::mbar_arrive(&bar[META_FULL + (it & (NM - 1))]);
+        // ---- RBF tile -> A1 (bf16, K-major rows of 128 B, 16-byte chunks XOR-swizzled by row & 7)
+        tc::mbar_wait(&bar[A1_EMPTY + (it & 1)], ((it >> 1) & 1) ^ 1);
+        unsigned char *A1 = S + OFF_A1 + (it & 1) * 16384 + p * 128;
+        const float uc = dist * uc_scale;         // C d / delta
+#pragma unroll 2
+        for (int ch = 0; ch < 8; ++ch) {
+            float g[8];
+#pragma unroll
+            for (int e = 0; e < 8; ++e) {
+                const float t = uc - RBF_C * (float)(ch * 8 + e);
+                g[e] = ex2_approx(-t * t);
+            }
+            *(uint4 *)(A1 + ((ch ^ (p & 7)) << 4)) =
+                make_uint4(tc::pack_bf16(g[0], g[1]), tc::pack_bf16(g[2], g[3]), tc::pack_bf16(g[4], g[5]), tc::pack_bf16(g[6], g[7]));
+        }
+        tc::fence_proxy_async_smem();
+        __syncwarp();
+        if (lane == 0) tc::mbar_arrive(&bar[A1_FULL + (it & 1)]);
+    }
+}
+
+// ---- role H: h1 = SiLU(2 (D1 + b_e1/2)) -> A2.  Thread p owns TMEM lane p (pair p) and all 128 columns.
+__device__ __forceinline__ void role_H(unsigned char *S, uint64_t *bar, uint32_t tmem, int n_my, int p, int lane)
+{
+    const float *b1 = (const float *)(S + OFF_BIAS);
+    const uint32_t lane_field = (uint32_t)(p & ~31) << 16;
+    for (int it = 0; it < n_my; ++it) {
+        const int s = it & 1, ph = (it >> 1) & 1;
+        tc::mbar_wait(&bar[A2_EMPTY + s], ph ^ 1);
+        tc::mbar_wait(&bar[D1_FULL + s], ph);
+        tc::tc_fence_after_sync();
+        unsigned char *rowp = S + OFF_A2 + s * 32768 + p * 128;
+        const uint32_t td1 = tmem + s * 128 + lane_field;
+#pragma unroll 1
+        for (int c2 = 0; c2 < 4; ++c2) {
+            uint32_t r0[16], r1[16];
+            tc::tmem_ld16_nowait(td1 + c2 * 32, r0);
+            tc::tmem_ld16_nowait(td1 + c2 * 32 + 16, r1);
+            tc::tmem_ld_wait();
+#pragma unroll
+            for (int hh = 0; hh < 2; ++hh) {
+                const int cc = c2 * 2 + hh;
+                uint32_t pk[8];
+#pragma unroll
+                for (int e = 0; e < 8; ++e) {
+                    const int col = cc * 16 + 2 * e;
+                    const float h0 = __uint_as_float(hh ? r1[2 * e] : r0[2 * e]) + b1[col];
+                    const float h1 = __uint_as_float(hh ? r1[2 * e + 1] : r0[2 * e + 1]) + b1[col + 1];
+                    pk[e] = tc::pack_bf16(fmaf(h0, tc::tanh_approx(h0), h0), fmaf(h1, tc::tanh_approx(h1), h1));
+                }
+                unsigned char *kb = rowp + (cc >> 2) * 16384;
+                const int ch0 = (cc & 3) * 2;
+                *(uint4 *)(kb + ((ch0 ^ (p & 7)) << 4)) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+                *(uint4 *)(kb + (((ch0 + 1) ^ (p & 7)) << 4)) = make_uint4(pk[4], pk[5], pk[6], pk[7]);
+            }
+        }
+        tc::tc_fence_before_sync();
+        tc::fence_proxy_async_smem();
+        __syncwarp();
+        if (lane == 0) { tc::mbar_arrive(&bar[D1_EMPTY + s]); tc::mbar_arrive(&bar[A2_FULL + s]); }
+    }
+}
+
+// ---- role E, message pass: m_i = agg_norm sum_j c_ij (e0_ij + E_i + E_j) (.) x_j  (S:G3, G5).
+// D2 is TRANSPOSED (TMEM lane = channel c, column = pair): the thread walks the 64 pairs of its half tile in CSR
+// order.  With wx = c_ij x_j:  m_i = sum_j (e0 + E_j) wx + (b + E_i) sum_j wx, so the two private running sums do not
+// depend on the row and a row boundary only cuts them.  x_j, E_j come from the gather ring (lanes = consecutive
+// channels: conflict-free).  Code is kept small on purpose (five roles share the instruction cache).
+struct MsgState {
+    int cur, kind, nx_row;       // current row (-1 none), its segment kind, row whose E_i is prefetched
+    uint32_t nx_val;
+    float s1, s2, be;
+};
+
+__device__ __forceinline__ void msg_flush(const PairArgs &a, const MsgState &st, int64_t gidx, int c)
+{
+    if (st.cur >= 0) {
+        float *dst = (st.kind == 0) ? a.m_out + (size_t)st.cur * H + c : a.carry_m + (size_t)(gidx * 2 + (st.kind - 1)) * H + c;
+        *dst = fmaf(st.be, st.s2, st.s1);
+    }
+}
+
+__device__ __forceinline__ void role_E_msg(const PairArgs &a, unsigned char *S, uint64_t *bar, uint32_t tmem, int n_my, int c,
+                                           int half, int lane)
+{
+    const float b2c = ((const float *)(S + OFF_BIAS))[H + c];
+    const uint32_t *__restrict__ XE = (const uint32_t *)a.gsrc;
+    const uint32_t lane_field = (uint32_t)(c & ~31) << 16;
+    const int64_t stride = (int64_t)gridDim.x * TP;
+    int64_t tile0 = (int64_t)blockIdx.x * TP;
+    MsgState st;
+    st.cur = -1; st.kind = 0; st.nx_row = -1; st.nx_val = 0; st.s1 = st.s2 = st.be = 0.f;
+    for (int it = 0; it < n_my; ++it, tile0 += stride) {
+        const Meta &M = meta_of(S, it);
+        const int64_t gidx = (tile0 >> 6) + half;
+        tc::mbar_wait(&bar[META_FULL + (it & (NM - 1))], (it / NM) & 1);
+        tc::mbar_wait(&bar[D2_FULL + (it & 1)], (it >> 1) & 1);
+        tc::tc_fence_after_sync();
+        const uint32_t td2 = tmem + 256 + (it & 1) * 128 + lane_field;
+        st.cur = -1; st.s1 = 0.f; st.s2 = 0.f;
+#pragma unroll 1
+        for (int cc = 0; cc < 4; ++cc) {
+            const int q0 = half * 64 + cc * 16, slot = half * 2 + (cc >> 1);
+            float v[16];
+            tc::tmem_ld16(td2 + q0, v);
+            if (cc == 3) {                       // accumulator drained: hand D2 back to the MMA warp
+                tc::tc_fence_before_sync();
+                __syncwarp();
+                if (lane == 0) tc::mbar_arrive(&bar[D2_EMPTY + (it & 1)]);
+            }
+            if ((cc & 1) == 0) tc::mbar_wait(&bar[XE_FULL + slot], it & 1);
+            const uint32_t *xr = (const uint32_t *)(S + OFF_RING + slot * 16384 + (cc & 1) * 8192) + c;
+            float wx[16];
+#pragma unroll
+            for (int e4 = 0; e4 < 4; ++e4) {
+                const float4 w4 = *(const float4 *)&M.w[q0 + e4 * 4];
+                const float wv[4] = {w4.x, w4.y, w4.z, w4.w};
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const uint32_t xe = xr[(e4 * 4 + k) * H];
+                    wx[e4 * 4 + k] = wv[k] * tc::bf16lo_to_f32(xe);       // c_ij x_j
+                    v[e4 * 4 + k] += tc::bf16hi_to_f32(xe);               // e0 + E_j
+                }
+            }
+            unsigned mask = M.fmask[half * 4 + cc];
+            if (mask == 0u) {
+#pragma unroll
+                for (int e = 0; e < 16; ++e) { st.s1 = fmaf(v[e], wx[e], st.s1); st.s2 += wx[e]; }
+            } else {
+                int lo = 0;
+#pragma unroll 1
+                while (true) {                   // warp-uniform: segments [lo, hi) between row boundaries
+                    const int hi = mask ? (__ffs(mask) - 1) : 16;
+#pragma unroll
+                    for (int e = 0; e < 16; ++e)
+                        if (e >= lo && e < hi) { st.s1 = fmaf(v[e], wx[e], st.s1); st.s2 += wx[e]; }
+                    if (!mask) break;
+                    mask &= mask - 1;
+                    lo = hi;
+                    msg_flush(a, st, gidx, c);   // a new row segment starts at pair q0 + hi
+                    const int rk = M.rowk[q0 + hi];
+                    st.cur = (rk < 0) ? -1 : (rk & 0x1FFFFFFF);
+                    st.kind = (rk < 0) ? 0 : (rk >> 29);
+                    st.s1 = 0.f; st.s2 = 0.f;
+                    if (st.cur >= 0) {           // E_i: prefetched at the previous boundary (CSR rows are consecutive)
+                        const uint32_t raw = (st.cur == st.nx_row) ? st.nx_val : __ldg(XE + (size_t)st.cur * H + c);
+                        st.be = b2c + tc::bf16hi_to_f32(raw);
+                        st.nx_row = (st.cur + 1 < a.rows) ? st.cur + 1 : st.cur;
+                        st.nx_val = __ldg(XE + (size_t)st.nx_row * H + c);
+                    }
+                }
+            }
+            if (cc & 1) {                        // both 16-pair chunks of this ring slot consumed
+                __syncwarp();
+                if (lane == 0) tc::mbar_arrive(&bar[XE_EMPTY + slot]);
+            }
+        }
+        msg_flush(a, st, gidx, c);
+        __syncwarp();
+        if (lane == 0) tc::mbar_arrive(&bar[META_EMPTY + (it & (NM - 1))]);
+    }
+}
+
+// ---- role E, force head: s_ij = w_f2 . SiLU(W_fe h1 + b_fe + G_i + G_j) + b_f2,  F_i = sum_j c_ij s_ij u_ij  (S:G4).
+// Everything is carried as h = t/2.  Per-thread term for channel c, then a fixed-tree transposing reduction over the
+// 32 lanes and the 4 lane quadrants; pair-level segmented warp scan over 32-pair granules.
+__device__ __forceinline__ void role_E_head(const PairArgs &a, unsigned char *S, uint64_t *bar, uint32_t tmem, int n_my, int c,
+                                            int half, int lane, int e_tid)
+{
+    const float b2c = 0.5f * ((const float *)(S + OFF_BIAS))[H + c];
+    const float wc = ((const float *)(S + OFF_BIAS))[2 * H + c];
+    const float *__restrict__ Gf = (const float *)a.gsrc;
+    float *s4 = (float *)(S + OFF_S4);           // [4][TP]
+    const int quarter = c >> 5;
+    const uint32_t lane_field = (uint32_t)(c & ~31) << 16;
+    const int64_t stride = (int64_t)gridDim.x * TP;
+    int64_t tile0 = (int64_t)blockIdx.x * TP;
+    int nx_row = -1;
+    float nx_val = 0.f;
+    for (int it = 0; it < n_my; ++it, tile0 += stride) {
+        const Meta &M = meta_of(S, it);
+        tc::mbar_wait(&bar[META_FULL + (it & (NM - 1))], (it / NM) & 1);
+        tc::mbar_wait(&bar[D2_FULL + (it & 1)], (it >> 1) & 1);
+        tc::tc_fence_after_sync();
+        const uint32_t td2 = tmem + 256 + (it & 1) * 128 + lane_field;
+        float be = 0.f;
+#pragma unroll 1
+        for (int cc = 0; cc < 4; ++cc) {
+            const int q0 = half * 64 + cc * 16, slot = half * 2 + (cc >> 1);
+            float v[16];
+            tc::tmem_ld16(td2 + q0, v);
+            if (cc == 3) {
+                tc::tc_fence_before_sync();
+                __syncwarp();
+                if (lane == 0) tc::mbar_arrive(&bar[D2_EMPTY + (it & 1)]);
+            }
+            if ((cc & 1) == 0) tc::mbar_wait(&bar[XE_FULL + slot], it & 1);
+            const float *gr = (const float *)(S + OFF_RING + slot * 16384 + (cc & 1) * 8192) + c;
+            float gj[16];
+#pragma unroll
+            for (int e = 0; e < 16; ++e) gj[e] = gr[e * H];
+            unsigned mask = M.fmask[half * 4 + cc];
+            if (mask == 0u) {
+#pragma unroll
+                for (int e = 0; e < 16; ++e) {
+                    const float h = fmaf(0.5f, gj[e], v[e] + be);
+                    v[e] = wc * fmaf(h, tc::tanh_approx(h), h);
+                }
+            } else {
+                int lo = 0;
+#pragma unroll 1
+                while (true) {                   // warp-uniform: segments [lo, hi) between row boundaries
+                    const int hi = mask ? (__ffs(mask) - 1) : 16;
+#pragma unroll
+                    for (int e = 0; e < 16; ++e)
+                        if (e >= lo && e < hi) {
+                            const float h = fmaf(0.5f, gj[e], v[e] + be);
+                            v[e] = wc * fmaf(h, tc::tanh_approx(h), h);
+                        }
+                    if (!mask) break;
+                    mask &= mask - 1;
+                    lo = hi;
+                    const int rk = M.rowk[q0 + hi];
+                    const int r = (rk < 0) ? -1 : (rk & 0x1FFFFFFF);
+                    if (r >= 0) {
+                        const float raw = (r == nx_row) ? nx_val : __ldg(Gf + (size_t)r * H + c);
+                        be = b2c + 0.5f * raw;
+                        nx_row = (r + 1 < a.rows) ? r + 1 : r;
+                        nx_val = __ldg(Gf + (size_t)nx_row * H + c);
+                    }
+                }
+            }
+            if (cc & 1) {
+                __syncwarp();
+                if (lane == 0) tc::mbar_arrive(&bar[XE_EMPTY + slot]);
+            }
+            // transposing reduction over the 32 lanes (channels of this quadrant): 16 pairs -> lanes
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                const float send = (lane & 16) ? v[i] : v[i + 8], keep = (lane & 16) ? v[i + 8] : v[i];
+                v[i] = keep + __shfl_xor_sync(FULL, send, 16);
+            }
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const float send = (lane & 8) ? v[i] : v[i + 4], keep = (lane & 8) ? v[i + 4] : v[i];
+                v[i] = keep + __shfl_xor_sync(FULL, send, 8);
+            }
+#pragma unroll
+            for (int i = 0; i < 2; ++i) {
+                const float send = (lane & 4) ? v[i] : v[i + 2], keep = (lane & 4) ? v[i + 2] : v[i];
+                v[i] = keep + __shfl_xor_sync(FULL, send, 4);
+            }
+            {
+                const float send = (lane & 2) ? v[0] : v[1], keep = (lane & 2) ? v[1] : v[0];
+                v[0] = keep + __shfl_xor_sync(FULL, send, 2);
+            }
+            v[0] += __shfl_xor_sync(FULL, v[0], 1);
+            // lane bits (4,3,2,1) select pair e = 8 b4 + 4 b3 + 2 b2 + b1
+            if ((lane & 1) == 0)
+                s4[quarter * TP + q0 + ((lane >> 4) & 1) * 8 + ((lane >> 3) & 1) * 4 + ((lane >> 2) & 1) * 2 + ((lane >> 1) & 1)] = v[0];
+        }
+        tc::named_bar_sync(1, 256);              // s4 of this tile complete
+        if (e_tid < TP) {
+            const int p = e_tid;
+            const int rk = M.rowk[p];
+            const int key = (rk < 0) ? -1 : (rk & 0x1FFFFFFF);
+            const float f = M.w[p] * (((s4[p] + s4[TP + p]) + (s4[2 * TP + p] + s4[3 * TP + p])) + a.bf2);
+            float fv[3] = {f * M.u[0][p], f * M.u[1][p], f * M.u[2][p]};
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int ko = __shfl_up_sync(FULL, key, o);
+#pragma unroll
+                for (int ax = 0; ax < 3; ++ax) {
+                    const float vo = __shfl_up_sync(FULL, fv[ax], o);
+                    if (lane >= o && ko == key) fv[ax] += vo;
+                }
+            }
+            const int knext = __shfl_down_sync(FULL, key, 1);
+            if (key >= 0 && (lane == 31 || knext != key)) {
+                const int kind = rk >> 29;
+                const int64_t gidx = (tile0 + (p & ~31)) >> 5;
+                float *dst = (kind == 0) ? a.Fraw + (size_t)key * 4 : a.carry_f + (size_t)(gidx * 2 + (kind - 1)) * 4;
+                dst[0] = fv[0]; dst[1] = fv[1]; dst[2] = fv[2];
+            }
+        }
+        tc::named_bar_sync(1, 256);              // s4 free for the next tile
+        if (lane == 0) tc::mbar_arrive(&bar[META_EMPTY + (it & (NM - 1))]);
+    }
+}
+
+// ---- role MMA: one elected lane issues both products; completion is committed to the consumers' mbarriers
+__device__ __forceinline__ void role_MMA(unsigned char *S, uint64_t *bar, uint32_t tmem, int n_my, int lane)
+{
+    const uint32_t idesc = tc::make_idesc_bf16(TP, H);
+    const uint32_t sW1 = tc::smem_u32(S + OFF_W1), sW2 = tc::smem_u32(S + OFF_W2);
+    const uint32_t sA1 = tc::smem_u32(S + OFF_A1), sA2 = tc::smem_u32(S + OFF_A2);
+    tc::mbar_wait(&bar[W_FULL], 0);
+    for (int k = 0; k <= n_my; ++k) {
+        if (k < n_my) {                          // D1[s] = G (W_e1/2)^T   (4 x UMMA 128x128x16)
+            const int s = k & 1, ph = (k >> 1) & 1;
+            tc::mbar_wait(&bar[D1_EMPTY + s], ph ^ 1);
+            tc::mbar_wait(&bar[A1_FULL + s], ph);
+            tc::tc_fence_after_sync();
+            if (lane == 0) {
+#pragma unroll
+                for (int kk = 0; kk < K / 16; ++kk)
+                    tc::mma_bf16_ss(tmem + s * 128, tc::make_desc_sw128(sA1 + s * 16384 + kk * 32),
+                                    tc::make_desc_sw128(sW1 + kk * 32), idesc, kk > 0);
+                tc::mma_commit(&bar[D1_FULL + s]);
+                tc::mma_commit(&bar[A1_EMPTY + s]);
+            }
+            __syncwarp();
+        }
+        if (k >= 1) {                            // D2[s]^T = W2 h1^T   (8 x UMMA; M = channels, N = pairs)
+            const int j = k - 1, s = j & 1, ph = (j >> 1) & 1;
+            tc::mbar_wait(&bar[D2_EMPTY + s], ph ^ 1);
+            tc::mbar_wait(&bar[A2_FULL + s], ph);
+            tc::tc_fence_after_sync();
+            if (lane == 0) {
+#pragma unroll
+                for (int kk = 0; kk < H / 16; ++kk) {
+                    const uint32_t off = (kk >> 2) * 16384 + (kk & 3) * 32;
+                    tc::mma_bf16_ss(tmem + 256 + s * 128, tc::make_desc_sw128(sW2 + off),
+                                    tc::make_desc_sw128(sA2 + s * 32768 + off), idesc, kk > 0);
+                }
+                tc::mma_commit(&bar[D2_FULL + s]);
+                tc::mma_commit(&bar[A2_EMPTY + s]);
+            }
+            __syncwarp();
+        }
+    }
+}
+
+// ---- role G: gathered rows (512 B each) -> ring slots by TMA bulk copies.  Warp g feeds slot g: one copy per lane
+// per tile (the copy instruction issues from the uniform datapath, one lane at a time: four warps keep up, one does not)
+__device__ __forceinline__ void role_G(const PairArgs &a, unsigned char *S, uint64_t *bar, int n_my, int slot, int lane)
+{
+    const unsigned char *src = (const unsigned char *)a.gsrc;
+    unsigned char *dst = S + OFF_RING + slot * 16384 + lane * 512;
+    for (int it = 0; it < n_my; ++it) {
+        const Meta &M = meta_of(S, it);
+        tc::mbar_wait(&bar[META_FULL + (it & (NM - 1))], (it / NM) & 1);
+        const int jrow = M.jrow[slot * 32 + lane];
+        tc::mbar_wait(&bar[XE_EMPTY + slot], (it & 1) ^ 1);
+        if (lane == 0) tc::mbar_arrive_expect_tx(&bar[XE_FULL + slot], 16384);
+        __syncwarp();
+        tc::bulk_g2s(dst, src + (size_t)jrow * 512, 512, &bar[XE_FULL + slot]);
+    }
+}
+
+template <bool HEAD>
+__global__ void __launch_bounds__(NTHREADS, 1) pair_pipe_kernel(const __grid_constant__ PairArgs a)
+{
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    unsigned char *S = smem_raw + ((1024u - (tc::smem_u32(smem_raw) & 1023u)) & 1023u);
+    uint64_t *bar = (uint64_t *)(S + OFF_BAR);
+    uint32_t *tmem_slot = (uint32_t *)(S + OFF_TMEM);
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int64_t n_pairs = a.row_ptr[a.rows];
+    const int n_my = n_my_tiles(n_pairs);
+
+    if (tid == 0) {
+        for (int s = 0; s < 2; ++s) {
+            tc::mbar_init(&bar[A1_FULL + s], 4);  tc::mbar_init(&bar[A1_EMPTY + s], 1);
+            tc::mbar_init(&bar[D1_FULL + s], 1);  tc::mbar_init(&bar[D1_EMPTY + s], 4);
+            tc::mbar_init(&bar[A2_FULL + s], 4);  tc::mbar_init(&bar[A2_EMPTY + s], 1);
+            tc::mbar_init(&bar[D2_FULL + s], 1);  tc::mbar_init(&bar[D2_EMPTY + s], 8);
+        }
+        for (int s = 0; s < NSLOT; ++s) { tc::mbar_init(&bar[XE_FULL + s], 1); tc::mbar_init(&bar[XE_EMPTY + s], 4); }
+        for (int s = 0; s < NM; ++s) { tc::mbar_init(&bar[META_FULL + s], 4); tc::mbar_init(&bar[META_EMPTY + s], 8); }
+        tc::mbar_init(&bar[W_FULL], 1);
+        tc::fence_mbar_init();
+    }
+    if (warp == 16) tc::tmem_alloc(tmem_slot, 512);
+    {
+        float *sb = (float *)(S + OFF_BIAS);
+        for (int i = tid; i < H; i += NTHREADS) {
+            sb[i] = 0.5f * a.b1[i];
+            sb[H + i] = a.b2[i];
+            sb[2 * H + i] = HEAD ? a.wf2[i] : 0.f;
+        }
+    }
+    tc::tc_fence_before_sync();
+    __syncthreads();
+    tc::tc_fence_after_sync();
+    const uint32_t tmem = *tmem_slot;
+    if (tid == 17 * 32) {                        // filter weights: two TMA bulk copies of pre-swizzled bf16 images
+        tc::mbar_arrive_expect_tx(&bar[W_FULL], 16384 + 32768);
+        tc::bulk_g2s(S + OFF_W1, a.W1img, 16384, &bar[W_FULL]);
+        tc::bulk_g2s(S + OFF_W2, a.W2img, 32768, &bar[W_FULL]);
+    }
+    if (warp < 4) {
+        role_P<HEAD>(a, S, bar, n_my, n_pairs, tid, lane);
+    } else if (warp < 8) {
+        role_H(S, bar, tmem, n_my, tid - 128, lane);
+    } else if (warp < 16) {
+        const int c = (warp & 3) * 32 + lane, half = (warp - 8) >> 2;
+        if (HEAD) role_E_head(a, S, bar, tmem, n_my, c, half, lane, tid - 256);
+        else role_E_msg(a, S, bar, tmem, n_my, c, half, lane);
+    } else if (warp == 16) {
+        role_MMA(S, bar, tmem, n_my, lane);
+    } else {
+        role_G(a, S, bar, n_my, warp - 17, lane);
+    }
+    tc::tc_fence_before_sync();
+    __syncthreads();
+    if (warp == 16) tc::tmem_dealloc(tmem, 512);
+}
+
+int launch_pair_pipe(pimd_ctx *c, bool head)
+{
+    PairArgs a;
+    a.N = c->N; a.periodic = c->periodic;
+    for (int k = 0; k < 3; ++k) { a.box[k] = c->box[k]; a.inv_box[k] = c->periodic ? 1.0 / c->box[k] : 0.0; }
+    a.r_cut = c->net.r_cut; a.wscale = head ? 1.0f : c->net.agg_norm;
+    a.row_ptr = c->nl.row_ptr; a.col = c->nl.col; a.pair_row = c->nl.pair_row; a.rows = c->rows; a.q = c->q;
+    a.W1img = c->wimg_e1; a.W2img = head ? c->wimg_fe : c->wimg_e2;
+    a.b1 = c->net.be1; a.b2 = head ? c->net.bfe : c->net.be2;
+    a.gsrc = head ? (const void *)c->Gfeat : (const void *)c->XE;
+    a.wf2 = c->net.wf2; a.bf2 = c->net.bf2;
+    a.m_out = c->mfeat; a.carry_m = c->carry_m; a.Fraw = c->Fraw; a.carry_f = c->carry_f;
+    const size_t smem = SMEM_BYTES + 1024;
+    static bool attr = false;
+    if (!attr) {
+        PIMD_CUDA_CHECK(cudaFuncSetAttribute(pair_pipe_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        PIMD_CUDA_CHECK(cudaFuncSetAttribute(pair_pipe_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr = true;
+    }
+    if (head) pair_pipe_kernel<true><<<c->num_sms, NTHREADS, smem, c->stream>>>(a);
+    else pair_pipe_kernel<false><<<c->num_sms, NTHREADS, smem, c->stream>>>(a);
+    c->launches++;
+    PIMD_CUDA_CHECK(cudaGetLastError());
+    return 0;
+}
+
+}  // namespace gfn_pipe
