@@ -86,6 +86,7 @@ struct pimd_ctx {
     int use_tc;                        // 1: tensor-core pair and node kernels (gemm_dtype 1, K=64, H=128)
     uint16_t *wimg_node;               // [L][5] bf16 UMMA images: W_vn/2, W_vm/2, W_v2, W_a, W_s^{l+1} (or W_f1)
     float *xs0;                        // [S][H] W_s^0 Emb[s]
+    float h_be1_half[128];             // HOST copy of b_e1 / 2 (passed to the pair kernels as kernel parameters)
     uint32_t *XE;                      // [rows][H] packed bf16 (x | E << 16) gathered by the pair kernels (aliases xfeat)
     float *nfeat, *xfeat, *mfeat, *Efeat, *Gfeat;   // [rows][H]
     float *carry_m;                    // [n_gran_m][2][H]

@@ -236,13 +236,12 @@ int launch_pair_t(pimd_ctx *c, const PairArgs &a, bool head)
 }
 
 }  // namespace gfn
-namespace gfn_tc { int launch_pair_tc(pimd_ctx *c, bool head); }
 namespace gfn_pipe { int launch_pair_pipe(pimd_ctx *c, bool head); }
 namespace gfn {
 
 int launch_pair(pimd_ctx *c, int layer, bool head)
 {
-    if (c->use_tc) return (c->use_tc == 2) ? gfn_tc::launch_pair_tc(c, head) : gfn_pipe::launch_pair_pipe(c, head);
+    if (c->use_tc) return gfn_pipe::launch_pair_pipe(c, head);
     PairArgs a;
     a.N = c->N; a.periodic = c->periodic;
     for (int k = 0; k < 3; ++k) a.box[k] = c->box[k];

@@ -10,24 +10,51 @@
 //   H   4 warps, thread = pair : D1 (TMEM) + b -> SiLU -> A2 (bf16 operand of the second product)
 //   G   4 warps                : TMA bulk copies of the gathered rows (x_j|E_j packed bf16, or G_j fp32; 512 B per pair)
 //                                into a 4-slot shared-memory ring, 32 pairs per slot
-//   E   8 warps, thread = (channel, half tile): D2^T (TMEM lane = channel) -> e_ij = e0_ij + E_i + E_j (S:G5) ->
+//   E   16 warps, thread = (channel, quarter tile): D2^T (TMEM lane = channel) -> e_ij = e0_ij + E_i + E_j (S:G5) ->
 //                                message: private running sums over CSR row segments, flushed at row boundaries;
 //                                head:    w_f2 . SiLU(.) reduced over channels by a fixed shuffle tree, then a
 //                                         segmented warp scan of c_ij s_ij u_ij over 32-pair granules.
+// Waiting: mbarrier try_wait does not suspend on this part (it polls, and every poll takes an issue slot from the warps
+// that have work).  So per role ONE warp polls the mbarriers that tensor-core commits and TMA transactions complete
+// on, and releases its role's other warps through a named barrier (bar.sync blocks in hardware); the pollers sit on
+// different SM sub-partitions.  Hand-offs between threads only (ring slot consumed: E -> G) are named barriers.
 // Row segments that straddle a reduction granule go through carry slots that the consumer adds in a fixed
 // order: no floating-point atomics, bitwise reproducible.
 // SiLU(x) = h tanh(h) + h with h = x/2: the factor 1/2 is folded (exactly) into the bf16 weight images.
 #include "common.cuh"
 #include "tc_ptx.cuh"
+#ifdef GFN_PIPE_STATS
+#include <stdio.h>
+#endif
 
 namespace gfn_pipe {
+
+// -DGFN_PIPE_STATS: every role counts the cycles it spends waiting; block 0 prints them (diagnostic builds only)
+#ifdef GFN_PIPE_STATS
+#define WAITED(stmt)                       \
+    do {                                   \
+        const long long t0_ = clock64();   \
+        stmt;                              \
+        g_wait_ += clock64() - t0_;        \
+    } while (0)
+#define STATS_BEGIN long long g_wait_ = 0; const long long g_start_ = clock64();
+#define STATS_END(name)                                                                                              \
+    if (blockIdx.x == 0 && (threadIdx.x & 31) == 0)                                                                  \
+        printf("%s warp %2d: total %lld cycles, waiting %lld (%.0f%%)\n", name, (int)(threadIdx.x >> 5), clock64() - g_start_, \
+               g_wait_, 100.0 * g_wait_ / (double)(clock64() - g_start_));
+#else
+#define WAITED(stmt) stmt
+#define STATS_BEGIN
+#define STATS_END(name)
+#endif
 
 constexpr int TP = 128;      // pairs per tile
 constexpr int H = 128;       // channels
 constexpr int K = 64;        // radial basis functions
 constexpr int NM = 4;        // meta ring depth (tiles)
 constexpr int NSLOT = 4;     // gather ring slots per tile (32 pairs each)
-constexpr int NTHREADS = 21 * 32;   // 4 P + 4 H + 8 E + 1 MMA + 4 G warps
+constexpr int NTHREADS = 29 * 32;   // 4 P + 4 H + 16 E + 1 MMA + 4 G warps
+constexpr int W_MMA = 24, W_G0 = 25; // warp indices of the MMA issuer and of the first gather warp
 
 struct PairArgs {
     int N, periodic;
@@ -37,7 +64,8 @@ struct PairArgs {
     int64_t rows;
     const double *q;
     const uint16_t *W1img, *W2img;        // bf16 UMMA images: 0.5 W_e1 [128][64]; W_e2 (message) or 0.5 W_f1 W_e2 (head), 2 x [128][64]
-    const float *b1, *b2;
+    float b1h[H];                         // b_e1 / 2 (kernel-parameter constant bank: immediate operands in role H)
+    const float *b2;
     const void *gsrc;                     // message: XE packed bf16 (x | E << 16) [rows][128] u32; head: G fp32 [rows][128]
     const float *wf2; float bf2;
     float *m_out, *carry_m, *Fraw, *carry_f;
@@ -65,9 +93,12 @@ constexpr int N_BAR = 40;
 constexpr int OFF_TMEM = OFF_BAR + N_BAR * 8;
 constexpr int SMEM_BYTES = OFF_TMEM + 16;
 
+// named barriers (0 is __syncthreads)
+enum { NB_P = 1, NB_H = 2, NB_E = 3 /* +quarter */, NB_S4 = 7, NB_SLOT = 8 /* +slot: ring slot consumed, E (128) -> G (32) */ };
+
 // mbarrier indices
 enum { A1_FULL = 0, A1_EMPTY = 2, D1_FULL = 4, D1_EMPTY = 6, A2_FULL = 8, A2_EMPTY = 10, D2_FULL = 12, D2_EMPTY = 14,
-       XE_FULL = 16, XE_EMPTY = 20, META_FULL = 24, META_EMPTY = 28, W_FULL = 32 };
+       XE_FULL = 16, META_FULL = 24, META_EMPTY = 28, W_FULL = 32 };
 
 __device__ __forceinline__ float ex2_approx(float x)
 {
@@ -101,7 +132,8 @@ template <bool HEAD>
 __device__ __forceinline__ void role_P(const PairArgs &a, unsigned char *S, uint64_t *bar, int n_my, int64_t n_pairs, int p,
                                        int lane)
 {
-    constexpr int GP = HEAD ? 32 : 64;            // pairs per reduction granule of the consumer
+    STATS_BEGIN
+    constexpr int GP = 32;                        // pairs per reduction granule of the consumer (a quarter tile)
     const float inv_rc = 1.0f / a.r_cut;
     const float uc_scale = (float)(K - 1) / a.r_cut * RBF_C;
     const int64_t stride = (int64_t)gridDim.x * TP;
@@ -141,7 +173,11 @@ __device__ __forceinline__ void role_P(const PairArgs &a, unsigned char *S, uint
         if (lane == 0) prev = ((p & (GP - 1)) == 0) ? -2 : prev_row;
         const unsigned fm = __ballot_sync(FULL, row != prev);
         // ---- meta slot
-        tc::mbar_wait(&bar[META_EMPTY + (it & (NM - 1))], ((it / NM) & 1) ^ 1);
+        if ((p >> 5) == 1) {                      // poller of role P (warp 1)
+            WAITED(tc::mbar_wait(&bar[META_EMPTY + (it & (NM - 1))], ((it / NM) & 1) ^ 1));
+            WAITED(tc::mbar_wait(&bar[A1_EMPTY + (it & 1)], ((it >> 1) & 1) ^ 1));
+        }
+        WAITED(tc::named_bar_sync(NB_P, 128));
         Meta &M = meta_of(S, it);
         if (lane == 0) { M.fmask[2 * (p >> 5)] = fm & 0xFFFFu; M.fmask[2 * (p >> 5) + 1] = fm >> 16; }
         M.w[p] = w; M.jrow[p] = jrow; M.rowk[p] = (row < 0) ? -1 : (row | (kind << 29));
@@ -149,10 +185,9 @@ __device__ __forceinline__ void role_P(const PairArgs &a, unsigned char *S, uint
         __syncwarp();
         if (lane == 0) tc::mbar_arrive(&bar[META_FULL + (it & (NM - 1))]);
         // ---- RBF tile -> A1 (bf16, K-major rows of 128 B, 16-byte chunks XOR-swizzled by row & 7)
-        tc::mbar_wait(&bar[A1_EMPTY + (it & 1)], ((it >> 1) & 1) ^ 1);
         unsigned char *A1 = S + OFF_A1 + (it & 1) * 16384 + p * 128;
         const float uc = dist * uc_scale;         // C d / delta
-#pragma unroll 2
+#pragma unroll
         for (int ch = 0; ch < 8; ++ch) {
             float g[8];
 #pragma unroll
@@ -167,21 +202,25 @@ __device__ __forceinline__ void role_P(const PairArgs &a, unsigned char *S, uint
         __syncwarp();
         if (lane == 0) tc::mbar_arrive(&bar[A1_FULL + (it & 1)]);
     }
+    STATS_END("P")
 }
 
 // ---- role H: h1 = SiLU(2 (D1 + b_e1/2)) -> A2.  Thread p owns TMEM lane p (pair p) and all 128 columns.
-__device__ __forceinline__ void role_H(unsigned char *S, uint64_t *bar, uint32_t tmem, int n_my, int p, int lane)
+__device__ __forceinline__ void role_H(const PairArgs &a, unsigned char *S, uint64_t *bar, uint32_t tmem, int n_my, int p, int lane)
 {
-    const float *b1 = (const float *)(S + OFF_BIAS);
+    STATS_BEGIN
     const uint32_t lane_field = (uint32_t)(p & ~31) << 16;
     for (int it = 0; it < n_my; ++it) {
         const int s = it & 1, ph = (it >> 1) & 1;
-        tc::mbar_wait(&bar[A2_EMPTY + s], ph ^ 1);
-        tc::mbar_wait(&bar[D1_FULL + s], ph);
+        if ((p >> 5) == 2) {                      // poller of role H (warp 6)
+            WAITED(tc::mbar_wait(&bar[A2_EMPTY + s], ph ^ 1));
+            WAITED(tc::mbar_wait(&bar[D1_FULL + s], ph));
+        }
+        WAITED(tc::named_bar_sync(NB_H, 128));
         tc::tc_fence_after_sync();
         unsigned char *rowp = S + OFF_A2 + s * 32768 + p * 128;
         const uint32_t td1 = tmem + s * 128 + lane_field;
-#pragma unroll 1
+#pragma unroll
         for (int c2 = 0; c2 < 4; ++c2) {
             uint32_t r0[16], r1[16];
             tc::tmem_ld16_nowait(td1 + c2 * 32, r0);
@@ -194,8 +233,8 @@ __device__ __forceinline__ void role_H(unsigned char *S, uint64_t *bar, uint32_t
 #pragma unroll
                 for (int e = 0; e < 8; ++e) {
                     const int col = cc * 16 + 2 * e;
-                    const float h0 = __uint_as_float(hh ? r1[2 * e] : r0[2 * e]) + b1[col];
-                    const float h1 = __uint_as_float(hh ? r1[2 * e + 1] : r0[2 * e + 1]) + b1[col + 1];
+                    const float h0 = __uint_as_float(hh ? r1[2 * e] : r0[2 * e]) + a.b1h[col];
+                    const float h1 = __uint_as_float(hh ? r1[2 * e + 1] : r0[2 * e + 1]) + a.b1h[col + 1];
                     pk[e] = tc::pack_bf16(fmaf(h0, tc::tanh_approx(h0), h0), fmaf(h1, tc::tanh_approx(h1), h1));
                 }
                 unsigned char *kb = rowp + (cc >> 2) * 16384;
@@ -209,10 +248,11 @@ __device__ __forceinline__ void role_H(unsigned char *S, uint64_t *bar, uint32_t
         __syncwarp();
         if (lane == 0) { tc::mbar_arrive(&bar[D1_EMPTY + s]); tc::mbar_arrive(&bar[A2_FULL + s]); }
     }
+    STATS_END("H")
 }
 
 // ---- role E, message pass: m_i = agg_norm sum_j c_ij (e0_ij + E_i + E_j) (.) x_j  (S:G3, G5).
-// D2 is TRANSPOSED (TMEM lane = channel c, column = pair): the thread walks the 64 pairs of its half tile in CSR
+// D2 is TRANSPOSED (TMEM lane = channel c, column = pair): the thread walks the 32 pairs of its quarter tile in CSR
 // order.  With wx = c_ij x_j:  m_i = sum_j (e0 + E_j) wx + (b + E_i) sum_j wx, so the two private running sums do not
 // depend on the row and a row boundary only cuts them.  x_j, E_j come from the gather ring (lanes = consecutive
 // channels: conflict-free).  Code is kept small on purpose (five roles share the instruction cache).
@@ -230,9 +270,19 @@ __device__ __forceinline__ void msg_flush(const PairArgs &a, const MsgState &st,
     }
 }
 
-__device__ __forceinline__ void role_E_msg(const PairArgs &a, unsigned char *S, uint64_t *bar, uint32_t tmem, int n_my, int c,
-                                           int half, int lane)
+// b + E_i of the row that starts: prefetched at the previous boundary (CSR rows are consecutive), else loaded now
+__device__ __forceinline__ void msg_row_bias(const uint32_t *__restrict__ XE, MsgState &st, int64_t rows, float b2c, int c)
 {
+    const uint32_t raw = (st.cur == st.nx_row) ? st.nx_val : __ldg(XE + (size_t)st.cur * H + c);
+    st.be = b2c + tc::bf16hi_to_f32(raw);
+    st.nx_row = (st.cur + 1 < rows) ? st.cur + 1 : st.cur;
+    st.nx_val = __ldg(XE + (size_t)st.nx_row * H + c);
+}
+
+__device__ __forceinline__ void role_E_msg(const PairArgs &a, unsigned char *S, uint64_t *bar, uint32_t tmem, int n_my, int c,
+                                           int qt, int lane, bool poller)
+{
+    STATS_BEGIN
     const float b2c = ((const float *)(S + OFF_BIAS))[H + c];
     const uint32_t *__restrict__ XE = (const uint32_t *)a.gsrc;
     const uint32_t lane_field = (uint32_t)(c & ~31) << 16;
@@ -242,23 +292,35 @@ __device__ __forceinline__ void role_E_msg(const PairArgs &a, unsigned char *S, 
     st.cur = -1; st.kind = 0; st.nx_row = -1; st.nx_val = 0; st.s1 = st.s2 = st.be = 0.f;
     for (int it = 0; it < n_my; ++it, tile0 += stride) {
         const Meta &M = meta_of(S, it);
-        const int64_t gidx = (tile0 >> 6) + half;
-        tc::mbar_wait(&bar[META_FULL + (it & (NM - 1))], (it / NM) & 1);
-        tc::mbar_wait(&bar[D2_FULL + (it & 1)], (it >> 1) & 1);
+        const int64_t gidx = (tile0 >> 5) + qt;
+        if (poller) {
+            WAITED(tc::mbar_wait(&bar[META_FULL + (it & (NM - 1))], (it / NM) & 1));
+            WAITED(tc::mbar_wait(&bar[D2_FULL + (it & 1)], (it >> 1) & 1));
+        }
+        WAITED(tc::named_bar_sync(NB_E + qt, 128));
         tc::tc_fence_after_sync();
         const uint32_t td2 = tmem + 256 + (it & 1) * 128 + lane_field;
-        st.cur = -1; st.s1 = 0.f; st.s2 = 0.f;
+        st.s1 = 0.f; st.s2 = 0.f;
+        {                                        // the quarter tile is one granule: its first pair always starts a segment
+            const int rk = M.rowk[qt * 32];
+            st.cur = (rk < 0) ? -1 : (rk & 0x1FFFFFFF);
+            st.kind = (rk < 0) ? 0 : (rk >> 29);
+            if (st.cur >= 0) msg_row_bias(XE, st, a.rows, b2c, c);
+        }
 #pragma unroll 1
-        for (int cc = 0; cc < 4; ++cc) {
-            const int q0 = half * 64 + cc * 16, slot = half * 2 + (cc >> 1);
+        for (int cc = 0; cc < 2; ++cc) {
+            const int q0 = qt * 32 + cc * 16, slot = qt;
             float v[16];
             tc::tmem_ld16(td2 + q0, v);
-            if (cc == 3) {                       // accumulator drained: hand D2 back to the MMA warp
+            if (cc == 1) {                       // accumulator drained: hand D2 back to the MMA warp
                 tc::tc_fence_before_sync();
                 __syncwarp();
                 if (lane == 0) tc::mbar_arrive(&bar[D2_EMPTY + (it & 1)]);
             }
-            if ((cc & 1) == 0) tc::mbar_wait(&bar[XE_FULL + slot], it & 1);
+            if ((cc & 1) == 0) {                 // gathered rows of this ring slot have landed
+                if (poller) WAITED(tc::mbar_wait(&bar[XE_FULL + slot], it & 1));
+                WAITED(tc::named_bar_sync(NB_E + qt, 128));
+            }
             const uint32_t *xr = (const uint32_t *)(S + OFF_RING + slot * 16384 + (cc & 1) * 8192) + c;
             float wx[16];
 #pragma unroll
@@ -272,7 +334,8 @@ __device__ __forceinline__ void role_E_msg(const PairArgs &a, unsigned char *S, 
                     v[e4 * 4 + k] += tc::bf16hi_to_f32(xe);               // e0 + E_j
                 }
             }
-            unsigned mask = M.fmask[half * 4 + cc];
+            unsigned mask = M.fmask[qt * 2 + cc];
+            if (cc == 0) mask &= ~1u;            // handled above
             if (mask == 0u) {
 #pragma unroll
                 for (int e = 0; e < 16; ++e) { st.s1 = fmaf(v[e], wx[e], st.s1); st.s2 += wx[e]; }
@@ -292,31 +355,27 @@ __device__ __forceinline__ void role_E_msg(const PairArgs &a, unsigned char *S, 
                     st.cur = (rk < 0) ? -1 : (rk & 0x1FFFFFFF);
                     st.kind = (rk < 0) ? 0 : (rk >> 29);
                     st.s1 = 0.f; st.s2 = 0.f;
-                    if (st.cur >= 0) {           // E_i: prefetched at the previous boundary (CSR rows are consecutive)
-                        const uint32_t raw = (st.cur == st.nx_row) ? st.nx_val : __ldg(XE + (size_t)st.cur * H + c);
-                        st.be = b2c + tc::bf16hi_to_f32(raw);
-                        st.nx_row = (st.cur + 1 < a.rows) ? st.cur + 1 : st.cur;
-                        st.nx_val = __ldg(XE + (size_t)st.nx_row * H + c);
-                    }
+                    if (st.cur >= 0) msg_row_bias(XE, st, a.rows, b2c, c);
                 }
             }
             if (cc & 1) {                        // both 16-pair chunks of this ring slot consumed
-                __syncwarp();
-                if (lane == 0) tc::mbar_arrive(&bar[XE_EMPTY + slot]);
+                if (it + 1 < n_my) tc::named_bar_arrive(NB_SLOT + slot, 160);
             }
         }
         msg_flush(a, st, gidx, c);
         __syncwarp();
         if (lane == 0) tc::mbar_arrive(&bar[META_EMPTY + (it & (NM - 1))]);
     }
+    STATS_END("E")
 }
 
 // ---- role E, force head: s_ij = w_f2 . SiLU(W_fe h1 + b_fe + G_i + G_j) + b_f2,  F_i = sum_j c_ij s_ij u_ij  (S:G4).
 // Everything is carried as h = t/2.  Per-thread term for channel c, then a fixed-tree transposing reduction over the
 // 32 lanes and the 4 lane quadrants; pair-level segmented warp scan over 32-pair granules.
 __device__ __forceinline__ void role_E_head(const PairArgs &a, unsigned char *S, uint64_t *bar, uint32_t tmem, int n_my, int c,
-                                            int half, int lane, int e_tid)
+                                            int qt, int lane, int e_tid, bool poller)
 {
+    STATS_BEGIN
     const float b2c = 0.5f * ((const float *)(S + OFF_BIAS))[H + c];
     const float wc = ((const float *)(S + OFF_BIAS))[2 * H + c];
     const float *__restrict__ Gf = (const float *)a.gsrc;
@@ -329,27 +388,38 @@ __device__ __forceinline__ void role_E_head(const PairArgs &a, unsigned char *S,
     float nx_val = 0.f;
     for (int it = 0; it < n_my; ++it, tile0 += stride) {
         const Meta &M = meta_of(S, it);
-        tc::mbar_wait(&bar[META_FULL + (it & (NM - 1))], (it / NM) & 1);
-        tc::mbar_wait(&bar[D2_FULL + (it & 1)], (it >> 1) & 1);
+        if (poller) {
+            WAITED(tc::mbar_wait(&bar[META_FULL + (it & (NM - 1))], (it / NM) & 1));
+            WAITED(tc::mbar_wait(&bar[D2_FULL + (it & 1)], (it >> 1) & 1));
+        }
+        WAITED(tc::named_bar_sync(NB_E + qt, 128));
         tc::tc_fence_after_sync();
         const uint32_t td2 = tmem + 256 + (it & 1) * 128 + lane_field;
         float be = 0.f;
+        int cur_row = -2;
 #pragma unroll 1
-        for (int cc = 0; cc < 4; ++cc) {
-            const int q0 = half * 64 + cc * 16, slot = half * 2 + (cc >> 1);
+        for (int cc = 0; cc < 2; ++cc) {
+            const int q0 = qt * 32 + cc * 16, slot = qt;
             float v[16];
             tc::tmem_ld16(td2 + q0, v);
-            if (cc == 3) {
+            if (cc == 1) {
                 tc::tc_fence_before_sync();
                 __syncwarp();
                 if (lane == 0) tc::mbar_arrive(&bar[D2_EMPTY + (it & 1)]);
             }
-            if ((cc & 1) == 0) tc::mbar_wait(&bar[XE_FULL + slot], it & 1);
+            if ((cc & 1) == 0) {                 // gathered rows of this ring slot have landed
+                if (poller) WAITED(tc::mbar_wait(&bar[XE_FULL + slot], it & 1));
+                WAITED(tc::named_bar_sync(NB_E + qt, 128));
+            }
             const float *gr = (const float *)(S + OFF_RING + slot * 16384 + (cc & 1) * 8192) + c;
             float gj[16];
 #pragma unroll
             for (int e = 0; e < 16; ++e) gj[e] = gr[e * H];
-            unsigned mask = M.fmask[half * 4 + cc];
+            unsigned mask = M.fmask[qt * 2 + cc];
+            if ((mask & 1u) && cc > 0) {         // granule start forced by P: a boundary for G_i only if the row changes
+                const int rk = M.rowk[q0];
+                if (((rk < 0) ? -1 : (rk & 0x1FFFFFFF)) == cur_row) mask &= ~1u;
+            }
             if (mask == 0u) {
 #pragma unroll
                 for (int e = 0; e < 16; ++e) {
@@ -372,6 +442,7 @@ __device__ __forceinline__ void role_E_head(const PairArgs &a, unsigned char *S,
                     lo = hi;
                     const int rk = M.rowk[q0 + hi];
                     const int r = (rk < 0) ? -1 : (rk & 0x1FFFFFFF);
+                    cur_row = r;
                     if (r >= 0) {
                         const float raw = (r == nx_row) ? nx_val : __ldg(Gf + (size_t)r * H + c);
                         be = b2c + 0.5f * raw;
@@ -381,8 +452,7 @@ __device__ __forceinline__ void role_E_head(const PairArgs &a, unsigned char *S,
                 }
             }
             if (cc & 1) {
-                __syncwarp();
-                if (lane == 0) tc::mbar_arrive(&bar[XE_EMPTY + slot]);
+                if (it + 1 < n_my) tc::named_bar_arrive(NB_SLOT + slot, 160);
             }
             // transposing reduction over the 32 lanes (channels of this quadrant): 16 pairs -> lanes
 #pragma unroll
@@ -409,7 +479,7 @@ __device__ __forceinline__ void role_E_head(const PairArgs &a, unsigned char *S,
             if ((lane & 1) == 0)
                 s4[quarter * TP + q0 + ((lane >> 4) & 1) * 8 + ((lane >> 3) & 1) * 4 + ((lane >> 2) & 1) * 2 + ((lane >> 1) & 1)] = v[0];
         }
-        tc::named_bar_sync(1, 256);              // s4 of this tile complete
+        WAITED(tc::named_bar_sync(NB_S4, 512));          // s4 of this tile complete
         if (e_tid < TP) {
             const int p = e_tid;
             const int rk = M.rowk[p];
@@ -433,14 +503,16 @@ __device__ __forceinline__ void role_E_head(const PairArgs &a, unsigned char *S,
                 dst[0] = fv[0]; dst[1] = fv[1]; dst[2] = fv[2];
             }
         }
-        tc::named_bar_sync(1, 256);              // s4 free for the next tile
+        WAITED(tc::named_bar_sync(NB_S4, 512));          // s4 free for the next tile
         if (lane == 0) tc::mbar_arrive(&bar[META_EMPTY + (it & (NM - 1))]);
     }
+    STATS_END("Eh")
 }
 
 // ---- role MMA: one elected lane issues both products; completion is committed to the consumers' mbarriers
 __device__ __forceinline__ void role_MMA(unsigned char *S, uint64_t *bar, uint32_t tmem, int n_my, int lane)
 {
+    STATS_BEGIN
     const uint32_t idesc = tc::make_idesc_bf16(TP, H);
     const uint32_t sW1 = tc::smem_u32(S + OFF_W1), sW2 = tc::smem_u32(S + OFF_W2);
     const uint32_t sA1 = tc::smem_u32(S + OFF_A1), sA2 = tc::smem_u32(S + OFF_A2);
@@ -448,8 +520,8 @@ __device__ __forceinline__ void role_MMA(unsigned char *S, uint64_t *bar, uint32
     for (int k = 0; k <= n_my; ++k) {
         if (k < n_my) {                          // D1[s] = G (W_e1/2)^T   (4 x UMMA 128x128x16)
             const int s = k & 1, ph = (k >> 1) & 1;
-            tc::mbar_wait(&bar[D1_EMPTY + s], ph ^ 1);
-            tc::mbar_wait(&bar[A1_FULL + s], ph);
+            WAITED(tc::mbar_wait(&bar[D1_EMPTY + s], ph ^ 1));
+            WAITED(tc::mbar_wait(&bar[A1_FULL + s], ph));
             tc::tc_fence_after_sync();
             if (lane == 0) {
 #pragma unroll
@@ -463,8 +535,8 @@ __device__ __forceinline__ void role_MMA(unsigned char *S, uint64_t *bar, uint32
         }
         if (k >= 1) {                            // D2[s]^T = W2 h1^T   (8 x UMMA; M = channels, N = pairs)
             const int j = k - 1, s = j & 1, ph = (j >> 1) & 1;
-            tc::mbar_wait(&bar[D2_EMPTY + s], ph ^ 1);
-            tc::mbar_wait(&bar[A2_FULL + s], ph);
+            WAITED(tc::mbar_wait(&bar[D2_EMPTY + s], ph ^ 1));
+            WAITED(tc::mbar_wait(&bar[A2_FULL + s], ph));
             tc::tc_fence_after_sync();
             if (lane == 0) {
 #pragma unroll
@@ -479,23 +551,26 @@ __device__ __forceinline__ void role_MMA(unsigned char *S, uint64_t *bar, uint32
             __syncwarp();
         }
     }
+    STATS_END("MMA")
 }
 
 // ---- role G: gathered rows (512 B each) -> ring slots by TMA bulk copies.  Warp g feeds slot g: one copy per lane
 // per tile (the copy instruction issues from the uniform datapath, one lane at a time: four warps keep up, one does not)
 __device__ __forceinline__ void role_G(const PairArgs &a, unsigned char *S, uint64_t *bar, int n_my, int slot, int lane)
 {
+    STATS_BEGIN
     const unsigned char *src = (const unsigned char *)a.gsrc;
     unsigned char *dst = S + OFF_RING + slot * 16384 + lane * 512;
     for (int it = 0; it < n_my; ++it) {
         const Meta &M = meta_of(S, it);
-        tc::mbar_wait(&bar[META_FULL + (it & (NM - 1))], (it / NM) & 1);
+        WAITED(tc::mbar_wait(&bar[META_FULL + (it & (NM - 1))], (it / NM) & 1));
         const int jrow = M.jrow[slot * 32 + lane];
-        tc::mbar_wait(&bar[XE_EMPTY + slot], (it & 1) ^ 1);
+        if (it > 0) WAITED(tc::named_bar_sync(NB_SLOT + slot, 160));   // the four E warps of this slot's quarter tile have consumed it
         if (lane == 0) tc::mbar_arrive_expect_tx(&bar[XE_FULL + slot], 16384);
         __syncwarp();
         tc::bulk_g2s(dst, src + (size_t)jrow * 512, 512, &bar[XE_FULL + slot]);
     }
+    STATS_END("G")
 }
 
 template <bool HEAD>
@@ -514,18 +589,17 @@ __global__ void __launch_bounds__(NTHREADS, 1) pair_pipe_kernel(const __grid_con
             tc::mbar_init(&bar[A1_FULL + s], 4);  tc::mbar_init(&bar[A1_EMPTY + s], 1);
             tc::mbar_init(&bar[D1_FULL + s], 1);  tc::mbar_init(&bar[D1_EMPTY + s], 4);
             tc::mbar_init(&bar[A2_FULL + s], 4);  tc::mbar_init(&bar[A2_EMPTY + s], 1);
-            tc::mbar_init(&bar[D2_FULL + s], 1);  tc::mbar_init(&bar[D2_EMPTY + s], 8);
+            tc::mbar_init(&bar[D2_FULL + s], 1);  tc::mbar_init(&bar[D2_EMPTY + s], 16);
         }
-        for (int s = 0; s < NSLOT; ++s) { tc::mbar_init(&bar[XE_FULL + s], 1); tc::mbar_init(&bar[XE_EMPTY + s], 4); }
-        for (int s = 0; s < NM; ++s) { tc::mbar_init(&bar[META_FULL + s], 4); tc::mbar_init(&bar[META_EMPTY + s], 8); }
+        for (int s = 0; s < NSLOT; ++s) { tc::mbar_init(&bar[XE_FULL + s], 1); }
+        for (int s = 0; s < NM; ++s) { tc::mbar_init(&bar[META_FULL + s], 4); tc::mbar_init(&bar[META_EMPTY + s], 16); }
         tc::mbar_init(&bar[W_FULL], 1);
         tc::fence_mbar_init();
     }
-    if (warp == 16) tc::tmem_alloc(tmem_slot, 512);
+    if (warp == W_MMA) tc::tmem_alloc(tmem_slot, 512);
     {
         float *sb = (float *)(S + OFF_BIAS);
         for (int i = tid; i < H; i += NTHREADS) {
-            sb[i] = 0.5f * a.b1[i];
             sb[H + i] = a.b2[i];
             sb[2 * H + i] = HEAD ? a.wf2[i] : 0.f;
         }
@@ -534,7 +608,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) pair_pipe_kernel(const __grid_con
     __syncthreads();
     tc::tc_fence_after_sync();
     const uint32_t tmem = *tmem_slot;
-    if (tid == 17 * 32) {                        // filter weights: two TMA bulk copies of pre-swizzled bf16 images
+    if (tid == W_G0 * 32) {                        // filter weights: two TMA bulk copies of pre-swizzled bf16 images
         tc::mbar_arrive_expect_tx(&bar[W_FULL], 16384 + 32768);
         tc::bulk_g2s(S + OFF_W1, a.W1img, 16384, &bar[W_FULL]);
         tc::bulk_g2s(S + OFF_W2, a.W2img, 32768, &bar[W_FULL]);
@@ -542,19 +616,20 @@ __global__ void __launch_bounds__(NTHREADS, 1) pair_pipe_kernel(const __grid_con
     if (warp < 4) {
         role_P<HEAD>(a, S, bar, n_my, n_pairs, tid, lane);
     } else if (warp < 8) {
-        role_H(S, bar, tmem, n_my, tid - 128, lane);
-    } else if (warp < 16) {
-        const int c = (warp & 3) * 32 + lane, half = (warp - 8) >> 2;
-        if (HEAD) role_E_head(a, S, bar, tmem, n_my, c, half, lane, tid - 256);
-        else role_E_msg(a, S, bar, tmem, n_my, c, half, lane);
-    } else if (warp == 16) {
+        role_H(a, S, bar, tmem, n_my, tid - 128, lane);
+    } else if (warp < 24) {
+        const int c = (warp & 3) * 32 + lane, qt = (warp - 8) >> 2;
+        const bool poller = (warp == 9) || (warp == 14) || (warp == 19) || (warp == 20);   // one per quarter, spread over the sub-partitions
+        if (HEAD) role_E_head(a, S, bar, tmem, n_my, c, qt, lane, tid - 256, poller);
+        else role_E_msg(a, S, bar, tmem, n_my, c, qt, lane, poller);
+    } else if (warp == W_MMA) {
         role_MMA(S, bar, tmem, n_my, lane);
     } else {
-        role_G(a, S, bar, n_my, warp - 17, lane);
+        role_G(a, S, bar, n_my, warp - W_G0, lane);
     }
     tc::tc_fence_before_sync();
     __syncthreads();
-    if (warp == 16) tc::tmem_dealloc(tmem, 512);
+    if (warp == W_MMA) tc::tmem_dealloc(tmem, 512);
 }
 
 int launch_pair_pipe(pimd_ctx *c, bool head)
@@ -565,7 +640,8 @@ int launch_pair_pipe(pimd_ctx *c, bool head)
     a.r_cut = c->net.r_cut; a.wscale = head ? 1.0f : c->net.agg_norm;
     a.row_ptr = c->nl.row_ptr; a.col = c->nl.col; a.pair_row = c->nl.pair_row; a.rows = c->rows; a.q = c->q;
     a.W1img = c->wimg_e1; a.W2img = head ? c->wimg_fe : c->wimg_e2;
-    a.b1 = c->net.be1; a.b2 = head ? c->net.bfe : c->net.be2;
+    for (int k = 0; k < H; ++k) a.b1h[k] = c->h_be1_half[k];
+    a.b2 = head ? c->net.bfe : c->net.be2;
     a.gsrc = head ? (const void *)c->Gfeat : (const void *)c->XE;
     a.wf2 = c->net.wf2; a.bf2 = c->net.bf2;
     a.m_out = c->mfeat; a.carry_m = c->carry_m; a.Fraw = c->Fraw; a.carry_f = c->carry_f;

@@ -134,7 +134,8 @@ int compute_layout(int N, int R, int P, const double box[3], const pimd_net_para
         if (cap_row < 1) cap_row = 1;
         L->pair_cap = (rows * cap_row + 255) / 256 * 256;
         if (L->pair_cap > 2000000000LL) { pimd_set_error("pair capacity exceeds int32 range"); return PIMD_ERR_ARG; }
-        L->gran_m = H / 2;   // pairs per message-reduction granule: TP * H / NT
+        // pairs per message-reduction granule: TP * H / NT in the fp32 kernel, a quarter tile in the tcgen05 pipeline
+        L->gran_m = (net->gemm_dtype == 1 && net->n_rbf == 64 && H == 128) ? 32 : H / 2;
         L->gran_f = 32;
         L->n_gran_m = L->pair_cap / L->gran_m + 2;
         L->n_gran_f = L->pair_cap / L->gran_f + 2;
@@ -418,7 +419,6 @@ extern "C" int pimd_create(pimd_ctx **out, int n_atoms, int n_replicas, const in
         RawNet raw;
         build_weights(net, wd, offs, Wfe, raw);
         c->use_tc = (net->gemm_dtype == 1 && net->n_rbf == 64 && net->hidden == 128) ? 1 : 0;
-        if (c->use_tc && getenv("PIMD_PAIR_LEGACY")) c->use_tc = 2;   // TEMPORARY A/B switch while the pipelined kernel lands
         c->wimg_e1 = (uint16_t *)(ws + L.wimg); c->wimg_e2 = c->wimg_e1 + 8192; c->wimg_fe = c->wimg_e2 + 16384;
         if (c->use_tc) {
             wimg.resize(5 * 8192);
@@ -431,6 +431,7 @@ extern "C" int pimd_create(pimd_ctx **out, int n_atoms, int n_replicas, const in
             // atom-wise layers: five images per layer; SiLU's 1/2 folded into W_vn, W_vm
             c->wimg_node = (uint16_t *)(ws + L.wimg_node); c->xs0 = (float *)(ws + L.xs0);
             c->XE = (uint32_t *)c->xfeat;
+            for (int k = 0; k < H && k < 128; ++k) c->h_be1_half[k] = 0.5f * raw.be1[k];
             const int Ln = net->n_layers;
             wimg_node.resize((size_t)(Ln > 0 ? Ln : 1) * 5 * 16384);
             for (int l = 0; l < Ln; ++l) {
