@@ -87,6 +87,7 @@ struct pimd_ctx {
     uint16_t *wimg_node;               // [L][5] bf16 UMMA images: W_vn/2, W_vm/2, W_v2, W_a, W_s^{l+1} (or W_f1)
     float *xs0;                        // [S][H] W_s^0 Emb[s]
     float h_be1_half[128];             // HOST copy of b_e1 / 2 (passed to the pair kernels as kernel parameters)
+    unsigned char *h1_img, *meta_img;  // [pair_cap/128 + 1] tile images kept between the pair passes of one evaluation (tc path)
     uint32_t *XE;                      // [rows][H] packed bf16 (x | E << 16) gathered by the pair kernels (aliases xfeat)
     float *nfeat, *xfeat, *mfeat, *Efeat, *Gfeat;   // [rows][H]
     float *carry_m;                    // [n_gran_m][2][H]

@@ -9,11 +9,15 @@
 //   MMA 1 thread               : D1 = A1 (W_e1/2)^T  (4 x UMMA 128x128x16);  D2^T = W2 A2^T  (8 x UMMA), W2 = W_e2 or W_f1 W_e2/2
 //   H   4 warps, thread = pair : D1 (TMEM) + b -> SiLU -> A2 (bf16 operand of the second product)
 //   G   4 warps                : TMA bulk copies of the gathered rows (x_j|E_j packed bf16, or G_j fp32; 512 B per pair)
-//                                into a 4-slot shared-memory ring, 32 pairs per slot
+//                                into an 8-slot shared-memory ring, 16 pairs per slot
 //   E   16 warps, thread = (channel, quarter tile): D2^T (TMEM lane = channel) -> e_ij = e0_ij + E_i + E_j (S:G5) ->
 //                                message: private running sums over CSR row segments, flushed at row boundaries;
 //                                head:    w_f2 . SiLU(.) reduced over channels by a fixed shuffle tree, then a
 //                                         segmented warp scan of c_ij s_ij u_ij over 32-pair granules.
+// The filter's first layer does not depend on the interaction layer: the first pair pass of a force evaluation
+// (MODE 0) also streams every tile's h1 operand image and meta record to HBM (role S, TMA bulk stores), and the later
+// passes (MODE 1: remaining message passes and the force head) replace roles P, H and the first product by one
+// loader warp (role L) that brings them back with two TMA bulk copies per tile.
 // Waiting: mbarrier try_wait does not suspend on this part (it polls, and every poll takes an issue slot from the warps
 // that have work).  So per role ONE warp polls the mbarriers that tensor-core commits and TMA transactions complete
 // on, and releases its role's other warps through a named barrier (bar.sync blocks in hardware); the pollers sit on
@@ -52,9 +56,9 @@ constexpr int TP = 128;      // pairs per tile
 constexpr int H = 128;       // channels
 constexpr int K = 64;        // radial basis functions
 constexpr int NM = 4;        // meta ring depth (tiles)
-constexpr int NSLOT = 4;     // gather ring slots per tile (32 pairs each)
-constexpr int NTHREADS = 29 * 32;   // 4 P + 4 H + 16 E + 1 MMA + 4 G warps
-constexpr int W_MMA = 24, W_G0 = 25; // warp indices of the MMA issuer and of the first gather warp
+constexpr int NSLOT = 4;     // quarter tiles; the gather ring has two 16-pair slots per quarter
+constexpr int NTHREADS = 30 * 32;   // 4 P + 4 H + 16 E + 1 MMA + 4 G + 1 S warps
+constexpr int W_MMA = 24, W_G0 = 25, W_S = 29;   // warp indices: MMA issuer, first gather warp, tile-image store warp
 
 struct PairArgs {
     int N, periodic;
@@ -69,15 +73,19 @@ struct PairArgs {
     const void *gsrc;                     // message: XE packed bf16 (x | E << 16) [rows][128] u32; head: G fp32 [rows][128]
     const float *wf2; float bf2;
     float *m_out, *carry_m, *Fraw, *carry_f;
+    unsigned char *h1_img, *meta_img;     // per tile: A2 operand image (32 KB) and Meta, written by the first pass of a force
+                                          // evaluation and re-read by the later ones (same pairs, same h1)
 };
 
 struct Meta {
-    float w[TP];                 // cutoff weight x wscale (0 for pairs past the end of the list)
+    float w[TP];                 // cutoff weight c_ij (0 for pairs past the end of the list)
     int jrow[TP];                // global row of atom j
     int rowk[TP];                // global row of atom i | kind << 29;  -1 past the end of the list
     float u[3][TP];              // unit vector (r_i - r_j)/d  (head)
     unsigned fmask[8];           // per 16-pair chunk: bit e set = pair starts a new row segment
 };
+
+static_assert(sizeof(Meta) == 3104 && sizeof(Meta) % 16 == 0, "Meta is copied by TMA bulk copies; pimd_api.cu sizes meta_img with 3104");
 
 // shared-memory carve (offsets from a 1024-aligned base)
 constexpr int OFF_W1 = 0;                          // 16 KB
@@ -166,7 +174,7 @@ __device__ __forceinline__ void role_P(const PairArgs &a, unsigned char *S, uint
             const float inv = rsqrtf(fmaxf(d2, 1e-24f));
             dist = d2 * inv;
             ux = -f[0] * inv; uy = -f[1] * inv; uz = -f[2] * inv;
-            w = a.wscale * 0.5f * (cospif(dist * inv_rc) + 1.0f);
+            w = 0.5f * (cospif(dist * inv_rc) + 1.0f);   // c_ij alone: the record is shared by the message and head passes
             kind = seg_kind(rs, re, pg & ~(int64_t)(GP - 1), GP);
         }
         int prev = __shfl_up_sync(FULL, row, 1);
@@ -181,7 +189,7 @@ __device__ __forceinline__ void role_P(const PairArgs &a, unsigned char *S, uint
         Meta &M = meta_of(S, it);
         if (lane == 0) { M.fmask[2 * (p >> 5)] = fm & 0xFFFFu; M.fmask[2 * (p >> 5) + 1] = fm >> 16; }
         M.w[p] = w; M.jrow[p] = jrow; M.rowk[p] = (row < 0) ? -1 : (row | (kind << 29));
-        if (HEAD) { M.u[0][p] = ux; M.u[1][p] = uy; M.u[2][p] = uz; }
+        M.u[0][p] = ux; M.u[1][p] = uy; M.u[2][p] = uz;   // used by the head pass, which re-reads this record
         __syncwarp();
         if (lane == 0) tc::mbar_arrive(&bar[META_FULL + (it & (NM - 1))]);
         // ---- RBF tile -> A1 (bf16, K-major rows of 128 B, 16-byte chunks XOR-swizzled by row & 7)
@@ -266,7 +274,7 @@ __device__ __forceinline__ void msg_flush(const PairArgs &a, const MsgState &st,
 {
     if (st.cur >= 0) {
         float *dst = (st.kind == 0) ? a.m_out + (size_t)st.cur * H + c : a.carry_m + (size_t)(gidx * 2 + (st.kind - 1)) * H + c;
-        *dst = fmaf(st.be, st.s2, st.s1);
+        *dst = a.wscale * fmaf(st.be, st.s2, st.s1);     // wscale = agg_norm
     }
 }
 
@@ -293,23 +301,27 @@ __device__ __forceinline__ void role_E_msg(const PairArgs &a, unsigned char *S, 
     for (int it = 0; it < n_my; ++it, tile0 += stride) {
         const Meta &M = meta_of(S, it);
         const int64_t gidx = (tile0 >> 5) + qt;
-        if (poller) {
-            WAITED(tc::mbar_wait(&bar[META_FULL + (it & (NM - 1))], (it / NM) & 1));
-            WAITED(tc::mbar_wait(&bar[D2_FULL + (it & 1)], (it >> 1) & 1));
-        }
-        WAITED(tc::named_bar_sync(NB_E + qt, 128));
-        tc::tc_fence_after_sync();
         const uint32_t td2 = tmem + 256 + (it & 1) * 128 + lane_field;
         st.s1 = 0.f; st.s2 = 0.f;
-        {                                        // the quarter tile is one granule: its first pair always starts a segment
-            const int rk = M.rowk[qt * 32];
-            st.cur = (rk < 0) ? -1 : (rk & 0x1FFFFFFF);
-            st.kind = (rk < 0) ? 0 : (rk >> 29);
-            if (st.cur >= 0) msg_row_bias(XE, st, a.rows, b2c, c);
-        }
 #pragma unroll 1
         for (int cc = 0; cc < 2; ++cc) {
-            const int q0 = qt * 32 + cc * 16, slot = qt;
+            const int q0 = qt * 32 + cc * 16, slot = qt * 2 + cc;   // ring slot = 16 pairs
+            if (poller) {
+                if (cc == 0) {
+                    WAITED(tc::mbar_wait(&bar[META_FULL + (it & (NM - 1))], (it / NM) & 1));
+                    WAITED(tc::mbar_wait(&bar[D2_FULL + (it & 1)], (it >> 1) & 1));
+                }
+                WAITED(tc::mbar_wait(&bar[XE_FULL + slot], it & 1));   // gathered rows of this slot have landed
+            }
+            WAITED(tc::named_bar_sync(NB_E + qt, 128));
+            if (cc == 0) {
+                tc::tc_fence_after_sync();
+                // the quarter tile is one granule: its first pair always starts a segment
+                const int rk = M.rowk[qt * 32];
+                st.cur = (rk < 0) ? -1 : (rk & 0x1FFFFFFF);
+                st.kind = (rk < 0) ? 0 : (rk >> 29);
+                if (st.cur >= 0) msg_row_bias(XE, st, a.rows, b2c, c);
+            }
             float v[16];
             tc::tmem_ld16(td2 + q0, v);
             if (cc == 1) {                       // accumulator drained: hand D2 back to the MMA warp
@@ -317,11 +329,7 @@ __device__ __forceinline__ void role_E_msg(const PairArgs &a, unsigned char *S, 
                 __syncwarp();
                 if (lane == 0) tc::mbar_arrive(&bar[D2_EMPTY + (it & 1)]);
             }
-            if ((cc & 1) == 0) {                 // gathered rows of this ring slot have landed
-                if (poller) WAITED(tc::mbar_wait(&bar[XE_FULL + slot], it & 1));
-                WAITED(tc::named_bar_sync(NB_E + qt, 128));
-            }
-            const uint32_t *xr = (const uint32_t *)(S + OFF_RING + slot * 16384 + (cc & 1) * 8192) + c;
+            const uint32_t *xr = (const uint32_t *)(S + OFF_RING + slot * 8192) + c;
             float wx[16];
 #pragma unroll
             for (int e4 = 0; e4 < 4; ++e4) {
@@ -358,9 +366,7 @@ __device__ __forceinline__ void role_E_msg(const PairArgs &a, unsigned char *S, 
                     if (st.cur >= 0) msg_row_bias(XE, st, a.rows, b2c, c);
                 }
             }
-            if (cc & 1) {                        // both 16-pair chunks of this ring slot consumed
-                if (it + 1 < n_my) tc::named_bar_arrive(NB_SLOT + slot, 160);
-            }
+            if (it + 1 < n_my) tc::named_bar_arrive(NB_SLOT + slot, 160);   // slot consumed: its refill overlaps the other chunk
         }
         msg_flush(a, st, gidx, c);
         __syncwarp();
@@ -388,18 +394,21 @@ __device__ __forceinline__ void role_E_head(const PairArgs &a, unsigned char *S,
     float nx_val = 0.f;
     for (int it = 0; it < n_my; ++it, tile0 += stride) {
         const Meta &M = meta_of(S, it);
-        if (poller) {
-            WAITED(tc::mbar_wait(&bar[META_FULL + (it & (NM - 1))], (it / NM) & 1));
-            WAITED(tc::mbar_wait(&bar[D2_FULL + (it & 1)], (it >> 1) & 1));
-        }
-        WAITED(tc::named_bar_sync(NB_E + qt, 128));
-        tc::tc_fence_after_sync();
         const uint32_t td2 = tmem + 256 + (it & 1) * 128 + lane_field;
         float be = 0.f;
         int cur_row = -2;
 #pragma unroll 1
         for (int cc = 0; cc < 2; ++cc) {
-            const int q0 = qt * 32 + cc * 16, slot = qt;
+            const int q0 = qt * 32 + cc * 16, slot = qt * 2 + cc;   // ring slot = 16 pairs
+            if (poller) {
+                if (cc == 0) {
+                    WAITED(tc::mbar_wait(&bar[META_FULL + (it & (NM - 1))], (it / NM) & 1));
+                    WAITED(tc::mbar_wait(&bar[D2_FULL + (it & 1)], (it >> 1) & 1));
+                }
+                WAITED(tc::mbar_wait(&bar[XE_FULL + slot], it & 1));
+            }
+            WAITED(tc::named_bar_sync(NB_E + qt, 128));
+            if (cc == 0) tc::tc_fence_after_sync();
             float v[16];
             tc::tmem_ld16(td2 + q0, v);
             if (cc == 1) {
@@ -407,11 +416,7 @@ __device__ __forceinline__ void role_E_head(const PairArgs &a, unsigned char *S,
                 __syncwarp();
                 if (lane == 0) tc::mbar_arrive(&bar[D2_EMPTY + (it & 1)]);
             }
-            if ((cc & 1) == 0) {                 // gathered rows of this ring slot have landed
-                if (poller) WAITED(tc::mbar_wait(&bar[XE_FULL + slot], it & 1));
-                WAITED(tc::named_bar_sync(NB_E + qt, 128));
-            }
-            const float *gr = (const float *)(S + OFF_RING + slot * 16384 + (cc & 1) * 8192) + c;
+            const float *gr = (const float *)(S + OFF_RING + slot * 8192) + c;
             float gj[16];
 #pragma unroll
             for (int e = 0; e < 16; ++e) gj[e] = gr[e * H];
@@ -451,9 +456,7 @@ __device__ __forceinline__ void role_E_head(const PairArgs &a, unsigned char *S,
                     }
                 }
             }
-            if (cc & 1) {
-                if (it + 1 < n_my) tc::named_bar_arrive(NB_SLOT + slot, 160);
-            }
+            if (it + 1 < n_my) tc::named_bar_arrive(NB_SLOT + slot, 160);
             // transposing reduction over the 32 lanes (channels of this quadrant): 16 pairs -> lanes
 #pragma unroll
             for (int i = 0; i < 8; ++i) {
@@ -510,6 +513,7 @@ __device__ __forceinline__ void role_E_head(const PairArgs &a, unsigned char *S,
 }
 
 // ---- role MMA: one elected lane issues both products; completion is committed to the consumers' mbarriers
+template <int MODE>
 __device__ __forceinline__ void role_MMA(unsigned char *S, uint64_t *bar, uint32_t tmem, int n_my, int lane)
 {
     STATS_BEGIN
@@ -518,7 +522,7 @@ __device__ __forceinline__ void role_MMA(unsigned char *S, uint64_t *bar, uint32
     const uint32_t sA1 = tc::smem_u32(S + OFF_A1), sA2 = tc::smem_u32(S + OFF_A2);
     tc::mbar_wait(&bar[W_FULL], 0);
     for (int k = 0; k <= n_my; ++k) {
-        if (k < n_my) {                          // D1[s] = G (W_e1/2)^T   (4 x UMMA 128x128x16)
+        if (MODE == 0 && k < n_my) {             // D1[s] = G (W_e1/2)^T   (4 x UMMA 128x128x16)
             const int s = k & 1, ph = (k >> 1) & 1;
             WAITED(tc::mbar_wait(&bar[D1_EMPTY + s], ph ^ 1));
             WAITED(tc::mbar_wait(&bar[A1_FULL + s], ph));
@@ -554,26 +558,75 @@ __device__ __forceinline__ void role_MMA(unsigned char *S, uint64_t *bar, uint32
     STATS_END("MMA")
 }
 
-// ---- role G: gathered rows (512 B each) -> ring slots by TMA bulk copies.  Warp g feeds slot g: one copy per lane
-// per tile (the copy instruction issues from the uniform datapath, one lane at a time: four warps keep up, one does not)
-__device__ __forceinline__ void role_G(const PairArgs &a, unsigned char *S, uint64_t *bar, int n_my, int slot, int lane)
+// ---- role G: gathered rows (512 B each) -> ring slots by TMA bulk copies.  Warp g feeds the two 16-pair slots of
+// quarter tile g, one copy per lane (the copy instruction issues from the uniform datapath, one lane at a time).  A slot
+// is refilled as soon as the E warps release it, i.e. while they work on the quarter's other slot.
+__device__ __forceinline__ void role_G(const PairArgs &a, unsigned char *S, uint64_t *bar, int n_my, int qt, int lane)
 {
     STATS_BEGIN
     const unsigned char *src = (const unsigned char *)a.gsrc;
-    unsigned char *dst = S + OFF_RING + slot * 16384 + lane * 512;
+    const int slot = qt * 2 + (lane >> 4);       // lanes 0-15 feed slot 2 qt, lanes 16-31 slot 2 qt + 1
+    unsigned char *dst = S + OFF_RING + slot * 8192 + (lane & 15) * 512;
     for (int it = 0; it < n_my; ++it) {
         const Meta &M = meta_of(S, it);
         WAITED(tc::mbar_wait(&bar[META_FULL + (it & (NM - 1))], (it / NM) & 1));
-        const int jrow = M.jrow[slot * 32 + lane];
-        if (it > 0) WAITED(tc::named_bar_sync(NB_SLOT + slot, 160));   // the four E warps of this slot's quarter tile have consumed it
-        if (lane == 0) tc::mbar_arrive_expect_tx(&bar[XE_FULL + slot], 16384);
-        __syncwarp();
-        tc::bulk_g2s(dst, src + (size_t)jrow * 512, 512, &bar[XE_FULL + slot]);
+        const int jrow = M.jrow[qt * 32 + lane];
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            if (it > 0) WAITED(tc::named_bar_sync(NB_SLOT + qt * 2 + h, 160));   // the four E warps have consumed it
+            if (lane == 16 * h) tc::mbar_arrive_expect_tx(&bar[XE_FULL + qt * 2 + h], 8192);
+            __syncwarp();
+            if ((lane >> 4) == h) tc::bulk_g2s(dst, src + (size_t)jrow * 512, 512, &bar[XE_FULL + slot]);
+        }
     }
     STATS_END("G")
 }
 
-template <bool HEAD>
+// ---- role S (MODE 0): stream every tile's h1 operand image and meta record to HBM for the later passes
+__device__ __forceinline__ void role_S(const PairArgs &a, unsigned char *S, uint64_t *bar, int n_my, int lane)
+{
+    STATS_BEGIN
+    for (int it = 0; it < n_my; ++it) {
+        const int s = it & 1;
+        const int64_t tile = (int64_t)blockIdx.x + (int64_t)it * gridDim.x;
+        WAITED(tc::mbar_wait(&bar[META_FULL + (it & (NM - 1))], (it / NM) & 1));
+        WAITED(tc::mbar_wait(&bar[A2_FULL + s], (it >> 1) & 1));
+        if (lane == 0) {
+            tc::fence_proxy_async_smem();       // generic-proxy writes of P and H (acquired above) -> async-proxy reads
+            tc::bulk_s2g(a.h1_img + tile * 32768, S + OFF_A2 + s * 32768, 32768);
+            tc::bulk_s2g(a.meta_img + tile * (int64_t)sizeof(Meta), &meta_of(S, it), (uint32_t)sizeof(Meta));
+            tc::bulk_commit();
+            tc::bulk_wait_read();               // shared-memory sources read: the buffers may be refilled
+            tc::mbar_arrive(&bar[A2_EMPTY + s]);
+            tc::mbar_arrive(&bar[META_EMPTY + (it & (NM - 1))]);
+        }
+        __syncwarp();
+    }
+    if (lane == 0) tc::bulk_wait_all();         // global writes complete before the kernel ends
+    STATS_END("S")
+}
+
+// ---- role L (MODE 1): bring the tile's h1 operand image and meta record back (two TMA bulk copies)
+__device__ __forceinline__ void role_L(const PairArgs &a, unsigned char *S, uint64_t *bar, int n_my, int lane)
+{
+    STATS_BEGIN
+    for (int it = 0; it < n_my; ++it) {
+        const int s = it & 1, m = it & (NM - 1);
+        const int64_t tile = (int64_t)blockIdx.x + (int64_t)it * gridDim.x;
+        WAITED(tc::mbar_wait(&bar[META_EMPTY + m], ((it / NM) & 1) ^ 1));
+        WAITED(tc::mbar_wait(&bar[A2_EMPTY + s], ((it >> 1) & 1) ^ 1));
+        if (lane == 0) {
+            tc::mbar_arrive_expect_tx(&bar[META_FULL + m], (uint32_t)sizeof(Meta));
+            tc::bulk_g2s(&meta_of(S, it), a.meta_img + tile * (int64_t)sizeof(Meta), (uint32_t)sizeof(Meta), &bar[META_FULL + m]);
+            tc::mbar_arrive_expect_tx(&bar[A2_FULL + s], 32768);
+            tc::bulk_g2s(S + OFF_A2 + s * 32768, a.h1_img + tile * 32768, 32768, &bar[A2_FULL + s]);
+        }
+        __syncwarp();
+    }
+    STATS_END("L")
+}
+
+template <bool HEAD, int MODE>
 __global__ void __launch_bounds__(NTHREADS, 1) pair_pipe_kernel(const __grid_constant__ PairArgs a)
 {
     extern __shared__ __align__(1024) unsigned char smem_raw[];
@@ -588,11 +641,11 @@ __global__ void __launch_bounds__(NTHREADS, 1) pair_pipe_kernel(const __grid_con
         for (int s = 0; s < 2; ++s) {
             tc::mbar_init(&bar[A1_FULL + s], 4);  tc::mbar_init(&bar[A1_EMPTY + s], 1);
             tc::mbar_init(&bar[D1_FULL + s], 1);  tc::mbar_init(&bar[D1_EMPTY + s], 4);
-            tc::mbar_init(&bar[A2_FULL + s], 4);  tc::mbar_init(&bar[A2_EMPTY + s], 1);
+            tc::mbar_init(&bar[A2_FULL + s], MODE == 0 ? 4 : 1);  tc::mbar_init(&bar[A2_EMPTY + s], MODE == 0 ? 2 : 1);
             tc::mbar_init(&bar[D2_FULL + s], 1);  tc::mbar_init(&bar[D2_EMPTY + s], 16);
         }
-        for (int s = 0; s < NSLOT; ++s) { tc::mbar_init(&bar[XE_FULL + s], 1); }
-        for (int s = 0; s < NM; ++s) { tc::mbar_init(&bar[META_FULL + s], 4); tc::mbar_init(&bar[META_EMPTY + s], 16); }
+        for (int s = 0; s < 2 * NSLOT; ++s) { tc::mbar_init(&bar[XE_FULL + s], 1); }
+        for (int s = 0; s < NM; ++s) { tc::mbar_init(&bar[META_FULL + s], MODE == 0 ? 4 : 1); tc::mbar_init(&bar[META_EMPTY + s], MODE == 0 ? 17 : 16); }
         tc::mbar_init(&bar[W_FULL], 1);
         tc::fence_mbar_init();
     }
@@ -609,30 +662,33 @@ __global__ void __launch_bounds__(NTHREADS, 1) pair_pipe_kernel(const __grid_con
     tc::tc_fence_after_sync();
     const uint32_t tmem = *tmem_slot;
     if (tid == W_G0 * 32) {                        // filter weights: two TMA bulk copies of pre-swizzled bf16 images
-        tc::mbar_arrive_expect_tx(&bar[W_FULL], 16384 + 32768);
-        tc::bulk_g2s(S + OFF_W1, a.W1img, 16384, &bar[W_FULL]);
+        tc::mbar_arrive_expect_tx(&bar[W_FULL], (MODE == 0 ? 16384 : 0) + 32768);
+        if (MODE == 0) tc::bulk_g2s(S + OFF_W1, a.W1img, 16384, &bar[W_FULL]);
         tc::bulk_g2s(S + OFF_W2, a.W2img, 32768, &bar[W_FULL]);
     }
     if (warp < 4) {
-        role_P<HEAD>(a, S, bar, n_my, n_pairs, tid, lane);
+        if (MODE == 0) role_P<HEAD>(a, S, bar, n_my, n_pairs, tid, lane);
+        else if (warp == 0) role_L(a, S, bar, n_my, lane);
     } else if (warp < 8) {
-        role_H(a, S, bar, tmem, n_my, tid - 128, lane);
+        if (MODE == 0) role_H(a, S, bar, tmem, n_my, tid - 128, lane);
     } else if (warp < 24) {
         const int c = (warp & 3) * 32 + lane, qt = (warp - 8) >> 2;
         const bool poller = (warp == 9) || (warp == 14) || (warp == 19) || (warp == 20);   // one per quarter, spread over the sub-partitions
         if (HEAD) role_E_head(a, S, bar, tmem, n_my, c, qt, lane, tid - 256, poller);
         else role_E_msg(a, S, bar, tmem, n_my, c, qt, lane, poller);
     } else if (warp == W_MMA) {
-        role_MMA(S, bar, tmem, n_my, lane);
-    } else {
+        role_MMA<MODE>(S, bar, tmem, n_my, lane);
+    } else if (warp < W_S) {
         role_G(a, S, bar, n_my, warp - W_G0, lane);
+    } else {
+        if (MODE == 0) role_S(a, S, bar, n_my, lane);
     }
     tc::tc_fence_before_sync();
     __syncthreads();
     if (warp == W_MMA) tc::tmem_dealloc(tmem, 512);
 }
 
-int launch_pair_pipe(pimd_ctx *c, bool head)
+int launch_pair_pipe(pimd_ctx *c, bool head, bool first)
 {
     PairArgs a;
     a.N = c->N; a.periodic = c->periodic;
@@ -645,15 +701,23 @@ int launch_pair_pipe(pimd_ctx *c, bool head)
     a.gsrc = head ? (const void *)c->Gfeat : (const void *)c->XE;
     a.wf2 = c->net.wf2; a.bf2 = c->net.bf2;
     a.m_out = c->mfeat; a.carry_m = c->carry_m; a.Fraw = c->Fraw; a.carry_f = c->carry_f;
+    a.h1_img = c->h1_img; a.meta_img = c->meta_img;
     const size_t smem = SMEM_BYTES + 1024;
     static bool attr = false;
     if (!attr) {
-        PIMD_CUDA_CHECK(cudaFuncSetAttribute(pair_pipe_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        PIMD_CUDA_CHECK(cudaFuncSetAttribute(pair_pipe_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        PIMD_CUDA_CHECK(cudaFuncSetAttribute(pair_pipe_kernel<false, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        PIMD_CUDA_CHECK(cudaFuncSetAttribute(pair_pipe_kernel<false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        PIMD_CUDA_CHECK(cudaFuncSetAttribute(pair_pipe_kernel<true, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        PIMD_CUDA_CHECK(cudaFuncSetAttribute(pair_pipe_kernel<true, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr = true;
     }
-    if (head) pair_pipe_kernel<true><<<c->num_sms, NTHREADS, smem, c->stream>>>(a);
-    else pair_pipe_kernel<false><<<c->num_sms, NTHREADS, smem, c->stream>>>(a);
+    if (head) {
+        if (first) pair_pipe_kernel<true, 0><<<c->num_sms, NTHREADS, smem, c->stream>>>(a);
+        else pair_pipe_kernel<true, 1><<<c->num_sms, NTHREADS, smem, c->stream>>>(a);
+    } else {
+        if (first) pair_pipe_kernel<false, 0><<<c->num_sms, NTHREADS, smem, c->stream>>>(a);
+        else pair_pipe_kernel<false, 1><<<c->num_sms, NTHREADS, smem, c->stream>>>(a);
+    }
     c->launches++;
     PIMD_CUDA_CHECK(cudaGetLastError());
     return 0;

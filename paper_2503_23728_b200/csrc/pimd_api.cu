@@ -61,7 +61,7 @@ namespace {
 struct Layout {
     size_t q, p, F, species, mass, C, CT, omega, err, est_partial, est_out;
     size_t cell_id, cell_count, cell_start, cell_cursor, sorted_atom, sorted_q, nnz, hits, row_ptr, block_sums, col, pair_row;
-    size_t wimg, wimg_node, xs0, weights, nfeat, xfeat, mfeat, Efeat, Gfeat, carry_m, carry_f, Fraw;
+    size_t wimg, wimg_node, xs0, h1_img, meta_img, weights, nfeat, xfeat, mfeat, Efeat, Gfeat, carry_m, carry_f, Fraw;
     size_t total;
     int ncell[3], nct;
     int64_t pair_cap, n_gran_m, n_gran_f, n_wfloats;
@@ -172,6 +172,11 @@ int compute_layout(int N, int R, int P, const double box[3], const pimd_net_para
         L->wimg = take(cur, 5 * 16384);   // bf16 UMMA images: W_e1 (16 KB), W_e2 (32 KB), W_f1 W_e2 (32 KB)
         L->wimg_node = take(cur, (size_t)(net->n_layers > 0 ? net->n_layers : 1) * 5 * 32768);
         L->xs0 = take(cur, sizeof(float) * (size_t)net->n_species * H);
+        if (net->gemm_dtype == 1 && net->n_rbf == 64 && H == 128) {   // tile images of the tcgen05 pair pipeline
+            const size_t n_tiles = (size_t)(L->pair_cap / 128 + 1);
+            L->h1_img = take(cur, n_tiles * 32768);
+            L->meta_img = take(cur, n_tiles * 3104);
+        }
         L->nfeat = take(cur, sizeof(float) * rows * H);
         L->xfeat = take(cur, sizeof(float) * rows * H);
         L->mfeat = take(cur, sizeof(float) * rows * H);
@@ -431,6 +436,7 @@ extern "C" int pimd_create(pimd_ctx **out, int n_atoms, int n_replicas, const in
             // atom-wise layers: five images per layer; SiLU's 1/2 folded into W_vn, W_vm
             c->wimg_node = (uint16_t *)(ws + L.wimg_node); c->xs0 = (float *)(ws + L.xs0);
             c->XE = (uint32_t *)c->xfeat;
+            c->h1_img = (unsigned char *)(ws + L.h1_img); c->meta_img = (unsigned char *)(ws + L.meta_img);
             for (int k = 0; k < H && k < 128; ++k) c->h_be1_half[k] = 0.5f * raw.be1[k];
             const int Ln = net->n_layers;
             wimg_node.resize((size_t)(Ln > 0 ? Ln : 1) * 5 * 16384);

@@ -56,7 +56,7 @@ def test_workspace_bytes_host_only(lib):
     n = C.c_size_t()
     box = np.ascontiguousarray(w.box)
     rc = lib.pimd_workspace_bytes(w.n_atoms, 1, w.P, box.ctypes.data_as(C.POINTER(C.c_double)), C.byref(npar), C.byref(n))
-    assert rc == 0 and 100e6 < n.value < 2e9
+    assert rc == 0 and 100e6 < n.value < 8e9   # incl. the tile images the tcgen05 pair passes keep (pair capacity x 280 B)
     bad = np.array([5.0, 5.0, 5.0])
     rc = lib.pimd_workspace_bytes(w.n_atoms, 1, w.P, bad.ctypes.data_as(C.POINTER(C.c_double)), C.byref(npar), C.byref(n))
     assert rc == -1 and b"r_cut" in lib.pimd_last_error()
