@@ -67,6 +67,7 @@ struct PairArgs {
     const int *row_ptr, *col, *pair_row;
     int64_t rows;
     const double *q;
+    const uint16_t *Wf2img;               // head: bf16 UMMA image of w_f2 replicated on 16 rows ([16][128], 4 KB)
     const uint16_t *W1img, *W2img;        // bf16 UMMA images: 0.5 W_e1 [128][64]; W_e2 (message) or 0.5 W_f1 W_e2 (head), 2 x [128][64]
     float b1h[H];                         // b_e1 / 2 (kernel-parameter constant bank: immediate operands in role H)
     const float *b2;
@@ -97,7 +98,7 @@ constexpr int OFF_META = OFF_RING + NSLOT * 16384; // NM x sizeof(Meta)
 constexpr int OFF_BIAS = OFF_META + NM * (int)sizeof(Meta);   // b1, b2, wf2
 constexpr int OFF_S4 = OFF_BIAS + 3 * H * 4;       // head: s4[4][TP]
 constexpr int OFF_BAR = OFF_S4 + 4 * TP * 4;
-constexpr int N_BAR = 40;
+constexpr int N_BAR = 42;
 constexpr int OFF_TMEM = OFF_BAR + N_BAR * 8;
 constexpr int SMEM_BYTES = OFF_TMEM + 16;
 
@@ -106,7 +107,7 @@ enum { NB_P = 1, NB_H = 2, NB_E = 3 /* +quarter */, NB_S4 = 7, NB_SLOT = 8 /* +s
 
 // mbarrier indices
 enum { A1_FULL = 0, A1_EMPTY = 2, D1_FULL = 4, D1_EMPTY = 6, A2_FULL = 8, A2_EMPTY = 10, D2_FULL = 12, D2_EMPTY = 14,
-       XE_FULL = 16, META_FULL = 24, META_EMPTY = 28, W_FULL = 32 };
+       XE_FULL = 16, META_FULL = 24, META_EMPTY = 28, W_FULL = 32, A3_FULL = 33, A3_EMPTY = 35, D3_FULL = 37, D3_EMPTY = 39 };
 
 __device__ __forceinline__ float ex2_approx(float x)
 {
@@ -512,16 +513,156 @@ __device__ __forceinline__ void role_E_head(const PairArgs &a, unsigned char *S,
     STATS_END("Eh")
 }
 
+// ---- role E, force head with the channel reduction on the tensor core (HEAD, MODE 1):
+// act[p][c] = SiLU(W_fe h1 + b_fe + G_i + G_j)[c] is written as a bf16 K-major operand (A3); the MMA warp forms
+// D3[p][.] = act[p][:] . w_f2 (128x16x128), and role F turns s_p into forces.  No shuffles, no CTA-wide barrier.
+__device__ __forceinline__ void role_E_head_tc(const PairArgs &a, unsigned char *S, uint64_t *bar, uint32_t tmem, int n_my, int c,
+                                               int qt, int lane, bool poller)
+{
+    STATS_BEGIN
+    const float b2c = 0.5f * ((const float *)(S + OFF_BIAS))[H + c];
+    const float *__restrict__ Gf = (const float *)a.gsrc;
+    const uint32_t lane_field = (uint32_t)(c & ~31) << 16;
+    const int a3_off = (c >> 6) * 16384 + (c & 7) * 2, a3_ch = (c & 63) >> 3;
+    int nx_row = -1;
+    float nx_val = 0.f;
+    for (int it = 0; it < n_my; ++it) {
+        const Meta &M = meta_of(S, it);
+        const int s3 = it & 1;
+        unsigned char *A3 = S + (s3 ? OFF_A1 : OFF_A2 + 32768) + a3_off;
+        const uint32_t td2 = tmem + 256 + (it & 1) * 128 + lane_field;
+        float be = 0.f;
+        int cur_row = -2;
+#pragma unroll 1
+        for (int cc = 0; cc < 2; ++cc) {
+            const int q0 = qt * 32 + cc * 16, slot = qt * 2 + cc;
+            if (poller) {
+                if (cc == 0) {
+                    WAITED(tc::mbar_wait(&bar[META_FULL + (it & (NM - 1))], (it / NM) & 1));
+                    WAITED(tc::mbar_wait(&bar[D2_FULL + (it & 1)], (it >> 1) & 1));
+                    WAITED(tc::mbar_wait(&bar[A3_EMPTY + s3], ((it >> 1) & 1) ^ 1));
+                }
+                WAITED(tc::mbar_wait(&bar[XE_FULL + slot], it & 1));
+            }
+            WAITED(tc::named_bar_sync(NB_E + qt, 128));
+            if (cc == 0) tc::tc_fence_after_sync();
+            float v[16];
+            tc::tmem_ld16(td2 + q0, v);
+            if (cc == 1) {
+                tc::tc_fence_before_sync();
+                __syncwarp();
+                if (lane == 0) tc::mbar_arrive(&bar[D2_EMPTY + (it & 1)]);
+            }
+            const float *gr = (const float *)(S + OFF_RING + slot * 8192) + c;
+            float gj[16];
+#pragma unroll
+            for (int e = 0; e < 16; ++e) gj[e] = gr[e * H];
+            unsigned mask = M.fmask[qt * 2 + cc];
+            if ((mask & 1u) && cc > 0) {
+                const int rk = M.rowk[q0];
+                if (((rk < 0) ? -1 : (rk & 0x1FFFFFFF)) == cur_row) mask &= ~1u;
+            }
+            if (mask == 0u) {
+#pragma unroll
+                for (int e = 0; e < 16; ++e) {
+                    const float h = fmaf(0.5f, gj[e], v[e] + be);
+                    v[e] = fmaf(h, tc::tanh_approx(h), h);
+                }
+            } else {
+                int lo = 0;
+#pragma unroll 1
+                while (true) {                   // warp-uniform: segments [lo, hi) between row boundaries
+                    const int hi = mask ? (__ffs(mask) - 1) : 16;
+#pragma unroll
+                    for (int e = 0; e < 16; ++e)
+                        if (e >= lo && e < hi) {
+                            const float h = fmaf(0.5f, gj[e], v[e] + be);
+                            v[e] = fmaf(h, tc::tanh_approx(h), h);
+                        }
+                    if (!mask) break;
+                    mask &= mask - 1;
+                    lo = hi;
+                    const int rk = M.rowk[q0 + hi];
+                    const int r = (rk < 0) ? -1 : (rk & 0x1FFFFFFF);
+                    cur_row = r;
+                    if (r >= 0) {
+                        const float raw = (r == nx_row) ? nx_val : __ldg(Gf + (size_t)r * H + c);
+                        be = b2c + 0.5f * raw;
+                        nx_row = (r + 1 < a.rows) ? r + 1 : r;
+                        nx_val = __ldg(Gf + (size_t)nx_row * H + c);
+                    }
+                }
+            }
+            if (it + 1 < n_my) tc::named_bar_arrive(NB_SLOT + slot, 160);
+            // act -> A3 (row = pair, K-major, 16-byte chunks XOR-swizzled by row & 7; (q0 + e) & 7 = e & 7)
+#pragma unroll
+            for (int e = 0; e < 16; ++e)
+                *(__nv_bfloat16 *)(A3 + (q0 + e) * 128 + ((a3_ch ^ (e & 7)) << 4)) = __float2bfloat16_rn(v[e]);
+        }
+        tc::fence_proxy_async_smem();
+        __syncwarp();
+        if (lane == 0) { tc::mbar_arrive(&bar[A3_FULL + s3]); tc::mbar_arrive(&bar[META_EMPTY + (it & (NM - 1))]); }
+    }
+    STATS_END("Et")
+}
+
+// ---- role F (HEAD, MODE 1; the four warps that are role H in the first pass): s_p from D3 -> F_i = sum_j c_ij s_ij u_ij by a
+// segmented warp scan over 32-pair granules (S:G4).  Thread p owns pair p = TMEM lane p.
+__device__ __forceinline__ void role_F(const PairArgs &a, unsigned char *S, uint64_t *bar, uint32_t tmem, int n_my, int p, int lane)
+{
+    STATS_BEGIN
+    const uint32_t lane_field = (uint32_t)(p & ~31) << 16;
+    const int64_t stride = (int64_t)gridDim.x * TP;
+    int64_t tile0 = (int64_t)blockIdx.x * TP;
+    for (int it = 0; it < n_my; ++it, tile0 += stride) {
+        const Meta &M = meta_of(S, it);
+        const int s = it & 1;
+        if ((p >> 5) == 2) {
+            WAITED(tc::mbar_wait(&bar[META_FULL + (it & (NM - 1))], (it / NM) & 1));
+            WAITED(tc::mbar_wait(&bar[D3_FULL + s], (it >> 1) & 1));
+        }
+        WAITED(tc::named_bar_sync(NB_H, 128));
+        tc::tc_fence_after_sync();
+        const float sp = tc::tmem_ld1(tmem + s * 32 + lane_field);
+        tc::tc_fence_before_sync();
+        const int rk = M.rowk[p];
+        const int key = (rk < 0) ? -1 : (rk & 0x1FFFFFFF);
+        const float f = M.w[p] * (sp + a.bf2);
+        float fv[3] = {f * M.u[0][p], f * M.u[1][p], f * M.u[2][p]};
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int ko = __shfl_up_sync(FULL, key, o);
+#pragma unroll
+            for (int ax = 0; ax < 3; ++ax) {
+                const float vo = __shfl_up_sync(FULL, fv[ax], o);
+                if (lane >= o && ko == key) fv[ax] += vo;
+            }
+        }
+        const int knext = __shfl_down_sync(FULL, key, 1);
+        if (key >= 0 && (lane == 31 || knext != key)) {
+            const int kind = rk >> 29;
+            const int64_t gidx = (tile0 + (p & ~31)) >> 5;
+            float *dst = (kind == 0) ? a.Fraw + (size_t)key * 4 : a.carry_f + (size_t)(gidx * 2 + (kind - 1)) * 4;
+            dst[0] = fv[0]; dst[1] = fv[1]; dst[2] = fv[2];
+        }
+        __syncwarp();
+        if (lane == 0) { tc::mbar_arrive(&bar[D3_EMPTY + s]); tc::mbar_arrive(&bar[META_EMPTY + (it & (NM - 1))]); }
+    }
+    STATS_END("F")
+}
+
 // ---- role MMA: one elected lane issues both products; completion is committed to the consumers' mbarriers
-template <int MODE>
+template <bool HEAD, int MODE>
 __device__ __forceinline__ void role_MMA(unsigned char *S, uint64_t *bar, uint32_t tmem, int n_my, int lane)
 {
     STATS_BEGIN
-    const uint32_t idesc = tc::make_idesc_bf16(TP, H);
+    constexpr bool TCH = HEAD && MODE == 1;      // head with the channel reduction on the tensor core
+    constexpr int NA2 = TCH ? 1 : 2;             // A2 stages (the second stage's space is an A3 stage there)
+    const uint32_t idesc = tc::make_idesc_bf16(TP, H), idesc16 = tc::make_idesc_bf16(TP, 16);
     const uint32_t sW1 = tc::smem_u32(S + OFF_W1), sW2 = tc::smem_u32(S + OFF_W2);
     const uint32_t sA1 = tc::smem_u32(S + OFF_A1), sA2 = tc::smem_u32(S + OFF_A2);
     tc::mbar_wait(&bar[W_FULL], 0);
-    for (int k = 0; k <= n_my; ++k) {
+    for (int k = 0; k <= n_my + (TCH ? 1 : 0); ++k) {
         if (MODE == 0 && k < n_my) {             // D1[s] = G (W_e1/2)^T   (4 x UMMA 128x128x16)
             const int s = k & 1, ph = (k >> 1) & 1;
             WAITED(tc::mbar_wait(&bar[D1_EMPTY + s], ph ^ 1));
@@ -537,20 +678,36 @@ __device__ __forceinline__ void role_MMA(unsigned char *S, uint64_t *bar, uint32
             }
             __syncwarp();
         }
-        if (k >= 1) {                            // D2[s]^T = W2 h1^T   (8 x UMMA; M = channels, N = pairs)
-            const int j = k - 1, s = j & 1, ph = (j >> 1) & 1;
+        if (k >= 1 && k <= n_my) {               // D2[s]^T = W2 h1^T   (8 x UMMA; M = channels, N = pairs)
+            const int j = k - 1, s = j & 1, ph = (j >> 1) & 1, sa = j % NA2, pha = (j / NA2) & 1;
             WAITED(tc::mbar_wait(&bar[D2_EMPTY + s], ph ^ 1));
-            WAITED(tc::mbar_wait(&bar[A2_FULL + s], ph));
+            WAITED(tc::mbar_wait(&bar[A2_FULL + sa], pha));
             tc::tc_fence_after_sync();
             if (lane == 0) {
 #pragma unroll
                 for (int kk = 0; kk < H / 16; ++kk) {
                     const uint32_t off = (kk >> 2) * 16384 + (kk & 3) * 32;
                     tc::mma_bf16_ss(tmem + 256 + s * 128, tc::make_desc_sw128(sW2 + off),
-                                    tc::make_desc_sw128(sA2 + s * 32768 + off), idesc, kk > 0);
+                                    tc::make_desc_sw128(sA2 + sa * 32768 + off), idesc, kk > 0);
                 }
                 tc::mma_commit(&bar[D2_FULL + s]);
-                tc::mma_commit(&bar[A2_EMPTY + s]);
+                tc::mma_commit(&bar[A2_EMPTY + sa]);
+            }
+            __syncwarp();
+        }
+        if (TCH && k >= 2) {                     // D3[s][p][0..15] = act[p][:] . w_f2   (8 x UMMA 128x16x16; M = pairs)
+            const int i = k - 2, s = i & 1, ph = (i >> 1) & 1;
+            WAITED(tc::mbar_wait(&bar[D3_EMPTY + s], ph ^ 1));
+            WAITED(tc::mbar_wait(&bar[A3_FULL + s], ph));
+            tc::tc_fence_after_sync();
+            if (lane == 0) {
+                const uint32_t sA3 = s ? sA1 : sA2 + 32768;
+#pragma unroll
+                for (int kk = 0; kk < H / 16; ++kk)
+                    tc::mma_bf16_ss(tmem + s * 32, tc::make_desc_sw128(sA3 + (kk >> 2) * 16384 + (kk & 3) * 32),
+                                    tc::make_desc_sw128(sW1 + (kk >> 2) * 2048 + (kk & 3) * 32), idesc16, kk > 0);
+                tc::mma_commit(&bar[D3_FULL + s]);
+                tc::mma_commit(&bar[A3_EMPTY + s]);
             }
             __syncwarp();
         }
@@ -607,14 +764,15 @@ __device__ __forceinline__ void role_S(const PairArgs &a, unsigned char *S, uint
 }
 
 // ---- role L (MODE 1): bring the tile's h1 operand image and meta record back (two TMA bulk copies)
+template <int NA2>
 __device__ __forceinline__ void role_L(const PairArgs &a, unsigned char *S, uint64_t *bar, int n_my, int lane)
 {
     STATS_BEGIN
     for (int it = 0; it < n_my; ++it) {
-        const int s = it & 1, m = it & (NM - 1);
+        const int s = it % NA2, m = it & (NM - 1);
         const int64_t tile = (int64_t)blockIdx.x + (int64_t)it * gridDim.x;
         WAITED(tc::mbar_wait(&bar[META_EMPTY + m], ((it / NM) & 1) ^ 1));
-        WAITED(tc::mbar_wait(&bar[A2_EMPTY + s], ((it >> 1) & 1) ^ 1));
+        WAITED(tc::mbar_wait(&bar[A2_EMPTY + s], ((it / NA2) & 1) ^ 1));
         if (lane == 0) {
             tc::mbar_arrive_expect_tx(&bar[META_FULL + m], (uint32_t)sizeof(Meta));
             tc::bulk_g2s(&meta_of(S, it), a.meta_img + tile * (int64_t)sizeof(Meta), (uint32_t)sizeof(Meta), &bar[META_FULL + m]);
@@ -641,11 +799,13 @@ __global__ void __launch_bounds__(NTHREADS, 1) pair_pipe_kernel(const __grid_con
         for (int s = 0; s < 2; ++s) {
             tc::mbar_init(&bar[A1_FULL + s], 4);  tc::mbar_init(&bar[A1_EMPTY + s], 1);
             tc::mbar_init(&bar[D1_FULL + s], 1);  tc::mbar_init(&bar[D1_EMPTY + s], 4);
+            tc::mbar_init(&bar[A3_FULL + s], 16); tc::mbar_init(&bar[A3_EMPTY + s], 1);
+            tc::mbar_init(&bar[D3_FULL + s], 1);  tc::mbar_init(&bar[D3_EMPTY + s], 4);
             tc::mbar_init(&bar[A2_FULL + s], MODE == 0 ? 4 : 1);  tc::mbar_init(&bar[A2_EMPTY + s], MODE == 0 ? 2 : 1);
             tc::mbar_init(&bar[D2_FULL + s], 1);  tc::mbar_init(&bar[D2_EMPTY + s], 16);
         }
         for (int s = 0; s < 2 * NSLOT; ++s) { tc::mbar_init(&bar[XE_FULL + s], 1); }
-        for (int s = 0; s < NM; ++s) { tc::mbar_init(&bar[META_FULL + s], MODE == 0 ? 4 : 1); tc::mbar_init(&bar[META_EMPTY + s], MODE == 0 ? 17 : 16); }
+        for (int s = 0; s < NM; ++s) { tc::mbar_init(&bar[META_FULL + s], MODE == 0 ? 4 : 1); tc::mbar_init(&bar[META_EMPTY + s], MODE == 0 ? 17 : (HEAD ? 20 : 16)); }
         tc::mbar_init(&bar[W_FULL], 1);
         tc::fence_mbar_init();
     }
@@ -662,22 +822,25 @@ __global__ void __launch_bounds__(NTHREADS, 1) pair_pipe_kernel(const __grid_con
     tc::tc_fence_after_sync();
     const uint32_t tmem = *tmem_slot;
     if (tid == W_G0 * 32) {                        // filter weights: two TMA bulk copies of pre-swizzled bf16 images
-        tc::mbar_arrive_expect_tx(&bar[W_FULL], (MODE == 0 ? 16384 : 0) + 32768);
+        tc::mbar_arrive_expect_tx(&bar[W_FULL], (MODE == 0 ? 16384 : (HEAD ? 4096 : 0)) + 32768);
         if (MODE == 0) tc::bulk_g2s(S + OFF_W1, a.W1img, 16384, &bar[W_FULL]);
+        else if (HEAD) tc::bulk_g2s(S + OFF_W1, a.Wf2img, 4096, &bar[W_FULL]);   // w_f2 operand of the readout product
         tc::bulk_g2s(S + OFF_W2, a.W2img, 32768, &bar[W_FULL]);
     }
     if (warp < 4) {
         if (MODE == 0) role_P<HEAD>(a, S, bar, n_my, n_pairs, tid, lane);
-        else if (warp == 0) role_L(a, S, bar, n_my, lane);
+        else if (warp == 0) role_L<(HEAD ? 1 : 2)>(a, S, bar, n_my, lane);
     } else if (warp < 8) {
         if (MODE == 0) role_H(a, S, bar, tmem, n_my, tid - 128, lane);
+        else if (HEAD) role_F(a, S, bar, tmem, n_my, tid - 128, lane);
     } else if (warp < 24) {
         const int c = (warp & 3) * 32 + lane, qt = (warp - 8) >> 2;
         const bool poller = (warp == 9) || (warp == 14) || (warp == 19) || (warp == 20);   // one per quarter, spread over the sub-partitions
-        if (HEAD) role_E_head(a, S, bar, tmem, n_my, c, qt, lane, tid - 256, poller);
+        if (HEAD && MODE == 1) role_E_head_tc(a, S, bar, tmem, n_my, c, qt, lane, poller);
+        else if (HEAD) role_E_head(a, S, bar, tmem, n_my, c, qt, lane, tid - 256, poller);
         else role_E_msg(a, S, bar, tmem, n_my, c, qt, lane, poller);
     } else if (warp == W_MMA) {
-        role_MMA<MODE>(S, bar, tmem, n_my, lane);
+        role_MMA<HEAD, MODE>(S, bar, tmem, n_my, lane);
     } else if (warp < W_S) {
         role_G(a, S, bar, n_my, warp - W_G0, lane);
     } else {
@@ -695,7 +858,7 @@ int launch_pair_pipe(pimd_ctx *c, bool head, bool first)
     for (int k = 0; k < 3; ++k) { a.box[k] = c->box[k]; a.inv_box[k] = c->periodic ? 1.0 / c->box[k] : 0.0; }
     a.r_cut = c->net.r_cut; a.wscale = head ? 1.0f : c->net.agg_norm;
     a.row_ptr = c->nl.row_ptr; a.col = c->nl.col; a.pair_row = c->nl.pair_row; a.rows = c->rows; a.q = c->q;
-    a.W1img = c->wimg_e1; a.W2img = head ? c->wimg_fe : c->wimg_e2;
+    a.W1img = c->wimg_e1; a.W2img = head ? c->wimg_fe : c->wimg_e2; a.Wf2img = c->wimg_wf2;
     for (int k = 0; k < H; ++k) a.b1h[k] = c->h_be1_half[k];
     a.b2 = head ? c->net.bfe : c->net.be2;
     a.gsrc = head ? (const void *)c->Gfeat : (const void *)c->XE;

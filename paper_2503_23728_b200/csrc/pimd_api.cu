@@ -169,7 +169,7 @@ int compute_layout(int N, int R, int P, const double box[3], const pimd_net_para
         L->col = take(cur, sizeof(int) * L->pair_cap);
         L->pair_row = take(cur, sizeof(int) * L->pair_cap);
         L->weights = take(cur, sizeof(float) * L->n_wfloats);
-        L->wimg = take(cur, 5 * 16384);   // bf16 UMMA images: W_e1 (16 KB), W_e2 (32 KB), W_f1 W_e2 (32 KB)
+        L->wimg = take(cur, 5 * 16384 + 4096);   // bf16 UMMA images: W_e1 (16 KB), W_e2 (32 KB), W_f1 W_e2 (32 KB)
         L->wimg_node = take(cur, (size_t)(net->n_layers > 0 ? net->n_layers : 1) * 5 * 32768);
         L->xs0 = take(cur, sizeof(float) * (size_t)net->n_species * H);
         if (net->gemm_dtype == 1 && net->n_rbf == 64 && H == 128) {   // tile images of the tcgen05 pair pipeline
@@ -426,12 +426,18 @@ extern "C" int pimd_create(pimd_ctx **out, int n_atoms, int n_replicas, const in
         c->use_tc = (net->gemm_dtype == 1 && net->n_rbf == 64 && net->hidden == 128) ? 1 : 0;
         c->wimg_e1 = (uint16_t *)(ws + L.wimg); c->wimg_e2 = c->wimg_e1 + 8192; c->wimg_fe = c->wimg_e2 + 16384;
         if (c->use_tc) {
-            wimg.resize(5 * 8192);
+            wimg.resize(5 * 8192 + 2048);
             const float *We1 = net->weights + (size_t)net->n_species * H;          // [H][K]
             const float *We2 = We1 + (size_t)H * net->n_rbf + H;                   // [H][H]
             build_umma_image(We1, H, net->n_rbf, 0.5f, wimg.data());   // SiLU(x) = h tanh(h) + h, h = x/2
             build_umma_image(We2, H, H, 1.0f, wimg.data() + 8192);
             build_umma_image(Wfe.data(), H, H, 0.5f, wimg.data() + 8192 + 16384);
+            {   // w_f2 on 16 identical rows: B operand of the head's 128x16x128 readout product
+                std::vector<float> rep((size_t)16 * H);
+                for (int r = 0; r < 16; ++r) for (int k = 0; k < H; ++k) rep[(size_t)r * H + k] = raw.wf2[k];
+                build_umma_image(rep.data(), 16, H, 1.0f, wimg.data() + 5 * 8192);
+            }
+            c->wimg_wf2 = c->wimg_e1 + 5 * 8192;
             CREATE_CHECK(cudaMemcpyAsync(c->wimg_e1, wimg.data(), sizeof(uint16_t) * wimg.size(), cudaMemcpyHostToDevice, st));
             // atom-wise layers: five images per layer; SiLU's 1/2 folded into W_vn, W_vm
             c->wimg_node = (uint16_t *)(ws + L.wimg_node); c->xs0 = (float *)(ws + L.xs0);
