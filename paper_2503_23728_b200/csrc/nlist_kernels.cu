@@ -1,8 +1,8 @@
 // nlist_kernels.cu -- per-bead-system periodic cell list -> CSR pair list (rows a1-a3 of SURVEY 8(a)).
 //
 // bin (wrapped fraction -> cell) -> counting sort (histogram, per-system exclusive scan, scatter of
-// atom index + fp64 position into cell order) -> warp-per-row stencil scan that counts the hits and
-// parks them in a fixed-stride scratch row -> row_ptr scan -> fill with an in-shared-memory rank sort
+// atom index + fp64 position into cell order) -> one CTA per cell stages its 3x3x3 stencil in shared memory, a warp per
+// home atom counts the hits and parks them in a fixed-stride scratch row -> row_ptr scan -> fill with an in-shared-memory rank sort
 // so that every CSR row lists j ascending.  The inclusion test is
 // the fp64 sequence of S:L3 written with explicit round-to-nearest intrinsics (no FMA contraction), so
 // the list is bit-identical to the oracle's.  Integer atomics only order the scatter inside a cell;
@@ -142,64 +142,99 @@ __device__ __forceinline__ bool within_cutoff_fast(const double qi[3], const dou
     return within_cutoff(qi, qj, a);
 }
 
-// Walks the de-duplicated 3x3x3 stencil of `row` with one warp.  FILL = false: returns the hit count.
-// FILL = true: also stores the hit atom indices in buf (capacity PIMD_MAX_NBR), unsorted.
-template <bool FILL>
-__device__ __forceinline__ int stencil_scan(const NlArgs &a, int64_t row, int *buf, int cap)
+// fp32 pre-filter + exact S:L3 test, candidate position given as three doubles
+__device__ __forceinline__ bool within_cutoff_fast3(const double qi[3], double xj, double yj, double zj, const NlArgs &a)
 {
-    const int lane = threadIdx.x & 31;
-    const int sys = (int)(row / a.N), i = (int)(row - (int64_t)sys * a.N);
-    double qi[3] = {a.q[row * 3], a.q[row * 3 + 1], a.q[row * 3 + 2]};
-    int cell = a.d.cell_id[row];
-    int cc[3];
-    cc[2] = cell % a.nc[2]; cc[1] = (cell / a.nc[2]) % a.nc[1]; cc[0] = cell / (a.nc[2] * a.nc[1]);
-    int lst[3][3], cnt[3];
-#pragma unroll
-    for (int ax = 0; ax < 3; ++ax) {
-        cnt[ax] = 0;
-        for (int o = -1; o <= 1; ++o) {
-            int c = cc[ax] + o;
-            if (a.periodic) c = ((c % a.nc[ax]) + a.nc[ax]) % a.nc[ax];
-            else if (c < 0 || c >= a.nc[ax]) continue;
-            bool dup = false;
-            for (int t = 0; t < cnt[ax]; ++t) dup |= (lst[ax][t] == c);
-            if (!dup) lst[ax][cnt[ax]++] = c;
-        }
-    }
-    const int *start = a.d.cell_start + (size_t)sys * (a.nct + 1);
-    const int64_t sbase = (int64_t)sys * a.N;
-    int total = 0;
-    for (int ix = 0; ix < cnt[0]; ++ix)
-        for (int iy = 0; iy < cnt[1]; ++iy)
-            for (int iz = 0; iz < cnt[2]; ++iz) {
-                int c = (lst[0][ix] * a.nc[1] + lst[1][iy]) * a.nc[2] + lst[2][iz];
-                int s0 = start[c], s1 = start[c + 1];
-                for (int s = s0 + lane; s - lane < s1; s += 32) {
-                    bool hit = false;
-                    int j = -1;
-                    if (s < s1) {
-                        j = a.d.sorted_atom[sbase + s];
-                        hit = (j != i) && within_cutoff_fast(qi, a.d.sorted_q + (sbase + s) * 3, a);
-                    }
-                    unsigned m = __ballot_sync(0xffffffffu, hit);
-                    if (FILL && hit) {
-                        int idx = total + __popc(m & ((1u << lane) - 1u));
-                        if (idx < cap) buf[idx] = j;
-                    }
-                    total += __popc(m);
-                }
-            }
-    return total;
+    const double qj[3] = {xj, yj, zj};
+    return within_cutoff_fast(qi, qj, a);
 }
 
-__global__ void __launch_bounds__(256) count_kernel(NlArgs a)
+// One CTA per (bead-system, cell).  The atoms of the cell's de-duplicated 3x3x3 stencil are staged in shared memory
+// once (index + fp64 position, CAND_CHUNK at a time) and every atom of the home cell is tested against them by one warp:
+// the candidates are read from HBM/L2 once per cell instead of once per row.  Hits are parked, unsorted, in the row's
+// fixed-stride scratch; the row's running count lives in nnz[] between chunks.
+constexpr int CAND_CHUNK = 1024, COUNT_THREADS = 128;
+
+__global__ void __launch_bounds__(COUNT_THREADS) count_cell_kernel(NlArgs a)
 {
-    int64_t row = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
-    if (row >= a.rows) return;
-    int n = stencil_scan<true>(a, row, a.d.hits + row * a.hit_stride, a.hit_stride);
-    if ((threadIdx.x & 31) == 0) {
-        if (n > a.hit_stride) { atomicOr(a.err, PIMD_FLAG_PAIRS); n = a.hit_stride; }
-        a.d.nnz[row] = n;
+    __shared__ double sq[3][CAND_CHUNK];
+    __shared__ int sj[CAND_CHUNK];
+    __shared__ int cfirst[28], cpre[28];       // first sorted position (relative to the system) and prefix count per stencil cell
+    __shared__ int n_st;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int sys = blockIdx.x / a.nct, cell = blockIdx.x - sys * a.nct;
+    const int *start = a.d.cell_start + (size_t)sys * (a.nct + 1);
+    const int h0 = start[cell], nh = start[cell + 1] - h0;
+    if (nh == 0) return;                       // uniform: every row belongs to exactly one (non-empty) cell
+    const int64_t sbase = (int64_t)sys * a.N;
+    if (tid == 0) {
+        int cc[3];
+        cc[2] = cell % a.nc[2]; cc[1] = (cell / a.nc[2]) % a.nc[1]; cc[0] = cell / (a.nc[2] * a.nc[1]);
+        int lst[3][3], cnt[3];
+        for (int ax = 0; ax < 3; ++ax) {
+            cnt[ax] = 0;
+            for (int o = -1; o <= 1; ++o) {
+                int c = cc[ax] + o;
+                if (a.periodic) c = ((c % a.nc[ax]) + a.nc[ax]) % a.nc[ax];
+                else if (c < 0 || c >= a.nc[ax]) continue;
+                bool dup = false;
+                for (int t = 0; t < cnt[ax]; ++t) dup |= (lst[ax][t] == c);
+                if (!dup) lst[ax][cnt[ax]++] = c;
+            }
+        }
+        int k = 0, tot = 0;
+        for (int ix = 0; ix < cnt[0]; ++ix)
+            for (int iy = 0; iy < cnt[1]; ++iy)
+                for (int iz = 0; iz < cnt[2]; ++iz) {
+                    const int c = (lst[0][ix] * a.nc[1] + lst[1][iy]) * a.nc[2] + lst[2][iz];
+                    cfirst[k] = start[c]; cpre[k] = tot;
+                    tot += start[c + 1] - start[c];
+                    ++k;
+                }
+        cpre[k] = tot;
+        n_st = k;
+    }
+    __syncthreads();
+    const int total = cpre[n_st];
+    for (int base = 0; base < total; base += CAND_CHUNK) {
+        const int n = min(CAND_CHUNK, total - base);
+        for (int t = tid; t < n; t += COUNT_THREADS) {
+            const int idx = base + t;
+            int k = 0;
+            while (idx >= cpre[k + 1]) ++k;    // <= 27 steps
+            const int64_t pos = sbase + cfirst[k] + (idx - cpre[k]);
+            sj[t] = a.d.sorted_atom[pos];
+            sq[0][t] = a.d.sorted_q[pos * 3 + 0]; sq[1][t] = a.d.sorted_q[pos * 3 + 1]; sq[2][t] = a.d.sorted_q[pos * 3 + 2];
+        }
+        __syncthreads();
+        const bool last = base + CAND_CHUNK >= total;
+        for (int ha = warp; ha < nh; ha += COUNT_THREADS / 32) {
+            const int64_t posi = sbase + h0 + ha;
+            const int i = a.d.sorted_atom[posi];
+            const int64_t row = sbase + i;
+            const double qi[3] = {a.d.sorted_q[posi * 3], a.d.sorted_q[posi * 3 + 1], a.d.sorted_q[posi * 3 + 2]};
+            int *buf = a.d.hits + row * a.hit_stride;
+            int cnt_i = (base == 0) ? 0 : a.d.nnz[row];
+            for (int s = lane; s - lane < n; s += 32) {
+                bool hit = false;
+                int j = -1;
+                if (s < n) {
+                    j = sj[s];
+                    hit = (j != i) && within_cutoff_fast3(qi, sq[0][s], sq[1][s], sq[2][s], a);
+                }
+                const unsigned m = __ballot_sync(0xffffffffu, hit);
+                if (hit) {
+                    const int idx = cnt_i + __popc(m & ((1u << lane) - 1u));
+                    if (idx < a.hit_stride) buf[idx] = j;
+                }
+                cnt_i += __popc(m);
+            }
+            if (lane == 0) {
+                if (last && cnt_i > a.hit_stride) { atomicOr(a.err, PIMD_FLAG_PAIRS); cnt_i = a.hit_stride; }
+                a.d.nnz[row] = cnt_i;
+            }
+        }
+        __syncthreads();
     }
 }
 
@@ -281,7 +316,7 @@ int pimd_launch_nlist(pimd_ctx *c)
     bin_kernel<<<gthr, 256, 0, c->stream>>>(a);
     scan_cells_kernel<<<a.nsys, 256, 0, c->stream>>>(a);
     scatter_kernel<<<gthr, 256, 0, c->stream>>>(a);
-    count_kernel<<<gwarp, 256, 0, c->stream>>>(a);
+    count_cell_kernel<<<(unsigned)(a.nsys * a.nct), COUNT_THREADS, 0, c->stream>>>(a);
     scan_rows_local_kernel<<<nblk, 1024, 0, c->stream>>>(a);
     scan_block_sums_kernel<<<1, 1024, 0, c->stream>>>(a, nblk);
     scan_rows_add_kernel<<<gthr, 256, 0, c->stream>>>(a);
