@@ -558,9 +558,19 @@ __device__ __forceinline__ void role_E_head_tc(const PairArgs &a, unsigned char 
 #pragma unroll
             for (int e = 0; e < 16; ++e) gj[e] = gr[e * H];
             unsigned mask = M.fmask[qt * 2 + cc];
-            if ((mask & 1u) && cc > 0) {
+            if (mask & 1u) {                     // granule start forced by P: a boundary for G_i only if the row changes
                 const int rk = M.rowk[q0];
-                if (((rk < 0) ? -1 : (rk & 0x1FFFFFFF)) == cur_row) mask &= ~1u;
+                const int r = (rk < 0) ? -1 : (rk & 0x1FFFFFFF);
+                if (r != cur_row) {              // handled here, so that the chunk takes the branch-free path
+                    cur_row = r;
+                    if (r >= 0) {
+                        const float raw = (r == nx_row) ? nx_val : __ldg(Gf + (size_t)r * H + c);
+                        be = b2c + 0.5f * raw;
+                        nx_row = (r + 1 < a.rows) ? r + 1 : r;
+                        nx_val = __ldg(Gf + (size_t)nx_row * H + c);
+                    }
+                }
+                mask &= ~1u;
             }
             if (mask == 0u) {
 #pragma unroll
