@@ -114,19 +114,56 @@ __global__ void __launch_bounds__(NTH, 1) node_tc_kernel(const __grid_constant__
 
     for (int tile = blockIdx.x; tile < a.n_tiles; tile += gridDim.x) {
         const int64_t row0 = (int64_t)tile * TR;
-        // ---- operands n, m (fp32 in HBM) -> bf16 swizzled tiles; one warp per row: coalesced 512-byte reads
-#pragma unroll 2
-        for (int it = 0; it < TR * H / 4 / NTH; ++it) {
-            const int idx = tid + it * NTH, rr = idx >> 5, k = (idx & 31) * 4;
-            const int64_t row = row0 + rr;
-            float4 nv = make_float4(0.f, 0.f, 0.f, 0.f), mv = nv;
-            if (row < a.rows) {
-                nv = *(const float4 *)(a.n + (size_t)row * H + k);
-                mv = assemble_m(a, row, k, n_pairs);
+        // ---- operands n, m (fp32 in HBM) -> bf16 swizzled tiles; one warp per row: coalesced 512-byte reads.
+        // m_i is assembled in fixed order from the direct row or the carry slots (tail slot of the first granule, head
+        // slots of the rest).  All loads of four rows are issued before the first use: the phase is latency-bound.
+        {
+            const int k = lane * 4, wrow = tid >> 5;
+            int rs[8], re[8];
+#pragma unroll
+            for (int it = 0; it < 8; ++it) {
+                const int64_t row = row0 + wrow + it * 16;
+                const bool ok = row < a.rows && n_pairs > 0;
+                rs[it] = ok ? __ldg(a.row_ptr + row) : 0;
+                re[it] = ok ? __ldg(a.row_ptr + row + 1) : 0;
             }
-            const int off = op_off(rr, k);
-            *(uint2 *)(A0 + off) = make_uint2(tc::pack_bf16(nv.x, nv.y), tc::pack_bf16(nv.z, nv.w));
-            *(uint2 *)(A1 + off) = make_uint2(tc::pack_bf16(mv.x, mv.y), tc::pack_bf16(mv.z, mv.w));
+#pragma unroll
+            for (int it0 = 0; it0 < 8; it0 += 4) {
+                float4 nv[4], pc[4][4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const int it = it0 + j;
+                    const int64_t row = row0 + wrow + it * 16;
+                    const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
+                    nv[j] = (row < a.rows) ? *(const float4 *)(a.n + (size_t)row * H + k) : z;
+                    pc[j][0] = pc[j][1] = pc[j][2] = pc[j][3] = z;
+                    if (re[it] > rs[it]) {       // warp-uniform
+                        const int g0 = rs[it] / a.gran_m, g1 = (re[it] - 1) / a.gran_m;
+                        if (g0 == g1) pc[j][0] = __ldg((const float4 *)(a.m + (size_t)row * H + k));
+                        else pc[j][0] = __ldg((const float4 *)(a.carry_m + ((size_t)g0 * 2 + 1) * H + k));
+#pragma unroll
+                        for (int t = 1; t < 4; ++t)
+                            if (g0 + t <= g1) pc[j][t] = __ldg((const float4 *)(a.carry_m + ((size_t)(g0 + t) * 2) * H + k));
+                    }
+                }
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const int it = it0 + j, rr = wrow + it * 16;
+                    float4 mv = pc[j][0];
+#pragma unroll
+                    for (int t = 1; t < 4; ++t) { mv.x += pc[j][t].x; mv.y += pc[j][t].y; mv.z += pc[j][t].z; mv.w += pc[j][t].w; }
+                    if (re[it] > rs[it]) {       // rows with more than four granules (very long rows): the rest, in order
+                        const int g0 = rs[it] / a.gran_m, g1 = (re[it] - 1) / a.gran_m;
+                        for (int g = g0 + 4; g <= g1; ++g) {
+                            const float4 t4 = __ldg((const float4 *)(a.carry_m + ((size_t)g * 2) * H + k));
+                            mv.x += t4.x; mv.y += t4.y; mv.z += t4.z; mv.w += t4.w;
+                        }
+                    }
+                    const int off = op_off(rr, k);
+                    *(uint2 *)(A0 + off) = make_uint2(tc::pack_bf16(nv[j].x, nv[j].y), tc::pack_bf16(nv[j].z, nv[j].w));
+                    *(uint2 *)(A1 + off) = make_uint2(tc::pack_bf16(mv.x, mv.y), tc::pack_bf16(mv.z, mv.w));
+                }
+            }
         }
         tc::fence_proxy_async_smem();
         __syncthreads();
