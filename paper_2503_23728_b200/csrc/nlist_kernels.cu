@@ -153,26 +153,31 @@ __device__ __forceinline__ bool within_cutoff_fast3(const double qi[3], double x
 // once (index + fp64 position, CAND_CHUNK at a time) and every atom of the home cell is tested against them by one warp:
 // the candidates are read from HBM/L2 once per cell instead of once per row.  Hits are parked, unsorted, in the row's
 // fixed-stride scratch; the row's running count lives in nnz[] between chunks.
-constexpr int CAND_CHUNK = 1024, COUNT_THREADS = 128;
+constexpr int CAND_CHUNK = 1024, COUNT_THREADS = 128, HOME_MAX = 128;
 
 __global__ void __launch_bounds__(COUNT_THREADS) count_cell_kernel(NlArgs a)
 {
-    __shared__ double sq[3][CAND_CHUNK];
-    __shared__ int sj[CAND_CHUNK];
+    __shared__ int sj[CAND_CHUNK], sp[CAND_CHUNK];   // candidate atom index; position in the cell-ordered arrays
     __shared__ int cfirst[28], cpre[28];       // first sorted position (relative to the system) and prefix count per stencil cell
     __shared__ int n_st;
+    __shared__ double hq[3][HOME_MAX];         // atoms of the home cell (the first HOME_MAX; the rest are read from global)
+    __shared__ int hj[HOME_MAX];
+    __shared__ float sqf[3][CAND_CHUNK];       // candidate positions relative to the cell's reference atom (minimum image), fp32
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int sys = blockIdx.x / a.nct, cell = blockIdx.x - sys * a.nct;
     const int *start = a.d.cell_start + (size_t)sys * (a.nct + 1);
     const int h0 = start[cell], nh = start[cell + 1] - h0;
     if (nh == 0) return;                       // uniform: every row belongs to exactly one (non-empty) cell
     const int64_t sbase = (int64_t)sys * a.N;
-    if (tid == 0) {
+    // stencil cells: every thread derives the de-duplicated per-axis lists; thread t < n_st loads cell t's range
+    {
         int cc[3];
         cc[2] = cell % a.nc[2]; cc[1] = (cell / a.nc[2]) % a.nc[1]; cc[0] = cell / (a.nc[2] * a.nc[1]);
         int lst[3][3], cnt[3];
+#pragma unroll
         for (int ax = 0; ax < 3; ++ax) {
             cnt[ax] = 0;
+#pragma unroll
             for (int o = -1; o <= 1; ++o) {
                 int c = cc[ax] + o;
                 if (a.periodic) c = ((c % a.nc[ax]) + a.nc[ax]) % a.nc[ax];
@@ -182,20 +187,38 @@ __global__ void __launch_bounds__(COUNT_THREADS) count_cell_kernel(NlArgs a)
                 if (!dup) lst[ax][cnt[ax]++] = c;
             }
         }
-        int k = 0, tot = 0;
-        for (int ix = 0; ix < cnt[0]; ++ix)
-            for (int iy = 0; iy < cnt[1]; ++iy)
-                for (int iz = 0; iz < cnt[2]; ++iz) {
-                    const int c = (lst[0][ix] * a.nc[1] + lst[1][iy]) * a.nc[2] + lst[2][iz];
-                    cfirst[k] = start[c]; cpre[k] = tot;
-                    tot += start[c + 1] - start[c];
-                    ++k;
-                }
-        cpre[k] = tot;
-        n_st = k;
+        const int ns = cnt[0] * cnt[1] * cnt[2];
+        if (tid < ns) {
+            const int iz = tid % cnt[2], iy = (tid / cnt[2]) % cnt[1], ix = tid / (cnt[2] * cnt[1]);
+            int cx = lst[0][0], cy = lst[1][0], cz = lst[2][0];   // dynamic index into a register array, by selection
+#pragma unroll
+            for (int t = 1; t < 3; ++t) { if (ix == t) cx = lst[0][t]; if (iy == t) cy = lst[1][t]; if (iz == t) cz = lst[2][t]; }
+            const int c = (cx * a.nc[1] + cy) * a.nc[2] + cz;
+            cfirst[tid] = start[c];
+            cpre[tid + 1] = start[c + 1] - start[c];   // counts; prefix below
+        }
+        __syncthreads();
+        if (tid == 0) {
+            int tot = 0;
+            cpre[0] = 0;
+            for (int k = 0; k < ns; ++k) { const int c = cpre[k + 1]; cpre[k] = tot; tot += c; }
+            cpre[ns] = tot;
+            n_st = ns;
+        }
+        for (int t = tid; t < nh && t < HOME_MAX; t += COUNT_THREADS) {   // home atoms
+            const int64_t posi = sbase + h0 + t;
+            hj[t] = a.d.sorted_atom[posi];
+            hq[0][t] = a.d.sorted_q[posi * 3]; hq[1][t] = a.d.sorted_q[posi * 3 + 1]; hq[2][t] = a.d.sorted_q[posi * 3 + 2];
+        }
     }
     __syncthreads();
     const int total = cpre[n_st];
+    // reference point of the cell: its first atom.  Relative fp32 coordinates are small whatever the absolute ones are.
+    const double ref[3] = {a.d.sorted_q[(sbase + h0) * 3], a.d.sorted_q[(sbase + h0) * 3 + 1], a.d.sorted_q[(sbase + h0) * 3 + 2]};
+    const float bxf[3] = {a.boxf[0], a.boxf[1], a.boxf[2]};
+    const float inf = __int_as_float(0x7f800000);
+    const float hbx[3] = {a.periodic ? 0.5f * bxf[0] : inf, a.periodic ? 0.5f * bxf[1] : inf, a.periodic ? 0.5f * bxf[2] : inf};
+    const float rc2_hi = a.rc2_hi, rc2_lo = a.rc2_lo;
     for (int base = 0; base < total; base += CAND_CHUNK) {
         const int n = min(CAND_CHUNK, total - base);
         for (int t = tid; t < n; t += COUNT_THREADS) {
@@ -204,23 +227,50 @@ __global__ void __launch_bounds__(COUNT_THREADS) count_cell_kernel(NlArgs a)
             while (idx >= cpre[k + 1]) ++k;    // <= 27 steps
             const int64_t pos = sbase + cfirst[k] + (idx - cpre[k]);
             sj[t] = a.d.sorted_atom[pos];
-            sq[0][t] = a.d.sorted_q[pos * 3 + 0]; sq[1][t] = a.d.sorted_q[pos * 3 + 1]; sq[2][t] = a.d.sorted_q[pos * 3 + 2];
+            sp[t] = (int)(pos - sbase);
+#pragma unroll
+            for (int ax = 0; ax < 3; ++ax) {
+                double d = a.d.sorted_q[pos * 3 + ax] - ref[ax];          // once per candidate and cell: fp64 image shift, then fp32
+                if (a.periodic) d -= a.box[ax] * rint(d / a.box[ax]);
+                sqf[ax][t] = (float)d;
+            }
         }
         __syncthreads();
         const bool last = base + CAND_CHUNK >= total;
         for (int ha = warp; ha < nh; ha += COUNT_THREADS / 32) {
             const int64_t posi = sbase + h0 + ha;
-            const int i = a.d.sorted_atom[posi];
+            const bool in_s = ha < HOME_MAX;     // warp-uniform
+            const int i = in_s ? hj[ha] : a.d.sorted_atom[posi];
             const int64_t row = sbase + i;
-            const double qi[3] = {a.d.sorted_q[posi * 3], a.d.sorted_q[posi * 3 + 1], a.d.sorted_q[posi * 3 + 2]};
+            const double qi[3] = {in_s ? hq[0][ha] : a.d.sorted_q[posi * 3], in_s ? hq[1][ha] : a.d.sorted_q[posi * 3 + 1],
+                                  in_s ? hq[2][ha] : a.d.sorted_q[posi * 3 + 2]};
             int *buf = a.d.hits + row * a.hit_stride;
             int cnt_i = (base == 0) ? 0 : a.d.nnz[row];
+            float qif[3];
+#pragma unroll
+            for (int ax = 0; ax < 3; ++ax) {
+                double d = qi[ax] - ref[ax];
+                if (a.periodic) d -= a.box[ax] * rint(d / a.box[ax]);
+                qif[ax] = (float)d;
+            }
             for (int s = lane; s - lane < n; s += 32) {
                 bool hit = false;
                 int j = -1;
                 if (s < n) {
                     j = sj[s];
-                    hit = (j != i) && within_cutoff_fast3(qi, sq[0][s], sq[1][s], sq[2][s], a);
+                    // fp32 estimate of d^2 from the relative coordinates (|.| <= L/2 each, so one wrap suffices): its
+                    // error is orders of magnitude below the 1e-3 band; inside the band the exact S:L3 sequence decides
+                    float d2 = 0.f;
+#pragma unroll
+                    for (int ax = 0; ax < 3; ++ax) {
+                        float dx = sqf[ax][s] - qif[ax];
+                        float sh = (dx > hbx[ax]) ? bxf[ax] : 0.f;      // selects, not branches (hbx = +inf when not periodic)
+                        sh = (dx < -hbx[ax]) ? -bxf[ax] : sh;
+                        dx -= sh;
+                        d2 = fmaf(dx, dx, d2);
+                    }
+                    if (j != i && d2 <= rc2_hi)   // in the band (about 0.2 % of the candidates): fp64 positions from global
+                        hit = (d2 < rc2_lo) || within_cutoff(qi, a.d.sorted_q + (sbase + sp[s]) * 3, a);
                 }
                 const unsigned m = __ballot_sync(0xffffffffu, hit);
                 if (hit) {
@@ -297,6 +347,48 @@ __global__ void __launch_bounds__(256) fill_kernel(NlArgs a)
     }
 }
 
+// Same result as fill_kernel without the O(n^2) rank sort: the row's hits set bits in a per-warp bitmask over the atoms of
+// the bead-system (shared memory, N/32 words), and the set bits are emitted in ascending order.  Used when N <= 32768.
+__global__ void __launch_bounds__(256) fill_bitmask_kernel(NlArgs a, int nw)
+{
+    extern __shared__ unsigned smask[];       // [8][nw]
+    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int64_t row = (int64_t)blockIdx.x * 8 + w;
+    if (row >= a.rows) return;
+    if (a.d.row_ptr[a.rows] == 0) return;     // empty or overflowed list
+    unsigned *mk = smask + (size_t)w * nw;
+    const int n = a.d.nnz[row];
+    const int *hits = a.d.hits + row * a.hit_stride;
+    const int64_t base = a.d.row_ptr[row];
+    for (int t = lane; t < nw; t += 32) mk[t] = 0u;
+    __syncwarp();
+    for (int e = lane; e < n; e += 32) {
+        const int j = hits[e];
+        atomicOr(&mk[j >> 5], 1u << (j & 31));
+    }
+    __syncwarp();
+    const int wpl = (nw + 31) >> 5, w0 = lane * wpl, w1 = min(w0 + wpl, nw);
+    int cnt = 0;
+    for (int t = w0; t < w1; ++t) cnt += __popc(mk[t]);
+    int inc = cnt;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int v = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += v;
+    }
+    int64_t pos = base + (inc - cnt);
+    for (int t = w0; t < w1; ++t) {
+        unsigned bits = mk[t];
+        while (bits) {
+            const int b = __ffs(bits) - 1;
+            a.d.col[pos] = t * 32 + b;
+            a.d.pair_row[pos] = (int)row;
+            ++pos;
+            bits &= bits - 1;
+        }
+    }
+}
+
 }  // namespace
 
 int pimd_launch_nlist(pimd_ctx *c)
@@ -320,7 +412,9 @@ int pimd_launch_nlist(pimd_ctx *c)
     scan_rows_local_kernel<<<nblk, 1024, 0, c->stream>>>(a);
     scan_block_sums_kernel<<<1, 1024, 0, c->stream>>>(a, nblk);
     scan_rows_add_kernel<<<gthr, 256, 0, c->stream>>>(a);
-    fill_kernel<<<gwarp, 256, 0, c->stream>>>(a);
+    const int nw = (c->N + 31) / 32;
+    if (nw <= 1024) fill_bitmask_kernel<<<gwarp, 256, (size_t)8 * nw * sizeof(unsigned), c->stream>>>(a, nw);
+    else fill_kernel<<<gwarp, 256, 0, c->stream>>>(a);
     c->launches += 8;
     PIMD_CUDA_CHECK(cudaGetLastError());
     return 0;
