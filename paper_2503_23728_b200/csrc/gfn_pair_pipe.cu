@@ -57,8 +57,21 @@ constexpr int H = 128;       // channels
 constexpr int K = 64;        // radial basis functions
 constexpr int NM = 4;        // meta ring depth (tiles)
 constexpr int NSLOT = 4;     // quarter tiles; the gather ring has two 16-pair slots per quarter
-constexpr int NTHREADS = 30 * 32;   // 4 P + 4 H + 16 E + 1 MMA + 4 G + 1 S warps
-constexpr int W_MMA = 24, W_G0 = 25, W_S = 29;   // warp indices: MMA issuer, first gather warp, tile-image store warp
+// Warp layout per kernel variant (fewer warps in the later passes -> more registers per thread for role E):
+//   MODE 0           : P 0-3, H 4-7, E 8-23, MMA 24, G 25-28, S 29           (30 warps, 64 registers)
+//   MODE 1, message  : E 0-15, G 16-19, MMA 20, L 21                          (22 warps, 88 registers)
+//   MODE 1, head     : E 0-15, F 16-19, G 20-23, MMA 24, L 25                 (26 warps, 72 registers)
+// E and F/H warps start at a multiple of 4: warp % 4 is the TMEM lane quadrant a warp may access.
+template <bool HEAD, int MODE>
+struct Warps {
+    static constexpr int E0 = (MODE == 0) ? 8 : 0;
+    static constexpr int F0 = (MODE == 0) ? 4 : 16;                      // H (MODE 0) or F (MODE 1 head)
+    static constexpr int G0 = (MODE == 0) ? 25 : (HEAD ? 20 : 16);
+    static constexpr int MMA = (MODE == 0) ? 24 : (HEAD ? 24 : 20);
+    static constexpr int SL = (MODE == 0) ? 29 : MMA + 1;                // S (MODE 0) or L (MODE 1)
+    static constexpr int N = SL + 1;
+    static constexpr int THREADS = N * 32;
+};
 
 struct PairArgs {
     int N, periodic;
@@ -795,8 +808,9 @@ __device__ __forceinline__ void role_L(const PairArgs &a, unsigned char *S, uint
 }
 
 template <bool HEAD, int MODE>
-__global__ void __launch_bounds__(NTHREADS, 1) pair_pipe_kernel(const __grid_constant__ PairArgs a)
+__global__ void __launch_bounds__(Warps<HEAD, MODE>::THREADS, 1) pair_pipe_kernel(const __grid_constant__ PairArgs a)
 {
+    using WL = Warps<HEAD, MODE>;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     unsigned char *S = smem_raw + ((1024u - (tc::smem_u32(smem_raw) & 1023u)) & 1023u);
     uint64_t *bar = (uint64_t *)(S + OFF_BAR);
@@ -819,10 +833,10 @@ __global__ void __launch_bounds__(NTHREADS, 1) pair_pipe_kernel(const __grid_con
         tc::mbar_init(&bar[W_FULL], 1);
         tc::fence_mbar_init();
     }
-    if (warp == W_MMA) tc::tmem_alloc(tmem_slot, 512);
+    if (warp == WL::MMA) tc::tmem_alloc(tmem_slot, 512);
     {
         float *sb = (float *)(S + OFF_BIAS);
-        for (int i = tid; i < H; i += NTHREADS) {
+        for (int i = tid; i < H; i += WL::THREADS) {
             sb[H + i] = a.b2[i];
             sb[2 * H + i] = HEAD ? a.wf2[i] : 0.f;
         }
@@ -831,34 +845,35 @@ __global__ void __launch_bounds__(NTHREADS, 1) pair_pipe_kernel(const __grid_con
     __syncthreads();
     tc::tc_fence_after_sync();
     const uint32_t tmem = *tmem_slot;
-    if (tid == W_G0 * 32) {                        // filter weights: two TMA bulk copies of pre-swizzled bf16 images
+    if (tid == WL::G0 * 32) {                        // filter weights: two TMA bulk copies of pre-swizzled bf16 images
         tc::mbar_arrive_expect_tx(&bar[W_FULL], (MODE == 0 ? 16384 : (HEAD ? 4096 : 0)) + 32768);
         if (MODE == 0) tc::bulk_g2s(S + OFF_W1, a.W1img, 16384, &bar[W_FULL]);
         else if (HEAD) tc::bulk_g2s(S + OFF_W1, a.Wf2img, 4096, &bar[W_FULL]);   // w_f2 operand of the readout product
         tc::bulk_g2s(S + OFF_W2, a.W2img, 32768, &bar[W_FULL]);
     }
-    if (warp < 4) {
-        if (MODE == 0) role_P<HEAD>(a, S, bar, n_my, n_pairs, tid, lane);
-        else if (warp == 0) role_L<(HEAD ? 1 : 2)>(a, S, bar, n_my, lane);
-    } else if (warp < 8) {
-        if (MODE == 0) role_H(a, S, bar, tmem, n_my, tid - 128, lane);
-        else if (HEAD) role_F(a, S, bar, tmem, n_my, tid - 128, lane);
-    } else if (warp < 24) {
-        const int c = (warp & 3) * 32 + lane, qt = (warp - 8) >> 2;
-        const bool poller = (warp == 9) || (warp == 14) || (warp == 19) || (warp == 20);   // one per quarter, spread over the sub-partitions
+    if (MODE == 0 && warp < 4) {
+        role_P<HEAD>(a, S, bar, n_my, n_pairs, tid, lane);
+    } else if (MODE == 0 && warp < 8) {
+        role_H(a, S, bar, tmem, n_my, tid - 128, lane);
+    } else if (warp >= WL::E0 && warp < WL::E0 + 16) {
+        const int we = warp - WL::E0, c = (we & 3) * 32 + lane, qt = we >> 2;
+        const bool poller = (we == 1) || (we == 6) || (we == 11) || (we == 12);   // one per quarter, spread over the sub-partitions
         if (HEAD && MODE == 1) role_E_head_tc(a, S, bar, tmem, n_my, c, qt, lane, poller);
-        else if (HEAD) role_E_head(a, S, bar, tmem, n_my, c, qt, lane, tid - 256, poller);
+        else if (HEAD) role_E_head(a, S, bar, tmem, n_my, c, qt, lane, tid - WL::E0 * 32, poller);
         else role_E_msg(a, S, bar, tmem, n_my, c, qt, lane, poller);
-    } else if (warp == W_MMA) {
+    } else if (HEAD && MODE == 1 && warp >= WL::F0 && warp < WL::F0 + 4) {
+        role_F(a, S, bar, tmem, n_my, tid - WL::F0 * 32, lane);
+    } else if (warp == WL::MMA) {
         role_MMA<HEAD, MODE>(S, bar, tmem, n_my, lane);
-    } else if (warp < W_S) {
-        role_G(a, S, bar, n_my, warp - W_G0, lane);
-    } else {
+    } else if (warp >= WL::G0 && warp < WL::G0 + 4) {
+        role_G(a, S, bar, n_my, warp - WL::G0, lane);
+    } else if (warp == WL::SL) {
         if (MODE == 0) role_S(a, S, bar, n_my, lane);
+        else role_L<(HEAD ? 1 : 2)>(a, S, bar, n_my, lane);
     }
     tc::tc_fence_before_sync();
     __syncthreads();
-    if (warp == W_MMA) tc::tmem_dealloc(tmem, 512);
+    if (warp == WL::MMA) tc::tmem_dealloc(tmem, 512);
 }
 
 int launch_pair_pipe(pimd_ctx *c, bool head, bool first)
@@ -885,11 +900,11 @@ int launch_pair_pipe(pimd_ctx *c, bool head, bool first)
         attr = true;
     }
     if (head) {
-        if (first) pair_pipe_kernel<true, 0><<<c->num_sms, NTHREADS, smem, c->stream>>>(a);
-        else pair_pipe_kernel<true, 1><<<c->num_sms, NTHREADS, smem, c->stream>>>(a);
+        if (first) pair_pipe_kernel<true, 0><<<c->num_sms, Warps<true, 0>::THREADS, smem, c->stream>>>(a);
+        else pair_pipe_kernel<true, 1><<<c->num_sms, Warps<true, 1>::THREADS, smem, c->stream>>>(a);
     } else {
-        if (first) pair_pipe_kernel<false, 0><<<c->num_sms, NTHREADS, smem, c->stream>>>(a);
-        else pair_pipe_kernel<false, 1><<<c->num_sms, NTHREADS, smem, c->stream>>>(a);
+        if (first) pair_pipe_kernel<false, 0><<<c->num_sms, Warps<false, 0>::THREADS, smem, c->stream>>>(a);
+        else pair_pipe_kernel<false, 1><<<c->num_sms, Warps<false, 1>::THREADS, smem, c->stream>>>(a);
     }
     c->launches++;
     PIMD_CUDA_CHECK(cudaGetLastError());
