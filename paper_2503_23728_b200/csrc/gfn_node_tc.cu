@@ -45,6 +45,10 @@ __device__ __forceinline__ int op_off(int r, int k)
     return (k >> 6) * (TR * 128) + r * 128 + ((((k & 63) >> 3) ^ (r & 7)) << 4) + (k & 7) * 2;
 }
 
+// fp32 masters n and E are private to these kernels and kept tile-blocked: [tile][c / 4][row in tile][4 floats], so that the
+// epilogue, where a thread owns a row (TMEM lane), reads and writes 512 contiguous bytes per warp instruction.
+__device__ __forceinline__ size_t blk_off(int64_t row0, int r, int c) { return ((size_t)(row0 >> 7) * (H / 4) + (c >> 2)) * (TR * 4) + (size_t)r * 4 + (c & 3); }
+
 __device__ __forceinline__ float4 assemble_m(const Args &a, int64_t row, int c0, int n_pairs)
 {
     const int rs = a.row_ptr[row], re = a.row_ptr[row + 1];
@@ -135,7 +139,7 @@ __global__ void __launch_bounds__(NTH, 1) node_tc_kernel(const __grid_constant__
                     const int it = it0 + j;
                     const int64_t row = row0 + wrow + it * 16;
                     const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
-                    nv[j] = (row < a.rows) ? *(const float4 *)(a.n + (size_t)row * H + k) : z;
+                    nv[j] = (row < a.rows) ? *(const float4 *)(a.n + blk_off(row0, wrow + it * 16, k)) : z;
                     pc[j][0] = pc[j][1] = pc[j][2] = pc[j][3] = z;
                     if (re[it] > rs[it]) {       // warp-uniform
                         const int g0 = rs[it] / a.gran_m, g1 = (re[it] - 1) / a.gran_m;
@@ -214,7 +218,7 @@ __global__ void __launch_bounds__(NTH, 1) node_tc_kernel(const __grid_constant__
             tc::tmem_ld16(tmem_d0 + lane_field + c0, v);
 #pragma unroll
             for (int e4 = 0; e4 < 4; ++e4) {
-                float4 t = valid ? *(const float4 *)(a.n + (size_t)row * H + c0 + e4 * 4) : make_float4(0.f, 0.f, 0.f, 0.f);
+                float4 t = valid ? *(const float4 *)(a.n + blk_off(row0, r, c0 + e4 * 4)) : make_float4(0.f, 0.f, 0.f, 0.f);
                 nn[e4 * 4 + 0] = t.x; nn[e4 * 4 + 1] = t.y; nn[e4 * 4 + 2] = t.z; nn[e4 * 4 + 3] = t.w;
             }
 #pragma unroll
@@ -222,7 +226,7 @@ __global__ void __launch_bounds__(NTH, 1) node_tc_kernel(const __grid_constant__
             if (valid)
 #pragma unroll
                 for (int e4 = 0; e4 < 4; ++e4)
-                    *(float4 *)(a.n + (size_t)row * H + c0 + e4 * 4) =
+                    *(float4 *)(a.n + blk_off(row0, r, c0 + e4 * 4)) =
                         make_float4(nn[e4 * 4], nn[e4 * 4 + 1], nn[e4 * 4 + 2], nn[e4 * 4 + 3]);
             store_operand16(A0, r, c0, nn);
         }
@@ -247,7 +251,7 @@ __global__ void __launch_bounds__(NTH, 1) node_tc_kernel(const __grid_constant__
             tc::tmem_ld16(tmem_d0 + lane_field + c0, v);
 #pragma unroll
             for (int e4 = 0; e4 < 4; ++e4) {
-                float4 t = valid ? *(const float4 *)(a.E + (size_t)row * H + c0 + e4 * 4) : make_float4(0.f, 0.f, 0.f, 0.f);
+                float4 t = valid ? *(const float4 *)(a.E + blk_off(row0, r, c0 + e4 * 4)) : make_float4(0.f, 0.f, 0.f, 0.f);
                 ee[e4 * 4 + 0] = t.x; ee[e4 * 4 + 1] = t.y; ee[e4 * 4 + 2] = t.z; ee[e4 * 4 + 3] = t.w;
             }
 #pragma unroll
@@ -255,7 +259,7 @@ __global__ void __launch_bounds__(NTH, 1) node_tc_kernel(const __grid_constant__
             if (valid)
 #pragma unroll
                 for (int e4 = 0; e4 < 4; ++e4)
-                    *(float4 *)(a.E + (size_t)row * H + c0 + e4 * 4) =
+                    *(float4 *)(a.E + blk_off(row0, r, c0 + e4 * 4)) =
                         make_float4(ee[e4 * 4], ee[e4 * 4 + 1], ee[e4 * 4 + 2], ee[e4 * 4 + 3]);
             if (!a.last) {
                 tc::tmem_ld16(tmem_d1 + lane_field + c0, v);
@@ -313,8 +317,9 @@ __global__ void node_init_tc_kernel(int64_t rows, int N, const int *__restrict__
     const int s = species[row % N];
     const float4 nv = __ldg((const float4 *)(Emb + (size_t)s * H + c0));
     const float4 xv = __ldg((const float4 *)(xs0 + (size_t)s * H + c0));
-    *(float4 *)(n + (size_t)row * H + c0) = nv;
-    *(float4 *)(E + (size_t)row * H + c0) = make_float4(0.f, 0.f, 0.f, 0.f);
+    const size_t o = blk_off(row & ~(int64_t)127, (int)(row & 127), c0);
+    *(float4 *)(n + o) = nv;
+    *(float4 *)(E + o) = make_float4(0.f, 0.f, 0.f, 0.f);
     *(uint4 *)(XE + (size_t)row * H + c0) =
         make_uint4(tc::pack_bf16(xv.x, 0.f), tc::pack_bf16(xv.y, 0.f), tc::pack_bf16(xv.z, 0.f), tc::pack_bf16(xv.w, 0.f));
 }

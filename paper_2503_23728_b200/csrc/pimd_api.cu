@@ -177,10 +177,11 @@ int compute_layout(int N, int R, int P, const double box[3], const pimd_net_para
             L->h1_img = take(cur, n_tiles * 32768);
             L->meta_img = take(cur, n_tiles * 3104);
         }
-        L->nfeat = take(cur, sizeof(float) * rows * H);
+        const int64_t rows128 = (rows + 127) / 128 * 128;   // the tcgen05 node kernel keeps n and E tile-blocked
+        L->nfeat = take(cur, sizeof(float) * rows128 * H);
         L->xfeat = take(cur, sizeof(float) * rows * H);
         L->mfeat = take(cur, sizeof(float) * rows * H);
-        L->Efeat = take(cur, sizeof(float) * rows * H);
+        L->Efeat = take(cur, sizeof(float) * rows128 * H);
         L->Gfeat = take(cur, sizeof(float) * rows * H);
         L->carry_m = take(cur, sizeof(float) * L->n_gran_m * 2 * H);
         L->carry_f = take(cur, sizeof(float) * L->n_gran_f * 2 * 4);
