@@ -208,25 +208,35 @@ def run_ours(args):
     rp1, _ = sim.nlist()
     pairs_last = int(rp1[-1].item())
 
-    # ---- end to end: host state -> H2D -> pimd_set_state -> pimd_step(1) -> pimd_get_state -> D2H, every step
+    # ---- end to end: the full dynamical state (q, p and the forces at q) of EVERY step comes from pinned host memory and
+    # goes back to it: H2D -> pimd_set_state + pimd_set_forces_cached -> pimd_step(1) -> pimd_get_state +
+    # pimd_get_forces_cached -> D2H, then a stream synchronisation (the host owns the result before the next step starts)
     q, p, st = sim.get_state()
-    hq, hp = q.cpu().pin_memory(), p.cpu().pin_memory()
-    dq, dp = torch.empty_like(q), torch.empty_like(p)
+    F = sim.get_forces_cached()
+    hq, hp, hF = q.cpu().pin_memory(), p.cpu().pin_memory(), F.cpu().pin_memory()
+    dq, dp, dF = torch.empty_like(q), torch.empty_like(p), torch.empty_like(F)
+    q2, p2, F2 = torch.empty_like(q), torch.empty_like(p), torch.empty_like(F)
     e2e_steps = max(3, min(args.steps, 10))
+    lib = pb.load_library()
+    import ctypes as C
     barrier()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record(stream)
     for i in range(e2e_steps):
-        dq.copy_(hq, non_blocking=True); dp.copy_(hp, non_blocking=True)
-        sim.set_state(dq, dp, st + i)
+        dq.copy_(hq, non_blocking=True); dp.copy_(hp, non_blocking=True); dF.copy_(hF, non_blocking=True)
+        sim.set_state_async(dq, dp, st + i)
+        sim.set_forces_cached(dF)
         sim.step(1)
-        q2, p2, _ = sim.get_state()
-        hq.copy_(q2, non_blocking=True); hp.copy_(p2, non_blocking=True)
+        stc = C.c_int64()
+        rc = lib.pimd_get_state(sim._h, C.c_void_p(q2.data_ptr()), C.c_void_p(p2.data_ptr()), C.byref(stc))
+        assert rc == 0, lib.pimd_last_error()
+        sim.get_forces_cached(F2)
+        hq.copy_(q2, non_blocking=True); hp.copy_(p2, non_blocking=True); hF.copy_(F2, non_blocking=True)
         stream.synchronize()
     e1.record(stream)
     barrier()
     t_e2e = e0.elapsed_time(e1) * 1e-3
-    state_bytes = int(q.numel() * 8 * 2)
+    state_bytes = int(q.numel() * 8 * 3)
 
     times = torch.tensor([t_dev, t_e2e], dtype=torch.float64, device=dev)
     if dist is not None:
@@ -287,7 +297,7 @@ def run_ours(args):
             "wall_ms_per_step_incl_flush": 1e3 * wall / args.steps,
             "e2e": {"value": w.rows * e2e_steps * world / t_e2e, "unit": UNIT, "h2d_bytes_per_step": state_bytes,
                     "d2h_bytes_per_step": state_bytes, "steps": e2e_steps,
-                    "path": "pinned host q,p -> H2D -> pimd_set_state -> pimd_step(1) -> pimd_get_state -> D2H"},
+                    "path": "pinned host q,p,F -> H2D -> pimd_set_state + pimd_set_forces_cached -> pimd_step(1) -> pimd_get_state + pimd_get_forces_cached -> D2H -> stream sync, every step"},
             "gpu_launches": int(launches),
             "clocks": clocks,
             "kernel_ms_per_step": {k: v[0] / args.steps for k, v in prof.items()},

@@ -117,6 +117,15 @@ int pimd_estimators(pimd_ctx *ctx, pimd_estimators_t *h_out);
 int pimd_get_state(pimd_ctx *ctx, double *d_q, double *d_p, int64_t *step);
 int pimd_set_state(pimd_ctx *ctx, const double *d_q, const double *d_p, int64_t step);
 
+/* The cached forces F(q) belong to a checkpoint too: a resume that restores them skips the force evaluation
+ * pimd_set_state would otherwise trigger (same trajectory bit for bit either way; S:N3 step 4 recomputes F from q).
+ *   pimd_get_forces_cached  d_F DEVICE double [R][P][N][3] eV/A, the forces at the current q (evaluated if stale);
+ *                           asynchronous.
+ *   pimd_set_forces_cached  d_F DEVICE; the caller asserts that d_F = F(q) for the q given to the last pimd_set_state.
+ *                           Asynchronous; marks the cached forces valid. */
+int pimd_get_forces_cached(pimd_ctx *ctx, double *d_F);
+int pimd_set_forces_cached(pimd_ctx *ctx, const double *d_F);
+
 /* Builds the neighbour list at the current positions and exports it as CSR over all rows.
  *   d_row_ptr DEVICE int32 [R*P*N + 1]; d_col DEVICE int32 [col_capacity] holds the atom index j
  *   (0..N-1, within the bead-system of the row), ascending within each row (S:L1);

@@ -573,6 +573,23 @@ extern "C" int pimd_set_state(pimd_ctx *c, const double *d_q, const double *d_p,
     return 0;
 }
 
+extern "C" int pimd_get_forces_cached(pimd_ctx *c, double *d_F)
+{
+    if (!c || !d_F) { pimd_set_error("null argument"); return PIMD_ERR_ARG; }
+    int rc;
+    if (!c->forces_valid && (rc = compute_forces(c))) return rc;
+    PIMD_CUDA_CHECK(cudaMemcpyAsync(d_F, c->F, sizeof(double) * (size_t)c->rows * 3, cudaMemcpyDeviceToDevice, c->stream));
+    return 0;
+}
+
+extern "C" int pimd_set_forces_cached(pimd_ctx *c, const double *d_F)
+{
+    if (!c || !d_F) { pimd_set_error("null argument"); return PIMD_ERR_ARG; }
+    PIMD_CUDA_CHECK(cudaMemcpyAsync(c->F, d_F, sizeof(double) * (size_t)c->rows * 3, cudaMemcpyDeviceToDevice, c->stream));
+    c->forces_valid = 1;
+    return 0;
+}
+
 extern "C" int pimd_nlist(pimd_ctx *c, int32_t *d_row_ptr, int32_t *d_col, int64_t col_capacity, int64_t *h_n_pairs)
 {
     if (!c || !d_row_ptr || !d_col || !h_n_pairs) { pimd_set_error("null argument"); return PIMD_ERR_ARG; }

@@ -57,6 +57,8 @@ def load_library():
     L.pimd_estimators.argtypes = [vp, C.POINTER(Estimators)]
     L.pimd_get_state.argtypes = [vp, vp, vp, C.POINTER(C.c_int64)]
     L.pimd_set_state.argtypes = [vp, vp, vp, C.c_int64]
+    L.pimd_get_forces_cached.argtypes = [vp, vp]
+    L.pimd_set_forces_cached.argtypes = [vp, vp]
     L.pimd_nlist.argtypes = [vp, vp, vp, C.c_int64, C.POINTER(C.c_int64)]
     L.pimd_sync.argtypes = [vp]
     L.pimd_profile.argtypes = [vp, C.c_int]
@@ -171,6 +173,21 @@ class PIMD:
         assert q.numel() == self.rows * 3 and p.numel() == self.rows * 3
         _check(load_library().pimd_set_state(self._h, C.c_void_p(q.data_ptr()), C.c_void_p(p.data_ptr()), int(step)))
         self.sync()  # q, p temporaries may be freed by the caller right after
+
+    def get_forces_cached(self, out=None):
+        t = self._torch
+        if out is None:
+            out = t.empty(self.shape, dtype=t.float64, device=self.device)
+        _check(load_library().pimd_get_forces_cached(self._h, C.c_void_p(out.data_ptr())))
+        return out
+
+    def set_forces_cached(self, F):
+        assert F.dtype == self._torch.float64 and F.is_contiguous() and F.numel() == self.rows * 3
+        _check(load_library().pimd_set_forces_cached(self._h, C.c_void_p(F.data_ptr())))
+
+    def set_state_async(self, q, p, step):
+        """pimd_set_state without the synchronisation: q, p must be contiguous float64 device tensors that outlive the call."""
+        _check(load_library().pimd_set_state(self._h, C.c_void_p(q.data_ptr()), C.c_void_p(p.data_ptr()), int(step)))
 
     def nlist(self, cap_per_row=None):
         t = self._torch

@@ -137,3 +137,30 @@ def test_water64_trajectory_short(cuda_device):
     assert np.abs(qg - qr).max() < 1e-4
     eg, er = gpu.estimators(), ref.estimators()
     assert np.allclose(eg[:, :3], er[:, :3], rtol=1e-3, atol=1e-3) and np.isnan(eg[0, 3])
+
+
+def test_resume_with_cached_forces_is_bit_exact(cuda_device):
+    """Checkpoint = (q, p, step) + the cached forces: restoring them skips the force evaluation and changes nothing."""
+    import torch
+    w = pi.make_workload("fad_p8")
+    a, _ = pair_from_workload(w)
+    a.step(6)
+    qa, pa, sa = a.get_state()
+    b, _ = pair_from_workload(w)
+    b.step(3)
+    q, p, st = b.get_state()
+    F = b.get_forces_cached()
+    c, _ = pair_from_workload(w)
+    c.set_state(q, p, st)
+    n0 = c.launch_count()
+    c.set_forces_cached(F)
+    c.step(3)
+    qc, pc, sc = c.get_state()
+    assert sc == sa == 6 and torch.equal(qa, qc) and torch.equal(pa, pc)
+    d, _ = pair_from_workload(w)          # same resume without the forces: one more force evaluation, same result
+    d.set_state(q, p, st)
+    m0 = d.launch_count()
+    d.step(3)
+    qd, pd, _ = d.get_state()
+    assert torch.equal(qa, qd) and torch.equal(pa, pd)
+    assert (d.launch_count() - m0) > (c.launch_count() - n0)
