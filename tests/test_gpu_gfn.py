@@ -164,3 +164,36 @@ def test_resume_with_cached_forces_is_bit_exact(cuda_device):
     qd, pd, _ = d.get_state()
     assert torch.equal(qa, qd) and torch.equal(pa, pd)
     assert (d.launch_count() - m0) > (c.launch_count() - n0)
+
+
+@pytest.mark.parametrize("gemm_dtype", [0, 1])
+def test_no_pairs_at_all_gives_zero_forces(cuda_device, gemm_dtype):
+    """Degenerate list: every atom isolated (open box, 100 A apart) -> empty CSR, F == 0, and stepping still works."""
+    x = (np.arange(6)[:, None] * np.array([100.0, 0.0, 0.0]))[None]
+    sp = np.array([0, 1, 2, 0, 1, 2], dtype=np.int32)
+    spec = _biased_spec(64, 128, 2, 3.0, 1.0 / 12.0, 0.2)
+    spec.gemm_dtype = gemm_dtype
+    gpu, ref = make_pair(sp, x, np.zeros(3), 4, 300.0, 0.25, 1.0, 0, spec)
+    rp, col = gpu.nlist()
+    assert int(rp[-1].item()) == 0 and col.numel() == 0
+    Fg, Fr = _forces_pair(gpu, ref)
+    assert np.all(Fg == 0.0) and np.all(Fr == 0.0)
+    gpu.step(3); ref.step(3)
+    qg, _, _ = gpu_state(gpu); qr, _, _ = ref.get_state()
+    assert np.abs(qg - qr).max() < 1e-10
+
+
+def test_tensor_core_path_is_bitwise_deterministic(cuda_device):
+    """tcgen05 pipeline: fixed-order segmented sums, carry slots, no floating-point atomics -> identical bits every time."""
+    import torch
+    rng = np.random.default_rng(21)
+    box = np.array([12.5, 13.0, 12.2]); n_at = 500
+    x = rng.uniform(0, 1, (1, n_at, 3)) * box
+    sp = rng.integers(0, 3, n_at).astype(np.int32)
+    spec = _biased_spec(64, 128, 3, 3.0, 1.0 / 12.0, 0.2)
+    spec.gemm_dtype = 1
+    gpu, ref = make_pair(sp, x, box, 3, 300.0, 0.25, 1.0, 0, spec)
+    spread_beads(gpu, ref, scale=0.05)
+    a = gpu.forces().clone()
+    for _ in range(3):
+        assert torch.equal(a, gpu.forces())
