@@ -105,6 +105,27 @@ def flops_per_pair_launch_as_built(K, H, L, tensor_path):
     return (full + L * later) / (L + 1.0)
 
 
+def max_over_ranks(times, dist, device):
+    """Device times of this rank -> the slowest rank's times (a multi-GPU number is the max over ranks, never a mean).
+
+    `dist` is torch.distributed (initialised; NCCL on the GPU box, gloo in the CPU test) or None for a single process."""
+    import torch
+    t = torch.tensor(list(times), dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t]
+
+
+def whole_job_value(rows_per_rank, steps, world, seconds):
+    """atom*bead*steps/s of the whole job: every rank steps its own replica of the workload ("replicas only", weak scaling)."""
+    return rows_per_rank * steps * world / seconds
+
+
+def rank_seed(base_seed, rank):
+    """Philox key of rank r: independent thermostat streams, same workload shape."""
+    return base_seed + rank
+
+
 # ------------------------------------------------------------------------------------------------
 def run_reference(args):
     """The oracle, as it stands, on the host cores; each step = one PIMD step of a bounded sample."""
@@ -168,7 +189,7 @@ def run_ours(args):
 
     w = pi.make_workload(args.workload)
     if world > 1:  # independent replica per rank: different thermostat stream, same workload shape
-        w.seed = w.seed + rank
+        w.seed = rank_seed(w.seed, rank)
     sim = pb.PIMD.from_workload(w, device=str(dev))
     stream = torch.cuda.current_stream(dev)
     flush = torch.empty(512 * 1024 * 1024 // 4, dtype=torch.float32, device=dev)  # 512 MB > 126 MB L2
@@ -238,14 +259,10 @@ def run_ours(args):
     t_e2e = e0.elapsed_time(e1) * 1e-3
     state_bytes = int(q.numel() * 8 * 3)
 
-    times = torch.tensor([t_dev, t_e2e], dtype=torch.float64, device=dev)
-    if dist is not None:
-        dist.all_reduce(times, op=dist.ReduceOp.MAX)
-    t_dev, t_e2e = float(times[0]), float(times[1])
+    t_dev, t_e2e = max_over_ranks([t_dev, t_e2e], dist, dev)
 
     if rank == 0:
-        units = w.rows * args.steps * world
-        value = units / t_dev
+        value = whole_job_value(w.rows, args.steps, world, t_dev)
         K, H, L = w.net.n_rbf, w.net.hidden, w.net.n_layers
         pairs = 0.5 * (pairs_first + pairs_last)
         pair_ms, pair_n = prof["gfn.pair"]
@@ -295,7 +312,7 @@ def run_ours(args):
                        "timing": "sum of per-step CUDA-event intervals on the launch stream"},
             "ns_per_day": args.steps / t_dev * w.dt * 86400e-6,
             "wall_ms_per_step_incl_flush": 1e3 * wall / args.steps,
-            "e2e": {"value": w.rows * e2e_steps * world / t_e2e, "unit": UNIT, "h2d_bytes_per_step": state_bytes,
+            "e2e": {"value": whole_job_value(w.rows, e2e_steps, world, t_e2e), "unit": UNIT, "h2d_bytes_per_step": state_bytes,
                     "d2h_bytes_per_step": state_bytes, "steps": e2e_steps,
                     "path": "pinned host q,p,F -> H2D -> pimd_set_state + pimd_set_forces_cached -> pimd_step(1) -> pimd_get_state + pimd_get_forces_cached -> D2H -> stream sync, every step"},
             "gpu_launches": int(launches),

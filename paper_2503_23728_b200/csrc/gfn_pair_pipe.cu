@@ -2,22 +2,26 @@
 // warp-specialised pipeline (rows a5, a7 of SURVEY 8(a)).  bf16 operands, fp32 accumulation
 // in TMEM.  Used when gemm_dtype == 1 and (K, H) == (64, 128)  (BASELINE configs[3..4]; tolerance 2e-2).
 //
-// One persistent CTA per SM walks 128-pair tiles of the flat CSR pair list.  Five roles run concurrently on
-// different tiles and hand buffers to each other through mbarriers only (no CTA-wide barrier in the loop):
+// One persistent CTA per SM walks 128-pair tiles of the flat CSR pair list.  The roles below run concurrently on
+// different tiles and hand buffers to each other through mbarriers and named barriers only (no CTA-wide barrier in the loop).
+// First pair pass of a force evaluation (MODE 0):
 //   P   4 warps, thread = pair : indices, fp64 minimum image -> distance, cutoff weight, row-segment flags (meta ring);
 //                                Gaussian RBF tile -> A1 (bf16, K-major, 128-byte swizzle)
 //   MMA 1 thread               : D1 = A1 (W_e1/2)^T  (4 x UMMA 128x128x16);  D2^T = W2 A2^T  (8 x UMMA), W2 = W_e2 or W_f1 W_e2/2
 //   H   4 warps, thread = pair : D1 (TMEM) + b -> SiLU -> A2 (bf16 operand of the second product)
+//   S   1 warp                 : TMA bulk stores of the tile's A2 image (32 KB) and meta record to HBM
 //   G   4 warps                : TMA bulk copies of the gathered rows (x_j|E_j packed bf16, or G_j fp32; 512 B per pair)
 //                                into an 8-slot shared-memory ring, 16 pairs per slot
 //   E   16 warps, thread = (channel, quarter tile): D2^T (TMEM lane = channel) -> e_ij = e0_ij + E_i + E_j (S:G5) ->
-//                                message: private running sums over CSR row segments, flushed at row boundaries;
-//                                head:    w_f2 . SiLU(.) reduced over channels by a fixed shuffle tree, then a
-//                                         segmented warp scan of c_ij s_ij u_ij over 32-pair granules.
-// The filter's first layer does not depend on the interaction layer: the first pair pass of a force evaluation
-// (MODE 0) also streams every tile's h1 operand image and meta record to HBM (role S, TMA bulk stores), and the later
-// passes (MODE 1: remaining message passes and the force head) replace roles P, H and the first product by one
-// loader warp (role L) that brings them back with two TMA bulk copies per tile.
+//                                private running sums over CSR row segments, cut at row boundaries.
+// The filter's first layer does not depend on the interaction layer, so the later passes (MODE 1: remaining message
+// passes and the force head) replace P, H and the first product by
+//   L   1 warp                 : two TMA bulk copies per tile bring the A2 image and the meta record back
+// and the head runs its channel reduction on the tensor core:
+//   E   (head)                 : act = SiLU(W_fe h1 + b_fe + G_i + G_j) written as a bf16 K-major operand A3
+//   MMA                        : D3[p][.] = act[p][:] . w_f2   (8 x UMMA 128x16x16)
+//   F   4 warps, thread = pair : s_p from D3 -> c_ij s_ij u_ij, segmented warp scan over 32-pair granules -> forces.
+// (When L = 0 the head is the first pass; it then reduces over channels with a fixed shuffle tree.)
 // Waiting: mbarrier try_wait does not suspend on this part (it polls, and every poll takes an issue slot from the warps
 // that have work).  So per role ONE warp polls the mbarriers that tensor-core commits and TMA transactions complete
 // on, and releases its role's other warps through a named barrier (bar.sync blocks in hardware); the pollers sit on
@@ -59,8 +63,8 @@ constexpr int NM = 4;        // meta ring depth (tiles)
 constexpr int NSLOT = 4;     // quarter tiles; the gather ring has two 16-pair slots per quarter
 // Warp layout per kernel variant (fewer warps in the later passes -> more registers per thread for role E):
 //   MODE 0           : P 0-3, H 4-7, E 8-23, MMA 24, G 25-28, S 29           (30 warps, 64 registers)
-//   MODE 1, message  : E 0-15, G 16-19, MMA 20, L 21                          (22 warps, 88 registers)
-//   MODE 1, head     : E 0-15, F 16-19, G 20-23, MMA 24, L 25                 (26 warps, 72 registers)
+//   MODE 1, message  : E 0-15, G 16-19, MMA 20, L 21                          (22 warps, 80 registers used)
+//   MODE 1, head     : E 0-15, F 16-19, G 20-23, MMA 24, L 25                 (26 warps, 71 registers used)
 // E and F/H warps start at a multiple of 4: warp % 4 is the TMEM lane quadrant a warp may access.
 template <bool HEAD, int MODE>
 struct Warps {
