@@ -62,7 +62,8 @@ constexpr int K = 64;        // radial basis functions
 constexpr int NM = 4;        // meta ring depth (tiles)
 constexpr int NSLOT = 4;     // quarter tiles; the gather ring has two 16-pair slots per quarter
 // Warp layout per kernel variant (fewer warps in the later passes -> more registers per thread for role E):
-//   MODE 0           : P 0-3, H 4-7, E 8-23, MMA 24, G 25-28, S 29           (30 warps, 64 registers)
+//   MODE 0           : P 0-3, H 4-7, E 8-23, MMA 24, G 25-28, S 29, idle 30-31 (32 warps, 64 registers at launch; setmaxnreg
+//                      moves registers from the P, H, MMA/G/S warpgroups (56, 56, 40) to the four E warpgroups (80))
 //   MODE 1, message  : E 0-15, G 16-19, MMA 20, L 21                          (22 warps, 80 registers used)
 //   MODE 1, head     : E 0-15, F 16-19, G 20-23, MMA 24, L 25                 (26 warps, 71 registers used)
 // E and F/H warps start at a multiple of 4: warp % 4 is the TMEM lane quadrant a warp may access.
@@ -73,7 +74,7 @@ struct Warps {
     static constexpr int G0 = (MODE == 0) ? 25 : (HEAD ? 20 : 16);
     static constexpr int MMA = (MODE == 0) ? 24 : (HEAD ? 24 : 20);
     static constexpr int SL = (MODE == 0) ? 29 : MMA + 1;                // S (MODE 0) or L (MODE 1)
-    static constexpr int N = SL + 1;
+    static constexpr int N = (MODE == 0) ? 32 : SL + 1;                  // MODE 0: whole warpgroups (setmaxnreg), warps 30-31 idle
     static constexpr int THREADS = N * 32;
 };
 
@@ -854,6 +855,11 @@ __global__ void __launch_bounds__(Warps<HEAD, MODE>::THREADS, 1) pair_pipe_kerne
         if (MODE == 0) tc::bulk_g2s(S + OFF_W1, a.W1img, 16384, &bar[W_FULL]);
         else if (HEAD) tc::bulk_g2s(S + OFF_W1, a.Wf2img, 4096, &bar[W_FULL]);   // w_f2 operand of the readout product
         tc::bulk_g2s(S + OFF_W2, a.W2img, 32768, &bar[W_FULL]);
+    }
+    if (MODE == 0) {                               // register re-balancing between warpgroups (aligned groups of 4 warps)
+        if (warp < 8) asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
+        else if (warp < 24) asm volatile("setmaxnreg.inc.sync.aligned.u32 80;");
+        else asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
     }
     if (MODE == 0 && warp < 4) {
         role_P<HEAD>(a, S, bar, n_my, n_pairs, tid, lane);
