@@ -56,6 +56,10 @@ namespace gfn_pipe {
 #define STATS_END(name)
 #endif
 
+// wait of a role that is idle most of the time (the MMA thread, the store warp S): polls at the pace of an L2 round trip (tc_ptx.cuh).
+// The polled word is any readable one, a different 32-byte sector per CTA; the scratch word is never read.
+#define LAZY_WAIT(barp, par) tc::mbar_wait_lazy(barp, par, a.h1_img + (size_t)blockIdx.x * 32, S + OFF_TMEM + 8)
+
 constexpr int TP = 128;      // pairs per tile
 constexpr int H = 128;       // channels
 constexpr int K = 64;        // radial basis functions
@@ -366,6 +370,22 @@ __device__ __forceinline__ void role_E_msg(const PairArgs &a, unsigned char *S, 
             if (mask == 0u) {
 #pragma unroll
                 for (int e = 0; e < 16; ++e) { st.s1 = fmaf(v[e], wx[e], st.s1); st.s2 += wx[e]; }
+            } else if ((mask & (mask - 1)) == 0u) {
+                // exactly one row boundary in the chunk (the usual case: rows are longer than 16 pairs): the pairs
+                // before it close the running sums, the pairs from it on open the next row's (warp-uniform predicates)
+                const int hi = __ffs(mask) - 1;
+                float t1 = 0.f, t2 = 0.f;
+#pragma unroll
+                for (int e = 0; e < 16; ++e) {
+                    if (e < hi) { st.s1 = fmaf(v[e], wx[e], st.s1); st.s2 += wx[e]; }
+                    else        { t1 = fmaf(v[e], wx[e], t1); t2 += wx[e]; }
+                }
+                msg_flush(a, st, gidx, c);
+                const int rk = M.rowk[q0 + hi];
+                st.cur = (rk < 0) ? -1 : (rk & 0x1FFFFFFF);
+                st.kind = (rk < 0) ? 0 : (rk >> 29);
+                st.s1 = t1; st.s2 = t2;
+                if (st.cur >= 0) msg_row_bias(XE, st, a.rows, b2c, c);
             } else {
                 int lo = 0;
 #pragma unroll 1
@@ -596,6 +616,25 @@ __device__ __forceinline__ void role_E_head_tc(const PairArgs &a, unsigned char 
                     const float h = fmaf(0.5f, gj[e], v[e] + be);
                     v[e] = fmaf(h, tc::tanh_approx(h), h);
                 }
+            } else if ((mask & (mask - 1)) == 0u) {
+                // exactly one row boundary in the chunk (the usual case): pairs before it take the old row's bias,
+                // pairs from it on the new row's (warp-uniform select)
+                const int hi = __ffs(mask) - 1;
+                const float be0 = be;
+                const int rk = M.rowk[q0 + hi];
+                const int r = (rk < 0) ? -1 : (rk & 0x1FFFFFFF);
+                cur_row = r;
+                if (r >= 0) {
+                    const float raw = (r == nx_row) ? nx_val : __ldg(Gf + (size_t)r * H + c);
+                    be = b2c + 0.5f * raw;
+                    nx_row = (r + 1 < a.rows) ? r + 1 : r;
+                    nx_val = __ldg(Gf + (size_t)nx_row * H + c);
+                }
+#pragma unroll
+                for (int e = 0; e < 16; ++e) {
+                    const float h = fmaf(0.5f, gj[e], v[e] + ((e < hi) ? be0 : be));
+                    v[e] = fmaf(h, tc::tanh_approx(h), h);
+                }
             } else {
                 int lo = 0;
 #pragma unroll 1
@@ -681,7 +720,7 @@ __device__ __forceinline__ void role_F(const PairArgs &a, unsigned char *S, uint
 
 // ---- role MMA: one elected lane issues both products; completion is committed to the consumers' mbarriers
 template <bool HEAD, int MODE>
-__device__ __forceinline__ void role_MMA(unsigned char *S, uint64_t *bar, uint32_t tmem, int n_my, int lane)
+__device__ __forceinline__ void role_MMA(const PairArgs &a, unsigned char *S, uint64_t *bar, uint32_t tmem, int n_my, int lane)
 {
     STATS_BEGIN
     constexpr bool TCH = HEAD && MODE == 1;      // head with the channel reduction on the tensor core
@@ -693,8 +732,8 @@ __device__ __forceinline__ void role_MMA(unsigned char *S, uint64_t *bar, uint32
     for (int k = 0; k <= n_my + (TCH ? 1 : 0); ++k) {
         if (MODE == 0 && k < n_my) {             // D1[s] = G (W_e1/2)^T   (4 x UMMA 128x128x16)
             const int s = k & 1, ph = (k >> 1) & 1;
-            WAITED(tc::mbar_wait(&bar[D1_EMPTY + s], ph ^ 1));
-            WAITED(tc::mbar_wait(&bar[A1_FULL + s], ph));
+            WAITED(LAZY_WAIT(&bar[D1_EMPTY + s], ph ^ 1));
+            WAITED(LAZY_WAIT(&bar[A1_FULL + s], ph));
             tc::tc_fence_after_sync();
             if (lane == 0) {
 #pragma unroll
@@ -708,8 +747,8 @@ __device__ __forceinline__ void role_MMA(unsigned char *S, uint64_t *bar, uint32
         }
         if (k >= 1 && k <= n_my) {               // D2[s]^T = W2 h1^T   (8 x UMMA; M = channels, N = pairs)
             const int j = k - 1, s = j & 1, ph = (j >> 1) & 1, sa = j % NA2, pha = (j / NA2) & 1;
-            WAITED(tc::mbar_wait(&bar[D2_EMPTY + s], ph ^ 1));
-            WAITED(tc::mbar_wait(&bar[A2_FULL + sa], pha));
+            WAITED(LAZY_WAIT(&bar[D2_EMPTY + s], ph ^ 1));
+            WAITED(LAZY_WAIT(&bar[A2_FULL + sa], pha));
             tc::tc_fence_after_sync();
             if (lane == 0) {
 #pragma unroll
@@ -725,8 +764,8 @@ __device__ __forceinline__ void role_MMA(unsigned char *S, uint64_t *bar, uint32
         }
         if (TCH && k >= 2) {                     // D3[s][p][0..15] = act[p][:] . w_f2   (8 x UMMA 128x16x16; M = pairs)
             const int i = k - 2, s = i & 1, ph = (i >> 1) & 1;
-            WAITED(tc::mbar_wait(&bar[D3_EMPTY + s], ph ^ 1));
-            WAITED(tc::mbar_wait(&bar[A3_FULL + s], ph));
+            WAITED(LAZY_WAIT(&bar[D3_EMPTY + s], ph ^ 1));
+            WAITED(LAZY_WAIT(&bar[A3_FULL + s], ph));
             tc::tc_fence_after_sync();
             if (lane == 0) {
                 const uint32_t sA3 = s ? sA1 : sA2 + 32768;
@@ -775,7 +814,7 @@ __device__ __forceinline__ void role_S(const PairArgs &a, unsigned char *S, uint
         const int s = it & 1;
         const int64_t tile = (int64_t)blockIdx.x + (int64_t)it * gridDim.x;
         WAITED(tc::mbar_wait(&bar[META_FULL + (it & (NM - 1))], (it / NM) & 1));
-        WAITED(tc::mbar_wait(&bar[A2_FULL + s], (it >> 1) & 1));
+        WAITED(LAZY_WAIT(&bar[A2_FULL + s], (it >> 1) & 1));
         if (lane == 0) {
             tc::fence_proxy_async_smem();       // generic-proxy writes of P and H (acquired above) -> async-proxy reads
             tc::bulk_s2g(a.h1_img + tile * 32768, S + OFF_A2 + s * 32768, 32768);
@@ -874,7 +913,7 @@ __global__ void __launch_bounds__(Warps<HEAD, MODE>::THREADS, 1) pair_pipe_kerne
     } else if (HEAD && MODE == 1 && warp >= WL::F0 && warp < WL::F0 + 4) {
         role_F(a, S, bar, tmem, n_my, tid - WL::F0 * 32, lane);
     } else if (warp == WL::MMA) {
-        role_MMA<HEAD, MODE>(S, bar, tmem, n_my, lane);
+        role_MMA<HEAD, MODE>(a, S, bar, tmem, n_my, lane);
     } else if (warp >= WL::G0 && warp < WL::G0 + 4) {
         role_G(a, S, bar, n_my, warp - WL::G0, lane);
     } else if (warp == WL::SL) {

@@ -47,6 +47,31 @@ __device__ __forceinline__ void mbar_wait_relaxed(uint64_t *bar, uint32_t parity
     }
 }
 
+// wait of a role that is not on the critical path: between two polls the warp sits on the scoreboard of one
+// uncached global load (an L2 round trip, a few hundred cycles, one issue slot) instead of spinning on try_wait,
+// which does not suspend on this part and takes issue slots from the warps that have work.  `g` is any readable word;
+// its value is only consumed (stored to `scratch`, a shared-memory word nobody reads) to create the dependency.
+__device__ __forceinline__ void mbar_wait_lazy(uint64_t *bar, uint32_t parity, const void *g, void *scratch)
+{
+    const uint32_t b = smem_u32(bar), sc = smem_u32(scratch);
+    while (true) {
+        uint32_t done;
+        asm volatile(
+            "{\n\t"
+            ".reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t"
+            "}\n"
+            : "=r"(done)
+            : "r"(b), "r"(parity)
+            : "memory");
+        if (done) break;
+        uint32_t t;
+        asm volatile("ld.volatile.global.u32 %0, [%1];" : "=r"(t) : "l"(g) : "memory");
+        asm volatile("st.volatile.shared.u32 [%0], %1;" ::"r"(sc), "r"(t) : "memory");
+    }
+}
+
 __device__ __forceinline__ void mbar_arrive(uint64_t *bar)
 {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
