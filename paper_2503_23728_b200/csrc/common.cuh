@@ -85,6 +85,7 @@ struct pimd_ctx {
     uint16_t *wimg_wf2;                // bf16 UMMA image of w_f2 replicated on 16 rows (readout product of the head)
     uint16_t *wimg_e1, *wimg_e2, *wimg_fe;   // bf16 UMMA images (K-major, 128B swizzle) for the tcgen05 path
     int use_tc;                        // 1: tensor-core pair and node kernels (gemm_dtype 1, K=64, H=128)
+    int msg_rowgemm;                   // 1: later message passes as one GEMM per CSR row (experimental, env PIMD_MSG_ROWGEMM=1)
     uint16_t *wimg_node;               // [L][5] bf16 UMMA images: W_vn/2, W_vm/2, W_v2, W_a, W_s^{l+1} (or W_f1)
     float *xs0;                        // [S][H] W_s^0 Emb[s]
     float h_be1_half[128];             // HOST copy of b_e1 / 2 (passed to the pair kernels as kernel parameters)

@@ -25,7 +25,7 @@ constexpr int NW = 5;              // resident weight images: W_vn/2, W_vm/2, W_
 
 struct Args {
     int64_t rows;
-    int N, last, gran_m, n_tiles;
+    int N, last, gran_m, n_tiles, xy_rows;
     const int *row_ptr;
     const uint16_t *Wimg;
     const float *bv1, *bv2, *ba;
@@ -263,12 +263,25 @@ __global__ void __launch_bounds__(NTH, 1) node_tc_kernel(const __grid_constant__
                         make_float4(ee[e4 * 4], ee[e4 * 4 + 1], ee[e4 * 4 + 2], ee[e4 * 4 + 3]);
             if (!a.last) {
                 tc::tmem_ld16(tmem_d1 + lane_field + c0, v);
-                if (valid)
+                if (valid && !a.xy_rows) {
 #pragma unroll
                     for (int e4 = 0; e4 < 4; ++e4)
                         *(uint4 *)(a.XE + (size_t)row * H + c0 + e4 * 4) =
                             make_uint4(tc::pack_bf16(v[e4 * 4], ee[e4 * 4]), tc::pack_bf16(v[e4 * 4 + 1], ee[e4 * 4 + 1]),
                                        tc::pack_bf16(v[e4 * 4 + 2], ee[e4 * 4 + 2]), tc::pack_bf16(v[e4 * 4 + 3], ee[e4 * 4 + 3]));
+                } else if (valid) {              // two bf16 rows per atom for the row-GEMM message pass: x | y = E (.) x
+                    uint32_t px[8], py[8];
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) {
+                        px[e] = tc::pack_bf16(v[2 * e], v[2 * e + 1]);
+                        py[e] = tc::pack_bf16(ee[2 * e] * v[2 * e], ee[2 * e + 1] * v[2 * e + 1]);
+                    }
+                    uint32_t *xr = a.XE + (size_t)row * H + (c0 >> 1);          // 128 words per row: x 0-63, y 64-127
+                    *(uint4 *)(xr) = make_uint4(px[0], px[1], px[2], px[3]);
+                    *(uint4 *)(xr + 4) = make_uint4(px[4], px[5], px[6], px[7]);
+                    *(uint4 *)(xr + 64) = make_uint4(py[0], py[1], py[2], py[3]);
+                    *(uint4 *)(xr + 68) = make_uint4(py[4], py[5], py[6], py[7]);
+                }
             } else {
                 store_operand16(A1, r, c0, ee);
             }
@@ -337,7 +350,8 @@ int launch_node_tc(pimd_ctx *c, int mode, int layer)
     }
     const GfnLayerW &w = n.layer[layer];
     Args a;
-    a.rows = c->rows; a.N = c->N; a.last = (layer == n.L - 1); a.gran_m = c->gran_m;
+    a.rows = c->rows; a.N = c->N; a.last = (layer == n.L - 1); a.gran_m = (layer == 0 || !c->msg_rowgemm) ? c->gran_m : 128;   // row-GEMM message passes: granule = tile
+    a.xy_rows = c->msg_rowgemm;
     a.n_tiles = (int)((c->rows + TR - 1) / TR);
     a.row_ptr = c->nl.row_ptr;
     a.Wimg = c->wimg_node + (size_t)layer * NW * (OPB / 2);

@@ -425,6 +425,10 @@ extern "C" int pimd_create(pimd_ctx **out, int n_atoms, int n_replicas, const in
         RawNet raw;
         build_weights(net, wd, offs, Wfe, raw);
         c->use_tc = (net->gemm_dtype == 1 && net->n_rbf == 64 && net->hidden == 128) ? 1 : 0;
+        {
+            const char *e = getenv("PIMD_MSG_ROWGEMM");      // experimental formulation of the later message passes (off by default)
+            c->msg_rowgemm = (c->use_tc && e && e[0] == '1') ? 1 : 0;
+        }
         c->wimg_e1 = (uint16_t *)(ws + L.wimg); c->wimg_e2 = c->wimg_e1 + 8192; c->wimg_fe = c->wimg_e2 + 16384;
         if (c->use_tc) {
             wimg.resize(5 * 8192 + 2048);

@@ -28,6 +28,25 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
         : "memory");
 }
 
+// latency-critical wait (a hand-off on a serial chain): plain spin on try_wait without a suspend hint.  The waiting
+// form above sleeps in hardware and was measured to wake up several hundred ns after the phase completes.
+__device__ __forceinline__ void mbar_wait_spin(uint64_t *bar, uint32_t parity)
+{
+    const uint32_t b = smem_u32(bar);
+    uint32_t done;
+    do {
+        asm volatile(
+            "{\n\t"
+            ".reg .pred p;\n\t"
+            "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t"
+            "}\n"
+            : "=r"(done)
+            : "r"(b), "r"(parity)
+            : "memory");
+    } while (!done);
+}
+
 // wait of a role that runs ahead of its consumer: poll, and sleep `ns` between polls instead of spinning on issue slots
 __device__ __forceinline__ void mbar_wait_relaxed(uint64_t *bar, uint32_t parity, uint32_t ns)
 {

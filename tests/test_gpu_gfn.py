@@ -197,3 +197,26 @@ def test_tensor_core_path_is_bitwise_deterministic(cuda_device):
     a = gpu.forces().clone()
     for _ in range(3):
         assert torch.equal(a, gpu.forces())
+
+
+def test_row_gemm_message_pass_parity_and_determinism(cuda_device, monkeypatch):
+    """Experimental formulation of the later message passes (one GEMM per CSR row with the pair index as the contraction
+    dimension, W_e2 applied per row in fp32; PIMD_MSG_ROWGEMM=1): same bound as the default path,
+    and the token chain fixes the accumulation order (identical bits every time)."""
+    import torch
+    monkeypatch.setenv("PIMD_MSG_ROWGEMM", "1")
+    rng = np.random.default_rng(31)
+    for box, n_at, P in [(np.zeros(3), 23, 3), (np.array([12.5, 13.0, 12.2]), 700, 2)]:
+        x = rng.uniform(0, 1, (1, n_at, 3)) * (box if box[0] > 0 else 4.5)
+        sp = rng.integers(0, 3, n_at).astype(np.int32)
+        spec = _biased_spec(64, 128, 3, 3.0, 1.0 / 12.0, 0.2)
+        spec.gemm_dtype = 1
+        gpu, ref = make_pair(sp, x, box, P, 300.0, 0.25, 1.0, 0, spec)
+        spread_beads(gpu, ref, scale=0.05)
+        a = gpu.forces().clone()
+        Fg, Fr = a.cpu().numpy().astype(np.float64), ref.forces()
+        gross = ref.force_gross()
+        err = np.abs(Fg - Fr).max(axis=-1)
+        assert np.all(err <= 2.0 ** -8 * gross + 1e-6), (n_at, (err / (gross + 1e-30)).max())
+        for _ in range(3):
+            assert torch.equal(a, gpu.forces())
