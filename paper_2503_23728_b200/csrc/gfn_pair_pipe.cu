@@ -18,7 +18,7 @@
 // passes and the force head) replace P, H and the first product by
 //   L   1 warp                 : two TMA bulk copies per tile bring the A2 image and the meta record back
 // and the head runs its channel reduction on the tensor core:
-//   E   (head)                 : act = SiLU(W_fe h1 + b_fe + G_i + G_j) written as a bf16 K-major operand A3
+//   E   (head)                 : act = SiLU(W_fe h1 + b_fe + G_i + G_j) written as a bf16 MN-major operand A3 (pairs contiguous)
 //   MMA                        : D3[p][.] = act[p][:] . w_f2   (8 x UMMA 128x16x16)
 //   F   4 warps, thread = pair : s_p from D3 -> c_ij s_ij u_ij, segmented warp scan over 32-pair granules -> forces.
 // (When L = 0 the head is the first pass; it then reduces over channels with a fixed shuffle tree.)
@@ -291,6 +291,14 @@ __device__ __forceinline__ void role_H(const PairArgs &a, unsigned char *S, uint
     STATS_END("H")
 }
 
+// UMMA shared-memory descriptor, MN-major operand (the contraction index is the shared-memory row), 128-byte swizzle:
+// LBO = bytes between 64-element atoms along M/N, SBO = bytes between 8-row groups along K
+__device__ __forceinline__ uint64_t make_desc_mn_sw128(uint32_t addr, uint32_t lbo, uint32_t sbo)
+{
+    return (uint64_t)((addr >> 4) & 0x3FFF) | ((uint64_t)((lbo >> 4) & 0x3FFF) << 16) | ((uint64_t)((sbo >> 4) & 0x3FFF) << 32) |
+           ((uint64_t)1 << 46) | ((uint64_t)2 << 61);
+}
+
 // ---- role E, message pass: m_i = agg_norm sum_j c_ij (e0_ij + E_i + E_j) (.) x_j  (S:G3, G5).
 // D2 is TRANSPOSED (TMEM lane = channel c, column = pair): the thread walks the 32 pairs of its quarter tile in CSR
 // order.  With wx = c_ij x_j:  m_i = sum_j (e0 + E_j) wx + (b + E_i) sum_j wx, so the two private running sums do not
@@ -561,7 +569,7 @@ __device__ __forceinline__ void role_E_head(const PairArgs &a, unsigned char *S,
 }
 
 // ---- role E, force head with the channel reduction on the tensor core (HEAD, MODE 1):
-// act[p][c] = SiLU(W_fe h1 + b_fe + G_i + G_j)[c] is written as a bf16 K-major operand (A3); the MMA warp forms
+// act[p][c] = SiLU(W_fe h1 + b_fe + G_i + G_j)[c] is written as a bf16 MN-major operand (A3: row = channel, pairs contiguous); the MMA warp forms
 // D3[p][.] = act[p][:] . w_f2 (128x16x128), and role F turns s_p into forces.  No shuffles, no CTA-wide barrier.
 __device__ __forceinline__ void role_E_head_tc(const PairArgs &a, unsigned char *S, uint64_t *bar, uint32_t tmem, int n_my, int c,
                                                int qt, int lane, bool poller)
@@ -570,7 +578,7 @@ __device__ __forceinline__ void role_E_head_tc(const PairArgs &a, unsigned char 
     const float b2c = 0.5f * ((const float *)(S + OFF_BIAS))[H + c];
     const float *__restrict__ Gf = (const float *)a.gsrc;
     const uint32_t lane_field = (uint32_t)(c & ~31) << 16;
-    const int a3_off = (c >> 6) * 16384 + (c & 7) * 2, a3_ch = (c & 63) >> 3;
+    const int a3_off = (c >> 3) * 1024 + (c & 7) * 128;      // A3 is MN-major (pairs contiguous): row = channel, 8-channel groups 1 KB apart
     int nx_row = -1;
     float nx_val = 0.f;
     for (int it = 0; it < n_my; ++it) {
@@ -670,10 +678,16 @@ __device__ __forceinline__ void role_E_head_tc(const PairArgs &a, unsigned char 
                 }
             }
             if (it + 1 < n_my) tc::named_bar_arrive(NB_SLOT + slot, 160);
-            // act -> A3 (row = pair, K-major, 16-byte chunks XOR-swizzled by row & 7; (q0 + e) & 7 = e & 7)
-#pragma unroll
-            for (int e = 0; e < 16; ++e)
-                *(__nv_bfloat16 *)(A3 + (q0 + e) * 128 + ((a3_ch ^ (e & 7)) << 4)) = __float2bfloat16_rn(v[e]);
+            // act -> A3: the thread's 16 pairs are two 16-byte chunks of its channel's row (64-pair atoms 16 KB apart,
+            // chunks XOR-swizzled by channel & 7): two 128-bit stores instead of sixteen 16-bit ones
+            {
+                unsigned char *row = A3 + (q0 >> 6) * 16384;
+                const int ch0 = (q0 & 63) >> 3;
+                *(uint4 *)(row + ((ch0 ^ (c & 7)) << 4)) =
+                    make_uint4(tc::pack_bf16(v[0], v[1]), tc::pack_bf16(v[2], v[3]), tc::pack_bf16(v[4], v[5]), tc::pack_bf16(v[6], v[7]));
+                *(uint4 *)(row + (((ch0 + 1) ^ (c & 7)) << 4)) =
+                    make_uint4(tc::pack_bf16(v[8], v[9]), tc::pack_bf16(v[10], v[11]), tc::pack_bf16(v[12], v[13]), tc::pack_bf16(v[14], v[15]));
+            }
         }
         tc::fence_proxy_async_smem();
         __syncwarp();
@@ -779,9 +793,9 @@ __device__ __forceinline__ void role_MMA(const PairArgs &a, unsigned char *S, ui
             if (lane == 0) {
                 const uint32_t sA3 = s ? sA1 : sA2 + 32768;
 #pragma unroll
-                for (int kk = 0; kk < H / 16; ++kk)
-                    tc::mma_bf16_ss(tmem + s * 32, tc::make_desc_sw128(sA3 + (kk >> 2) * 16384 + (kk & 3) * 32),
-                                    tc::make_desc_sw128(sW1 + (kk >> 2) * 2048 + (kk & 3) * 32), idesc16, kk > 0);
+                for (int kk = 0; kk < H / 16; ++kk)      // A3 MN-major: a K step is two 8-channel groups (2 KB); 64-pair atoms 16 KB apart
+                    tc::mma_bf16_ss(tmem + s * 32, make_desc_mn_sw128(sA3 + kk * 2048, 16384, 1024),
+                                    tc::make_desc_sw128(sW1 + (kk >> 2) * 2048 + (kk & 3) * 32), idesc16 | (1u << 15), kk > 0);
                 tc::mma_commit(&bar[D3_FULL + s]);
                 tc::mma_commit(&bar[A3_EMPTY + s]);
             }
@@ -1048,17 +1062,11 @@ __device__ __forceinline__ void role_R(const PairArgs &a, unsigned char *S, uint
         const uint64_t bdesc = desc_mn(tc::smem_u32(S + OFF_A2 + s * 32768 + kb * 2048), 16384, 1024);
         int lo = 0;
         bool have_token = false;
-#ifdef GFN_PIPE_STATS
-        long long tcs_ = 0;
-#endif
 #pragma unroll 1
         while (true) {                                       // one A block per row segment that the block touches
             const int hi = bnd ? (__ffs(bnd) - 1) : 16;
             WAITEDK(2, tc::mbar_wait_spin(&bar[AB_EMPTY + kb], (use & 1) ^ 1));    // own products of the last A block have read the slot
             ++use;
-#ifdef GFN_PIPE_STATS
-            const long long tr0_ = clock64();
-#endif
             unsigned char *dst = S + OFF_AB + kb * 8192;
 #pragma unroll
             for (int rr = 0; rr < 4; ++rr) {
@@ -1075,17 +1083,11 @@ __device__ __forceinline__ void role_R(const PairArgs &a, unsigned char *S, uint
             }
             tc::fence_proxy_async_smem();
             __syncwarp();
-#ifdef GFN_PIPE_STATS
-            g_wk_[0] += clock64() - tr0_;
-#endif
             if (!have_token) {
                 WAITED(tc::mbar_wait_spin(&bar[A2_FULL + s], (it >> 1) & 1));     // h1 rows of the tile
                 // token: every product of the earlier blocks (and tiles) has been issued
                 if (kb > 0 || it > 0) tc::named_bar_sync(NB_TOKEN + kb, 64);
                 have_token = true;
-#ifdef GFN_PIPE_STATS
-                tcs_ = clock64();
-#endif
             }
             const int row = row_of(M.rowk[kb * 16 + lo]);
             const bool seg_start = (lo > 0) || (starts & 1u);
@@ -1114,9 +1116,6 @@ __device__ __forceinline__ void role_R(const PairArgs &a, unsigned char *S, uint
             bnd &= bnd - 1;
             lo = hi;
         }
-#ifdef GFN_PIPE_STATS
-        g_wk_[3] += clock64() - tcs_;
-#endif
         if (kb < 7 || it + 1 < n_my) tc::named_bar_arrive(NB_TOKEN + ((kb + 1) & 7), 64);   // next block (or block 0 of the next tile) may issue
         if (lane == 0) {
             tc::mma_commit(&bar[A2_EMPTY + s]);              // h1 tile free once the products of all eight blocks have completed
