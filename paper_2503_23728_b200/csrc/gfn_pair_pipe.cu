@@ -77,7 +77,7 @@ constexpr int NSLOT = 4;     // quarter tiles; the gather ring has two 16-pair s
 //   MODE 0           : P 0-3, H 4-7, E 8-23, MMA 24, G 25-28, S 29, idle 30-31 (32 warps, 64 registers at launch; setmaxnreg
 //                      moves registers from the P, H, MMA/G/S warpgroups (56, 56, 40) to the four E warpgroups (80))
 //   MODE 1, message  : E 0-15, G 16-19, MMA 20, L 21                          (22 warps, 80 registers used)
-//   MODE 1, head     : E 0-15, F 16-19, G 20-23, MMA 24, L 25                 (26 warps, 71 registers used)
+//   MODE 1, head     : E 0-15, F 16-19, G 20-23, MMA 24, L 25, idle 26-27     (28 warps, 72 at launch; setmaxnreg: E 88, F 56, rest 40)
 // E and F/H warps start at a multiple of 4: warp % 4 is the TMEM lane quadrant a warp may access.
 template <bool HEAD, int MODE>
 struct Warps {
@@ -86,7 +86,7 @@ struct Warps {
     static constexpr int G0 = (MODE == 0) ? 25 : (HEAD ? 20 : 16);
     static constexpr int MMA = (MODE == 0) ? 24 : (HEAD ? 24 : 20);
     static constexpr int SL = (MODE == 0) ? 29 : MMA + 1;                // S (MODE 0) or L (MODE 1)
-    static constexpr int N = (MODE == 0) ? 32 : SL + 1;                  // MODE 0: whole warpgroups (setmaxnreg), warps 30-31 idle
+    static constexpr int N = (MODE == 0) ? 32 : (HEAD ? 28 : SL + 1);    // whole warpgroups where setmaxnreg is used; the last warps are idle
     static constexpr int THREADS = N * 32;
 };
 
@@ -925,6 +925,11 @@ __global__ void __launch_bounds__(Warps<HEAD, MODE>::THREADS, 1) pair_pipe_kerne
     if (MODE == 0) {                               // register re-balancing between warpgroups (aligned groups of 4 warps)
         if (warp < 8) asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
         else if (warp < 24) asm volatile("setmaxnreg.inc.sync.aligned.u32 80;");
+        else asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
+    } else if (HEAD) {                             // 28 warps, 72 at launch: F 56, G and MMA/L 40 -> E 88  (measured: no gain for the
+                                                   // later message passes, which run 22 warps at 80 registers)
+        if (warp < 16) asm volatile("setmaxnreg.inc.sync.aligned.u32 88;");
+        else if (warp < 20) asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
         else asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
     }
     if (MODE == 0 && warp < 4) {
