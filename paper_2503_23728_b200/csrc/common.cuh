@@ -1,6 +1,7 @@
 // common.cuh -- shared declarations of the sm_100a PIMD library (host context, device views).
 // Product code: shares nothing with oracle/.
 #pragma once
+#include <cuda.h>            // CUtensorMap (type only: the encoder is fetched through cudaGetDriverEntryPoint)
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <stddef.h>
@@ -91,6 +92,7 @@ struct pimd_ctx {
     float h_be1_half[128];             // HOST copy of b_e1 / 2 (passed to the pair kernels as kernel parameters)
     unsigned char *h1_img, *meta_img;  // [pair_cap/128 + 1] tile images kept between the pair passes of one evaluation (tc path)
     uint32_t *XE;                      // [rows][H] packed bf16 (x | E << 16) gathered by the pair kernels (aliases xfeat)
+    CUtensorMap tmap_xe, tmap_g;       // 2-D tensor maps [rows][128 x 32 bit] of XE and G for TMA tile::gather4 (four gathered rows per copy)
     float *nfeat, *xfeat, *mfeat, *Efeat, *Gfeat;   // [rows][H]
     float *carry_m;                    // [n_gran_m][2][H]
     float *carry_f;                    // [n_gran_f][2][4]

@@ -10,7 +10,7 @@
 //   MMA 1 thread               : D1 = A1 (W_e1/2)^T  (4 x UMMA 128x128x16);  D2^T = W2 A2^T  (8 x UMMA), W2 = W_e2 or W_f1 W_e2/2
 //   H   4 warps, thread = pair : D1 (TMEM) + b -> SiLU -> A2 (bf16 operand of the second product)
 //   S   1 warp                 : TMA bulk stores of the tile's A2 image (32 KB) and meta record to HBM
-//   G   4 warps                : TMA bulk copies of the gathered rows (x_j|E_j packed bf16, or G_j fp32; 512 B per pair)
+//   G   4 warps                : TMA tile::gather4 copies of the gathered rows (x_j|E_j packed bf16, or G_j fp32; 4 x 512 B per copy)
 //                                into an 8-slot shared-memory ring, 16 pairs per slot
 //   E   16 warps, thread = (channel, quarter tile): D2^T (TMEM lane = channel) -> e_ij = e0_ij + E_i + E_j (S:G5) ->
 //                                private running sums over CSR row segments, cut at row boundaries.
@@ -91,6 +91,7 @@ struct Warps {
 };
 
 struct PairArgs {
+    alignas(64) CUtensorMap gmap;         // the gathered table (XE or G) as a 2-D tensor [rows][128 x 32 bit] for TMA tile::gather4
     int N, periodic;
     double box[3], inv_box[3];
     float r_cut, wscale;
@@ -812,13 +813,13 @@ template <int SLOT_THREADS>   // threads on the slot-consumed barrier: the consu
 __device__ __forceinline__ void role_G(const PairArgs &a, unsigned char *S, uint64_t *bar, int n_my, int qt, int lane)
 {
     STATS_BEGIN
-    const unsigned char *src = (const unsigned char *)a.gsrc;
     const int slot = qt * 2 + (lane >> 4);       // lanes 0-15 feed slot 2 qt, lanes 16-31 slot 2 qt + 1
     unsigned char *dst = S + OFF_RING + slot * 8192 + (lane & 15) * 512;
     for (int it = 0; it < n_my; ++it) {
         const Meta &M = meta_of(S, it);
         WAITED(tc::mbar_wait(&bar[META_FULL + (it & (NM - 1))], (it / NM) & 1));
         const int jrow = M.jrow[qt * 32 + lane];
+        const int j1 = __shfl_down_sync(FULL, jrow, 1), j2 = __shfl_down_sync(FULL, jrow, 2), j3 = __shfl_down_sync(FULL, jrow, 3);
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
             if (it > 0) {                                    // the consumers have read the slot
@@ -827,7 +828,8 @@ __device__ __forceinline__ void role_G(const PairArgs &a, unsigned char *S, uint
             }
             if (lane == 16 * h) tc::mbar_arrive_expect_tx(&bar[XE_FULL + qt * 2 + h], 8192);
             __syncwarp();
-            if ((lane >> 4) == h) tc::bulk_g2s(dst, src + (size_t)jrow * 512, 512, &bar[XE_FULL + slot]);
+            // four gathered rows (4 x 512 B, consecutive in the slot) per copy: lanes 0, 4, 8, 12 of the half warp issue
+            if ((lane >> 4) == h && (lane & 3) == 0) tc::tma_gather4(dst, &a.gmap, jrow, j1, j2, j3, &bar[XE_FULL + slot]);
         }
     }
     STATS_END("G")
@@ -1291,6 +1293,7 @@ int launch_pair_pipe(pimd_ctx *c, bool head, bool first)
     a.wf2 = c->net.wf2; a.bf2 = c->net.bf2;
     a.m_out = c->mfeat; a.carry_m = c->carry_m; a.Fraw = c->Fraw; a.carry_f = c->carry_f;
     a.h1_img = c->h1_img; a.meta_img = c->meta_img;
+    a.gmap = head ? c->tmap_g : c->tmap_xe;
     a.W2T = c->net.We2T; a.Emaster = c->Efeat;
     const size_t smem = SMEM_BYTES + 1024;
     static bool attr = false;

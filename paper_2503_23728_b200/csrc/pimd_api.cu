@@ -447,6 +447,25 @@ extern "C" int pimd_create(pimd_ctx **out, int n_atoms, int n_replicas, const in
             // atom-wise layers: five images per layer; SiLU's 1/2 folded into W_vn, W_vm
             c->wimg_node = (uint16_t *)(ws + L.wimg_node); c->xs0 = (float *)(ws + L.xs0);
             c->XE = (uint32_t *)c->xfeat;
+            {   // tensor maps of the two gathered tables (rows of 512 B; box = one row; used with tile::gather4)
+                typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                              const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                              CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+                void *fn = nullptr;
+                cudaDriverEntryPointQueryResult qres;
+                CREATE_CHECK(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
+                if (!fn || qres != cudaDriverEntryPointSuccess) { pimd_set_error("cuTensorMapEncodeTiled is not available in this driver"); delete c; return PIMD_ERR_CUDA; }
+                const cuuint64_t gdim[2] = {128, (cuuint64_t)c->rows};
+                const cuuint64_t gstr[1] = {512};
+                const cuuint32_t box[2] = {128, 1}, estr[2] = {1, 1};
+                void *bases[2] = {c->XE, c->Gfeat};
+                CUtensorMap *maps[2] = {&c->tmap_xe, &c->tmap_g};
+                for (int t = 0; t < 2; ++t) {
+                    const CUresult rc = ((encode_fn)fn)(maps[t], CU_TENSOR_MAP_DATA_TYPE_UINT32, 2, bases[t], gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                                        CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                    if (rc != CUDA_SUCCESS) { pimd_set_error("cuTensorMapEncodeTiled failed (%d)", (int)rc); delete c; return PIMD_ERR_CUDA; }
+                }
+            }
             c->h1_img = (unsigned char *)(ws + L.h1_img); c->meta_img = (unsigned char *)(ws + L.meta_img);
             for (int k = 0; k < H && k < 128; ++k) c->h_be1_half[k] = 0.5f * raw.be1[k];
             const int Ln = net->n_layers;

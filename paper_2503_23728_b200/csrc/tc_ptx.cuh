@@ -108,6 +108,16 @@ __device__ __forceinline__ void bulk_g2s(void *smem_dst, const void *gsrc, uint3
                  : "memory");
 }
 
+// TMA gather: four rows r0..r3 of a 2-D tensor (tensor map with box = one row; column offset 0) land consecutively at
+// smem_dst; completes on `bar` with 4 x row bytes.  `tmap` must live in kernel-parameter (__grid_constant__) or global memory.
+__device__ __forceinline__ void tma_gather4(void *smem_dst, const void *tmap, int r0, int r1, int r2, int r3, uint64_t *bar)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.tile::gather4.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5, %6}], [%7];"
+        ::"r"(smem_u32(smem_dst)), "l"(tmap), "r"(0), "r"(r0), "r"(r1), "r"(r2), "r"(r3), "r"(smem_u32(bar))
+        : "memory");
+}
+
 // TMA bulk copy shared -> global (bulk async-group completion)
 __device__ __forceinline__ void bulk_s2g(void *gdst, const void *smem_src, uint32_t bytes)
 {
