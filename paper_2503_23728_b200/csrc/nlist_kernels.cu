@@ -155,14 +155,19 @@ __device__ __forceinline__ bool within_cutoff_fast3(const double qi[3], double x
 // fixed-stride scratch; the row's running count lives in nnz[] between chunks.
 constexpr int CAND_CHUNK = 1024, COUNT_THREADS = 128, HOME_MAX = 128;
 
+// WRAP = false when every periodic axis has at least four cells: home atom and candidate are both stored relative to the same
+// reference atom (minimum image), the candidate's cell is at most one cell away from the home cell, so |dx| < 3 cells; when
+// |dx| > L/2 the other image is farther than L - 3 L/nc >= one cell width >= r_c: not a neighbour with either image, and the
+// per-pair image shift can be left out.
+template <bool WRAP>
 __global__ void __launch_bounds__(COUNT_THREADS) count_cell_kernel(NlArgs a)
 {
-    __shared__ int sj[CAND_CHUNK], sp[CAND_CHUNK];   // candidate atom index; position in the cell-ordered arrays
+    __shared__ int sp[CAND_CHUNK];             // candidate: position in the cell-ordered arrays
     __shared__ int cfirst[28], cpre[28];       // first sorted position (relative to the system) and prefix count per stencil cell
     __shared__ int n_st;
     __shared__ double hq[3][HOME_MAX];         // atoms of the home cell (the first HOME_MAX; the rest are read from global)
     __shared__ int hj[HOME_MAX];
-    __shared__ float sqf[3][CAND_CHUNK];       // candidate positions relative to the cell's reference atom (minimum image), fp32
+    __shared__ float4 sc[CAND_CHUNK];          // candidate: position relative to the cell's reference atom (minimum image, fp32) | atom index
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int sys = blockIdx.x / a.nct, cell = blockIdx.x - sys * a.nct;
     const int *start = a.d.cell_start + (size_t)sys * (a.nct + 1);
@@ -226,14 +231,15 @@ __global__ void __launch_bounds__(COUNT_THREADS) count_cell_kernel(NlArgs a)
             int k = 0;
             while (idx >= cpre[k + 1]) ++k;    // <= 27 steps
             const int64_t pos = sbase + cfirst[k] + (idx - cpre[k]);
-            sj[t] = a.d.sorted_atom[pos];
             sp[t] = (int)(pos - sbase);
+            float rel[3];
 #pragma unroll
             for (int ax = 0; ax < 3; ++ax) {
                 double d = a.d.sorted_q[pos * 3 + ax] - ref[ax];          // once per candidate and cell: fp64 image shift, then fp32
                 if (a.periodic) d -= a.box[ax] * rint(d / a.box[ax]);
-                sqf[ax][t] = (float)d;
+                rel[ax] = (float)d;
             }
+            sc[t] = make_float4(rel[0], rel[1], rel[2], __int_as_float(a.d.sorted_atom[pos]));   // one 128-bit load per test
         }
         __syncthreads();
         const bool last = base + CAND_CHUNK >= total;
@@ -257,16 +263,20 @@ __global__ void __launch_bounds__(COUNT_THREADS) count_cell_kernel(NlArgs a)
                 bool hit = false;
                 int j = -1;
                 if (s < n) {
-                    j = sj[s];
+                    const float4 cj = sc[s];
+                    const float cq[3] = {cj.x, cj.y, cj.z};
+                    j = __float_as_int(cj.w);
                     // fp32 estimate of d^2 from the relative coordinates (|.| <= L/2 each, so one wrap suffices): its
                     // error is orders of magnitude below the 1e-3 band; inside the band the exact S:L3 sequence decides
                     float d2 = 0.f;
 #pragma unroll
                     for (int ax = 0; ax < 3; ++ax) {
-                        float dx = sqf[ax][s] - qif[ax];
-                        float sh = (dx > hbx[ax]) ? bxf[ax] : 0.f;      // selects, not branches (hbx = +inf when not periodic)
-                        sh = (dx < -hbx[ax]) ? -bxf[ax] : sh;
-                        dx -= sh;
+                        float dx = cq[ax] - qif[ax];
+                        if (WRAP) {
+                            float sh = (dx > hbx[ax]) ? bxf[ax] : 0.f;  // selects, not branches (hbx = +inf when not periodic)
+                            sh = (dx < -hbx[ax]) ? -bxf[ax] : sh;
+                            dx -= sh;
+                        }
                         d2 = fmaf(dx, dx, d2);
                     }
                     if (j != i && d2 <= rc2_hi)   // in the band (about 0.2 % of the candidates): fp64 positions from global
@@ -408,7 +418,9 @@ int pimd_launch_nlist(pimd_ctx *c)
     bin_kernel<<<gthr, 256, 0, c->stream>>>(a);
     scan_cells_kernel<<<a.nsys, 256, 0, c->stream>>>(a);
     scatter_kernel<<<gthr, 256, 0, c->stream>>>(a);
-    count_cell_kernel<<<(unsigned)(a.nsys * a.nct), COUNT_THREADS, 0, c->stream>>>(a);
+    const bool wrap = a.periodic && (a.nc[0] < 4 || a.nc[1] < 4 || a.nc[2] < 4);
+    if (wrap) count_cell_kernel<true><<<(unsigned)(a.nsys * a.nct), COUNT_THREADS, 0, c->stream>>>(a);
+    else count_cell_kernel<false><<<(unsigned)(a.nsys * a.nct), COUNT_THREADS, 0, c->stream>>>(a);
     scan_rows_local_kernel<<<nblk, 1024, 0, c->stream>>>(a);
     scan_block_sums_kernel<<<1, 1024, 0, c->stream>>>(a, nblk);
     scan_rows_add_kernel<<<gthr, 256, 0, c->stream>>>(a);
