@@ -150,9 +150,10 @@ __device__ __forceinline__ bool within_cutoff_fast3(const double qi[3], double x
 }
 
 // One CTA per (bead-system, cell).  The atoms of the cell's de-duplicated 3x3x3 stencil are staged in shared memory
-// once (index + fp64 position, CAND_CHUNK at a time) and every atom of the home cell is tested against them by one warp:
-// the candidates are read from HBM/L2 once per cell instead of once per row.  Hits are parked, unsorted, in the row's
-// fixed-stride scratch; the row's running count lives in nnz[] between chunks.
+// once (index + fp32 position relative to the cell's first atom, CAND_CHUNK at a time); a lane is a home atom and the four
+// warps share the candidates, so one broadcast 128-bit shared-memory load serves 32 tests.  The candidates are read from
+// HBM/L2 once per cell instead of once per row.  Hits are parked, unsorted, in the row's fixed-stride scratch through a
+// shared-memory counter per home atom (integer atomics: the order varies, the fill kernel sorts).
 constexpr int CAND_CHUNK = 1024, COUNT_THREADS = 128, HOME_MAX = 128;
 
 // WRAP = false when every periodic axis has at least four cells: home atom and candidate are both stored relative to the same
@@ -167,6 +168,7 @@ __global__ void __launch_bounds__(COUNT_THREADS) count_cell_kernel(NlArgs a)
     __shared__ int n_st;
     __shared__ double hq[3][HOME_MAX];         // atoms of the home cell (the first HOME_MAX; the rest are read from global)
     __shared__ int hj[HOME_MAX];
+    __shared__ int scnt[HOME_MAX];             // hits per home atom so far
     __shared__ float4 sc[CAND_CHUNK];          // candidate: position relative to the cell's reference atom (minimum image, fp32) | atom index
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int sys = blockIdx.x / a.nct, cell = blockIdx.x - sys * a.nct;
@@ -210,8 +212,10 @@ __global__ void __launch_bounds__(COUNT_THREADS) count_cell_kernel(NlArgs a)
             cpre[ns] = tot;
             n_st = ns;
         }
-        for (int t = tid; t < nh && t < HOME_MAX; t += COUNT_THREADS) {   // home atoms
+        for (int t = tid; t < nh; t += COUNT_THREADS) {                   // home atoms
             const int64_t posi = sbase + h0 + t;
+            if (t >= HOME_MAX) { a.d.nnz[sbase + a.d.sorted_atom[posi]] = 0; continue; }   // (very full cells: counter in global memory)
+            scnt[t] = 0;
             hj[t] = a.d.sorted_atom[posi];
             hq[0][t] = a.d.sorted_q[posi * 3]; hq[1][t] = a.d.sorted_q[posi * 3 + 1]; hq[2][t] = a.d.sorted_q[posi * 3 + 2];
         }
@@ -242,59 +246,60 @@ __global__ void __launch_bounds__(COUNT_THREADS) count_cell_kernel(NlArgs a)
             sc[t] = make_float4(rel[0], rel[1], rel[2], __int_as_float(a.d.sorted_atom[pos]));   // one 128-bit load per test
         }
         __syncthreads();
-        const bool last = base + CAND_CHUNK >= total;
-        for (int ha = warp; ha < nh; ha += COUNT_THREADS / 32) {
-            const int64_t posi = sbase + h0 + ha;
-            const bool in_s = ha < HOME_MAX;     // warp-uniform
-            const int i = in_s ? hj[ha] : a.d.sorted_atom[posi];
-            const int64_t row = sbase + i;
-            const double qi[3] = {in_s ? hq[0][ha] : a.d.sorted_q[posi * 3], in_s ? hq[1][ha] : a.d.sorted_q[posi * 3 + 1],
-                                  in_s ? hq[2][ha] : a.d.sorted_q[posi * 3 + 2]};
+        // lane = home atom (groups of 32), the four warps share the candidates: one broadcast 128-bit load serves 32 tests.
+        // Hits are appended to the row's scratch through a shared-memory counter (their order is free: the fill kernel sorts).
+        for (int hg = 0; hg < nh; hg += 32) {
+            const int ha = hg + lane;
+            const bool act = ha < nh, in_s = ha < HOME_MAX;
+            const int64_t posi = sbase + h0 + (act ? ha : 0);
+            const int i = !act ? -1 : (in_s ? hj[ha] : a.d.sorted_atom[posi]);
+            const int64_t row = sbase + (act ? i : 0);
             int *buf = a.d.hits + row * a.hit_stride;
-            int cnt_i = (base == 0) ? 0 : a.d.nnz[row];
             float qif[3];
 #pragma unroll
             for (int ax = 0; ax < 3; ++ax) {
-                double d = qi[ax] - ref[ax];
+                double d = ((act && in_s) ? hq[ax][ha] : a.d.sorted_q[posi * 3 + ax]) - ref[ax];
                 if (a.periodic) d -= a.box[ax] * rint(d / a.box[ax]);
                 qif[ax] = (float)d;
             }
-            for (int s = lane; s - lane < n; s += 32) {
-                bool hit = false;
-                int j = -1;
-                if (s < n) {
-                    const float4 cj = sc[s];
-                    const float cq[3] = {cj.x, cj.y, cj.z};
-                    j = __float_as_int(cj.w);
-                    // fp32 estimate of d^2 from the relative coordinates (|.| <= L/2 each, so one wrap suffices): its
-                    // error is orders of magnitude below the 1e-3 band; inside the band the exact S:L3 sequence decides
-                    float d2 = 0.f;
+            for (int s0 = warp; s0 < n; s0 += COUNT_THREADS / 32) {
+                const float4 cj = sc[s0];
+                const float cq[3] = {cj.x, cj.y, cj.z};
+                const int j = __float_as_int(cj.w);
+                // fp32 estimate of d^2 from the relative coordinates: its error is orders of magnitude below the 1e-3 band;
+                // inside the band the exact S:L3 sequence decides
+                float d2 = 0.f;
 #pragma unroll
-                    for (int ax = 0; ax < 3; ++ax) {
-                        float dx = cq[ax] - qif[ax];
-                        if (WRAP) {
-                            float sh = (dx > hbx[ax]) ? bxf[ax] : 0.f;  // selects, not branches (hbx = +inf when not periodic)
-                            sh = (dx < -hbx[ax]) ? -bxf[ax] : sh;
-                            dx -= sh;
-                        }
-                        d2 = fmaf(dx, dx, d2);
+                for (int ax = 0; ax < 3; ++ax) {
+                    float dx = cq[ax] - qif[ax];
+                    if (WRAP) {
+                        float sh = (dx > hbx[ax]) ? bxf[ax] : 0.f;      // selects, not branches (hbx = +inf when not periodic)
+                        sh = (dx < -hbx[ax]) ? -bxf[ax] : sh;
+                        dx -= sh;
                     }
-                    if (j != i && d2 <= rc2_hi)   // in the band (about 0.2 % of the candidates): fp64 positions from global
-                        hit = (d2 < rc2_lo) || within_cutoff(qi, a.d.sorted_q + (sbase + sp[s]) * 3, a);
+                    d2 = fmaf(dx, dx, d2);
                 }
-                const unsigned m = __ballot_sync(0xffffffffu, hit);
-                if (hit) {
-                    const int idx = cnt_i + __popc(m & ((1u << lane) - 1u));
-                    if (idx < a.hit_stride) buf[idx] = j;
+                if (act && j != i && d2 <= rc2_hi) {
+                    bool hit = d2 < rc2_lo;
+                    if (!hit) {                  // in the band (about 0.2 % of the candidates): fp64 positions
+                        const double qi[3] = {in_s ? hq[0][ha] : a.d.sorted_q[posi * 3], in_s ? hq[1][ha] : a.d.sorted_q[posi * 3 + 1],
+                                              in_s ? hq[2][ha] : a.d.sorted_q[posi * 3 + 2]};
+                        hit = within_cutoff(qi, a.d.sorted_q + (sbase + sp[s0]) * 3, a);
+                    }
+                    if (hit) {
+                        const int idx = in_s ? atomicAdd(&scnt[ha], 1) : atomicAdd(&a.d.nnz[row], 1);
+                        if (idx < a.hit_stride) buf[idx] = j;
+                    }
                 }
-                cnt_i += __popc(m);
-            }
-            if (lane == 0) {
-                if (last && cnt_i > a.hit_stride) { atomicOr(a.err, PIMD_FLAG_PAIRS); cnt_i = a.hit_stride; }
-                a.d.nnz[row] = cnt_i;
             }
         }
         __syncthreads();
+    }
+    for (int t = tid; t < nh; t += COUNT_THREADS) {                       // counts; a row with more hits than its scratch holds is an error
+        const int64_t row = sbase + ((t < HOME_MAX) ? hj[t] : a.d.sorted_atom[sbase + h0 + t]);
+        int cnt = (t < HOME_MAX) ? scnt[t] : a.d.nnz[row];
+        if (cnt > a.hit_stride) { atomicOr(a.err, PIMD_FLAG_PAIRS); cnt = a.hit_stride; }
+        a.d.nnz[row] = cnt;
     }
 }
 
