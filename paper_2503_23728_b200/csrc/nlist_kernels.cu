@@ -262,6 +262,7 @@ __global__ void __launch_bounds__(COUNT_THREADS) count_cell_kernel(NlArgs a)
                 if (a.periodic) d -= a.box[ax] * rint(d / a.box[ax]);
                 qif[ax] = (float)d;
             }
+#pragma unroll 4
             for (int s0 = warp; s0 < n; s0 += COUNT_THREADS / 32) {
                 const float4 cj = sc[s0];
                 const float cq[3] = {cj.x, cj.y, cj.z};
