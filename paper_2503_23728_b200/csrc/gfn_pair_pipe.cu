@@ -968,14 +968,16 @@ __global__ void __launch_bounds__(Warps<HEAD, MODE>::THREADS, 1) pair_pipe_kerne
 // already in the right shared-memory form), and W_e2 is applied once per row by the epilogue (fp32, one register per k).
 // s and t are products of the same A operands with a block of ones.  The node kernel delivers x and y = E (.) x as two
 // bf16 rows per atom.  Roles (one persistent CTA per SM, 128-pair tiles, 16-pair K blocks):
-//   L   1 warp   : TMA bulk copies of the tile's h1 image (B operand, 32 KB) and meta record
-//   G   4 warps  : TMA bulk copies of the gathered rows (x_j | y_j, 512 B per pair) into an 8-slot staging ring
-//   R   8 warps  : (one per K block of a tile) staging -> A blocks: scale by c_ij (bf16x2), 128-byte swizzle, zero the pairs outside the row
-//                  segment (a block that straddles row boundaries is written once per segment)
-//   MMA 1 thread : per A block T += x'^T h1, s += x'^T 1, t += y'^T 1 into one of three TMEM accumulators (160 columns);
-//                  a row segment ends at a row boundary or at the end of the tile
+//   LT, LM 2 warps : TMA bulk copies of the tile's h1 image (B operand, 32 KB, two stages) and of the meta records (four ahead)
+//   G   4 warps  : TMA tile::gather4 copies of the gathered rows (x_j | y_j, 512 B per pair) into an 8-slot staging ring
+//   R   8 warps  : warp kb owns K block kb of every tile: staging -> A block (scale by c_ij as bf16x2, 128-byte swizzle, zero the
+//                  pairs outside the row segment; a block that straddles row boundaries is written once per segment), then it
+//                  ISSUES the block's products T += x'^T h1, s += x'^T 1, t += y'^T 1 into one of three TMEM accumulators
+//                  (160 columns).  The eight warps issue in block order through a token chain of named barriers, so the
+//                  accumulation order is fixed.  A row segment ends at a row boundary or at the end of the tile.
 //   E   4 warps  : thread = channel = TMEM lane: the 128 columns of T against W_e2[c][:] held in registers, + s, t terms;
 //                  direct store or carry slot (granule = tile).
+// Experimental (PIMD_MSG_ROWGEMM=1): correct and reproducible, slower than the default pipeline; DESIGN.md section 11 says why.
 namespace mg {
 constexpr int NA = 8;                        // A-block slots of 8 KB, one per K block of a tile: x' (2 x 2 KB halves) | y' (2 x 2 KB halves)
 constexpr int NACC = 3;                      // TMEM accumulators of 160 columns: T 0-127, s 128-143, t 144-159
