@@ -118,10 +118,23 @@ __global__ void __launch_bounds__(NTH, 1) node_tc_kernel(const __grid_constant__
 
     for (int tile = blockIdx.x; tile < a.n_tiles; tile += gridDim.x) {
         const int64_t row0 = (int64_t)tile * TR;
-        // ---- operands n, m (fp32 in HBM) -> bf16 swizzled tiles; one warp per row: coalesced 512-byte reads.
+        // ---- operands n, m (fp32 in HBM) -> bf16 swizzled tiles; m: one warp per row, coalesced 512-byte reads.
         // m_i is assembled in fixed order from the direct row or the carry slots (tail slot of the first granule, head
         // slots of the rest).  All loads of four rows are issued before the first use: the phase is latency-bound.
         {
+            // n: the masters are tile-blocked ([c / 4][row][4 floats]), so with thread = row a warp reads 512 contiguous bytes
+            // per instruction; eight loads in flight per thread (columns cgrp * 32 .. + 31), issued before everything else
+            {
+                const int nr = tid & 127, cgrp = tid >> 7;
+                const bool nok = row0 + nr < a.rows;
+                float4 nv8[8];
+#pragma unroll
+                for (int i = 0; i < 8; ++i)
+                    nv8[i] = nok ? *(const float4 *)(a.n + blk_off(row0, nr, cgrp * 32 + i * 4)) : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+                for (int i = 0; i < 8; ++i)
+                    *(uint2 *)(A0 + op_off(nr, cgrp * 32 + i * 4)) = make_uint2(tc::pack_bf16(nv8[i].x, nv8[i].y), tc::pack_bf16(nv8[i].z, nv8[i].w));
+            }
             const int k = lane * 4, wrow = tid >> 5;
             int rs[8], re[8];
 #pragma unroll
@@ -133,13 +146,12 @@ __global__ void __launch_bounds__(NTH, 1) node_tc_kernel(const __grid_constant__
             }
 #pragma unroll
             for (int it0 = 0; it0 < 8; it0 += 4) {
-                float4 nv[4], pc[4][4];
+                float4 pc[4][4];
 #pragma unroll
                 for (int j = 0; j < 4; ++j) {
                     const int it = it0 + j;
                     const int64_t row = row0 + wrow + it * 16;
                     const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
-                    nv[j] = (row < a.rows) ? *(const float4 *)(a.n + blk_off(row0, wrow + it * 16, k)) : z;
                     pc[j][0] = pc[j][1] = pc[j][2] = pc[j][3] = z;
                     if (re[it] > rs[it]) {       // warp-uniform
                         const int g0 = rs[it] / a.gran_m, g1 = (re[it] - 1) / a.gran_m;
@@ -163,9 +175,7 @@ __global__ void __launch_bounds__(NTH, 1) node_tc_kernel(const __grid_constant__
                             mv.x += t4.x; mv.y += t4.y; mv.z += t4.z; mv.w += t4.w;
                         }
                     }
-                    const int off = op_off(rr, k);
-                    *(uint2 *)(A0 + off) = make_uint2(tc::pack_bf16(nv[j].x, nv[j].y), tc::pack_bf16(nv[j].z, nv[j].w));
-                    *(uint2 *)(A1 + off) = make_uint2(tc::pack_bf16(mv.x, mv.y), tc::pack_bf16(mv.z, mv.w));
+                    *(uint2 *)(A1 + op_off(rr, k)) = make_uint2(tc::pack_bf16(mv.x, mv.y), tc::pack_bf16(mv.z, mv.w));
                 }
             }
         }
@@ -263,10 +273,14 @@ __global__ void __launch_bounds__(NTH, 1) node_tc_kernel(const __grid_constant__
                         make_float4(ee[e4 * 4], ee[e4 * 4 + 1], ee[e4 * 4 + 2], ee[e4 * 4 + 3]);
             if (!a.last) {
                 tc::tmem_ld16(tmem_d1 + lane_field + c0, v);
-                if (valid && !a.xy_rows) {
+                if (!a.xy_rows) {
+                    // A thread owns a row, so a direct store is 16 bytes per lane at a 512-byte stride (32 sectors per
+                    // instruction).  The warp's 32 x 128-byte block goes through shared memory instead (the operand tiles
+                    // are free now; 16-byte chunks XOR-swizzled by row & 7) and leaves as whole 128-byte lines below.
+                    unsigned char *xs = A0 + warp * 4096 + lane * 128;
 #pragma unroll
                     for (int e4 = 0; e4 < 4; ++e4)
-                        *(uint4 *)(a.XE + (size_t)row * H + c0 + e4 * 4) =
+                        *(uint4 *)(xs + (((j * 4 + e4) ^ (lane & 7)) << 4)) =
                             make_uint4(tc::pack_bf16(v[e4 * 4], ee[e4 * 4]), tc::pack_bf16(v[e4 * 4 + 1], ee[e4 * 4 + 1]),
                                        tc::pack_bf16(v[e4 * 4 + 2], ee[e4 * 4 + 2]), tc::pack_bf16(v[e4 * 4 + 3], ee[e4 * 4 + 3]));
                 } else if (valid) {              // two bf16 rows per atom for the row-GEMM message pass: x | y = E (.) x
@@ -286,6 +300,16 @@ __global__ void __launch_bounds__(NTH, 1) node_tc_kernel(const __grid_constant__
                 store_operand16(A1, r, c0, ee);
             }
         }
+        if (!a.last && !a.xy_rows) {             // the warp's XE block: 4 rows x 128 bytes per store instruction
+            __syncwarp();
+#pragma unroll
+            for (int it = 0; it < 8; ++it) {
+                const int rr = it * 4 + (lane >> 3), ch = lane & 7;
+                const uint4 w4 = *(const uint4 *)(A0 + warp * 4096 + rr * 128 + ((ch ^ (rr & 7)) << 4));
+                const int64_t orow = row0 + q * 32 + rr;
+                if (orow < a.rows) *(uint4 *)(a.XE + (size_t)orow * H + g * 32 + ch * 4) = w4;
+            }
+        }
         if (a.last) {
             tc::tc_fence_before_sync();
             tc::fence_proxy_async_smem();
@@ -303,11 +327,19 @@ __global__ void __launch_bounds__(NTH, 1) node_tc_kernel(const __grid_constant__
                 const int c0 = g * 32 + j * 16;
                 float v[16];
                 tc::tmem_ld16(tmem_d1 + lane_field + c0, v);
-                if (valid)
+                // through shared memory like XE (both operand tiles are free: the last product has completed), whole 128-byte lines to HBM
+                unsigned char *xs = A0 + warp * 4096 + lane * 128;
 #pragma unroll
-                    for (int e4 = 0; e4 < 4; ++e4)
-                        *(float4 *)(a.G + (size_t)row * H + c0 + e4 * 4) =
-                            make_float4(v[e4 * 4], v[e4 * 4 + 1], v[e4 * 4 + 2], v[e4 * 4 + 3]);
+                for (int e4 = 0; e4 < 4; ++e4)
+                    *(float4 *)(xs + (((j * 4 + e4) ^ (lane & 7)) << 4)) = make_float4(v[e4 * 4], v[e4 * 4 + 1], v[e4 * 4 + 2], v[e4 * 4 + 3]);
+            }
+            __syncwarp();
+#pragma unroll
+            for (int it = 0; it < 8; ++it) {
+                const int rr = it * 4 + (lane >> 3), ch = lane & 7;
+                const float4 w4 = *(const float4 *)(A0 + warp * 4096 + rr * 128 + ((ch ^ (rr & 7)) << 4));
+                const int64_t orow = row0 + q * 32 + rr;
+                if (orow < a.rows) *(float4 *)(a.G + (size_t)orow * H + g * 32 + ch * 4) = w4;
             }
         }
         tc::tc_fence_before_sync();
