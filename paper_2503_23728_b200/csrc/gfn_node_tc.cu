@@ -355,16 +355,23 @@ __global__ void node_init_tc_kernel(int64_t rows, int N, const int *__restrict__
                                     const float *__restrict__ xs0, float *__restrict__ n, float *__restrict__ E,
                                     uint32_t *__restrict__ XE)
 {
-    const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;      // over the rows rounded up to whole tiles
+    {   // tile-blocked masters: consecutive threads = consecutive rows of one 4-column group (16 contiguous bytes each)
+        const int64_t tile = idx >> 12;
+        const int c0 = (int)((idx >> 7) & 31) * 4;
+        const int64_t row = tile * 128 + (idx & 127);
+        if (row < rows) {
+            const float4 nv = __ldg((const float4 *)(Emb + (size_t)species[row % N] * H + c0));
+            const size_t o = blk_off(tile * 128, (int)(idx & 127), c0);
+            *(float4 *)(n + o) = nv;
+            *(float4 *)(E + o) = make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+    }
+    // row-major XE: consecutive threads = consecutive columns of one row
     if (idx >= rows * (H / 4)) return;
     const int64_t row = idx >> 5;
     const int c0 = (int)(idx & 31) * 4;
-    const int s = species[row % N];
-    const float4 nv = __ldg((const float4 *)(Emb + (size_t)s * H + c0));
-    const float4 xv = __ldg((const float4 *)(xs0 + (size_t)s * H + c0));
-    const size_t o = blk_off(row & ~(int64_t)127, (int)(row & 127), c0);
-    *(float4 *)(n + o) = nv;
-    *(float4 *)(E + o) = make_float4(0.f, 0.f, 0.f, 0.f);
+    const float4 xv = __ldg((const float4 *)(xs0 + (size_t)species[row % N] * H + c0));
     *(uint4 *)(XE + (size_t)row * H + c0) =
         make_uint4(tc::pack_bf16(xv.x, 0.f), tc::pack_bf16(xv.y, 0.f), tc::pack_bf16(xv.z, 0.f), tc::pack_bf16(xv.w, 0.f));
 }
@@ -373,7 +380,7 @@ int launch_node_tc(pimd_ctx *c, int mode, int layer)
 {
     const GfnDev &n = c->net;
     if (mode == 0) {
-        const int64_t work = c->rows * (H / 4);
+        const int64_t work = (c->rows + 127) / 128 * 128 * (H / 4);
         node_init_tc_kernel<<<(unsigned)((work + 255) / 256), 256, 0, c->stream>>>(c->rows, c->N, c->species, n.Emb, c->xs0,
                                                                                  c->nfeat, c->Efeat, c->XE);
         c->launches++;
