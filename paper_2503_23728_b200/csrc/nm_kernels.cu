@@ -55,11 +55,24 @@ __device__ __forceinline__ double normal_component(unsigned long long seed, uint
 __device__ __forceinline__ void xform(const double *__restrict__ M, const double *in, double *out, int P, int TC)
 {
     const int c = threadIdx.x;
-    for (int k = threadIdx.y; k < P; k += NM_TY) {
-        const double *m = M + (size_t)k * P;
-        double s = 0.0;
-        for (int j = 0; j < P; ++j) s += __ldg(m + j) * in[j * TC + c];
-        out[k * TC + c] = s;
+    // four output rows per pass: four independent accumulation chains (each in the same order j = 0 .. P-1 as a single row
+    // would be, so the result is bit-identical), and one shared-memory read of in[j] serves all four
+    for (int k0 = threadIdx.y; k0 < P; k0 += 4 * NM_TY) {
+        const int k1 = k0 + NM_TY, k2 = k0 + 2 * NM_TY, k3 = k0 + 3 * NM_TY;
+        const double *m0 = M + (size_t)k0 * P, *m1 = M + (size_t)(k1 < P ? k1 : k0) * P, *m2 = M + (size_t)(k2 < P ? k2 : k0) * P,
+                     *m3 = M + (size_t)(k3 < P ? k3 : k0) * P;
+        double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+        for (int j = 0; j < P; ++j) {
+            const double x = in[j * TC + c];
+            s0 += __ldg(m0 + j) * x;
+            s1 += __ldg(m1 + j) * x;
+            s2 += __ldg(m2 + j) * x;
+            s3 += __ldg(m3 + j) * x;
+        }
+        out[k0 * TC + c] = s0;
+        if (k1 < P) out[k1 * TC + c] = s1;
+        if (k2 < P) out[k2 * TC + c] = s2;
+        if (k3 < P) out[k3 * TC + c] = s3;
     }
 }
 
