@@ -392,17 +392,15 @@ __global__ void __launch_bounds__(256) fill_bitmask_kernel(NlArgs a, int nw)
         const int v = __shfl_up_sync(0xffffffffu, inc, o);
         if (lane >= o) inc += v;
     }
-    int64_t pos = base + (inc - cnt);
+    int *colp = a.d.col + base + (inc - cnt);
     for (int t = w0; t < w1; ++t) {
         unsigned bits = mk[t];
         while (bits) {
-            const int b = __ffs(bits) - 1;
-            a.d.col[pos] = t * 32 + b;
-            a.d.pair_row[pos] = (int)row;
-            ++pos;
+            *colp++ = t * 32 + (__ffs(bits) - 1);
             bits &= bits - 1;
         }
     }
+    for (int e = lane; e < n; e += 32) a.d.pair_row[base + e] = (int)row;   // coalesced, outside the divergent loop
 }
 
 }  // namespace
