@@ -320,14 +320,19 @@ __device__ __forceinline__ void msg_flush(const PairArgs &a, const MsgState &st,
 }
 
 // b + E_i of the row that starts: prefetched at the previous boundary (CSR rows are consecutive), else loaded now
+template <bool FIRST>
 __device__ __forceinline__ void msg_row_bias(const uint32_t *__restrict__ XE, MsgState &st, int64_t rows, float b2c, int c)
 {
+    if (FIRST) { st.be = b2c; return; }
     const uint32_t raw = (st.cur == st.nx_row) ? st.nx_val : __ldg(XE + (size_t)st.cur * H + c);
     st.be = b2c + tc::bf16hi_to_f32(raw);
     st.nx_row = (st.cur + 1 < rows) ? st.cur + 1 : st.cur;
     st.nx_val = __ldg(XE + (size_t)st.nx_row * H + c);
 }
 
+// FIRST: the first message pass of an evaluation is layer 0, where E = 0 for every atom (a4): e_ij = e0_ij + b, so the E_j unpack
+// and add, and the E_i loads, are left out (adding the zeros would give the same bits).
+template <bool FIRST>
 __device__ __forceinline__ void role_E_msg(const PairArgs &a, unsigned char *S, uint64_t *bar, uint32_t tmem, int n_my, int c,
                                            int qt, int lane, bool poller)
 {
@@ -361,7 +366,7 @@ __device__ __forceinline__ void role_E_msg(const PairArgs &a, unsigned char *S, 
                 const int rk = M.rowk[qt * 32];
                 st.cur = (rk < 0) ? -1 : (rk & 0x1FFFFFFF);
                 st.kind = (rk < 0) ? 0 : (rk >> 29);
-                if (st.cur >= 0) msg_row_bias(XE, st, a.rows, b2c, c);
+                if (st.cur >= 0) msg_row_bias<FIRST>(XE, st, a.rows, b2c, c);
             }
             float v[16];
             tc::tmem_ld16(td2 + q0, v);
@@ -380,7 +385,7 @@ __device__ __forceinline__ void role_E_msg(const PairArgs &a, unsigned char *S, 
                 for (int k = 0; k < 4; ++k) {
                     const uint32_t xe = xr[(e4 * 4 + k) * H];
                     wx[e4 * 4 + k] = wv[k] * tc::bf16lo_to_f32(xe);       // c_ij x_j
-                    v[e4 * 4 + k] += tc::bf16hi_to_f32(xe);               // e0 + E_j
+                    if (!FIRST) v[e4 * 4 + k] += tc::bf16hi_to_f32(xe);   // e0 + E_j
                 }
             }
             unsigned mask = M.fmask[qt * 2 + cc];
@@ -403,7 +408,7 @@ __device__ __forceinline__ void role_E_msg(const PairArgs &a, unsigned char *S, 
                 st.cur = (rk < 0) ? -1 : (rk & 0x1FFFFFFF);
                 st.kind = (rk < 0) ? 0 : (rk >> 29);
                 st.s1 = t1; st.s2 = t2;
-                if (st.cur >= 0) msg_row_bias(XE, st, a.rows, b2c, c);
+                if (st.cur >= 0) msg_row_bias<FIRST>(XE, st, a.rows, b2c, c);
             } else {
                 int lo = 0;
 #pragma unroll 1
@@ -420,7 +425,7 @@ __device__ __forceinline__ void role_E_msg(const PairArgs &a, unsigned char *S, 
                     st.cur = (rk < 0) ? -1 : (rk & 0x1FFFFFFF);
                     st.kind = (rk < 0) ? 0 : (rk >> 29);
                     st.s1 = 0.f; st.s2 = 0.f;
-                    if (st.cur >= 0) msg_row_bias(XE, st, a.rows, b2c, c);
+                    if (st.cur >= 0) msg_row_bias<FIRST>(XE, st, a.rows, b2c, c);
                 }
             }
             if (it + 1 < n_my) tc::named_bar_arrive(NB_SLOT + slot, 160);   // slot consumed: its refill overlaps the other chunk
@@ -943,7 +948,7 @@ __global__ void __launch_bounds__(Warps<HEAD, MODE>::THREADS, 1) pair_pipe_kerne
         const bool poller = (we == 1) || (we == 6) || (we == 11) || (we == 12);   // one per quarter, spread over the sub-partitions
         if (HEAD && MODE == 1) role_E_head_tc(a, S, bar, tmem, n_my, c, qt, lane, poller);
         else if (HEAD) role_E_head(a, S, bar, tmem, n_my, c, qt, lane, tid - WL::E0 * 32, poller);
-        else role_E_msg(a, S, bar, tmem, n_my, c, qt, lane, poller);
+        else role_E_msg<MODE == 0>(a, S, bar, tmem, n_my, c, qt, lane, poller);
     } else if (HEAD && MODE == 1 && warp >= WL::F0 && warp < WL::F0 + 4) {
         role_F(a, S, bar, tmem, n_my, tid - WL::F0 * 32, lane);
     } else if (warp == WL::MMA) {
