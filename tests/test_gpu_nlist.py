@@ -90,3 +90,17 @@ def test_pair_capacity_overflow_is_reported(cuda_device):
     with pytest.raises(pb.PimdError) as e:
         gpu.nlist()
     assert e.value.code == -3
+
+
+def test_crowded_cells_bit_exact(cuda_device):
+    """More atoms in a cell than the count kernel stages in shared memory (128): the rest of the home atoms is read from
+    global memory and counted through global counters.  Two cells per axis, each 1.49 r_c wide, about 135 atoms per cell."""
+    rng = np.random.default_rng(77)
+    rc = 2.0
+    box = np.array([5.97, 5.9, 5.99])
+    x = rng.uniform(0, 1, (1, 1080, 3)) * box
+    sp = rng.integers(0, 3, x.shape[1]).astype(np.int32)
+    gpu, ref = make_pair(sp, x, box, 2, 300.0, 0.25, 1.0, 0, _net(rc))
+    spread_beads(gpu, ref, scale=0.05)
+    rp, _ = _compare(gpu, ref)
+    assert np.diff(rp).max() < 512 and np.diff(rp).mean() > 100
