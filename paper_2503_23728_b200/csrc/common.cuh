@@ -70,6 +70,8 @@ struct pimd_ctx {
     int forces_valid;
     int64_t launches;
     int num_sms;
+    int device;                        // CUDA device the workspace and stream belong to (set current at every entry point)
+    unsigned attr_done;                // per-context (= per-device) bits: opt-in shared-memory attribute set for a kernel family
 
     // workspace views
     double *q, *p, *F;                 // [rows][3]
@@ -86,8 +88,7 @@ struct pimd_ctx {
     uint16_t *wimg_wf2;                // bf16 UMMA image of w_f2 replicated on 16 rows (readout product of the head)
     uint16_t *wimg_e1, *wimg_e2, *wimg_fe;   // bf16 UMMA images (K-major, 128B swizzle) for the tcgen05 path
     int use_tc;                        // 1: tensor-core pair and node kernels (gemm_dtype 1, K=64, H=128)
-    int msg_rowgemm;                   // 1: later message passes as one GEMM per CSR row (experimental, env PIMD_MSG_ROWGEMM=1)
-    uint16_t *wimg_node;               // [L][5] bf16 UMMA images: W_vn/2, W_vm/2, W_v2, W_a, W_s^{l+1} (or W_f1)
+    uint16_t *wimg_node;               // [L][20] bf16 UMMA half-images (16 KB): (W_vn/2, W_vm/2, W_v2, W_a, W_s^{l+1} or W_f1) x (hi, lo) x 2 K blocks
     float *xs0;                        // [S][H] W_s^0 Emb[s]
     float h_be1_half[128];             // HOST copy of b_e1 / 2 (passed to the pair kernels as kernel parameters)
     unsigned char *h1_img, *meta_img;  // [pair_cap/128 + 1] tile images kept between the pair passes of one evaluation (tc path)
@@ -110,6 +111,7 @@ struct ProfScope {
     ProfScope(pimd_ctx *ctx, int kind) : c(ctx) { if (c->prof) pimd_prof_begin(c, kind); }
     ~ProfScope() { if (c->prof) pimd_prof_end(c); }
 };
+enum { ATTR_PAIR32 = 1, ATTR_NODE32 = 2, ATTR_PIPE = 4, ATTR_NODETC = 8, ATTR_NM = 256 /* << MODE */ };
 enum { PROF_NM = 0, PROF_NLIST = 1, PROF_PAIR = 2, PROF_NODE = 3, PROF_HEAD = 4, PROF_OTHER = 5 };
 
 void pimd_set_error(const char *fmt, ...);
@@ -129,7 +131,6 @@ int pimd_launch_nm_pre(pimd_ctx *c, uint32_t t);
 int pimd_launch_nm_post(pimd_ctx *c, uint32_t t);
 int pimd_launch_simple_forces(pimd_ctx *c);          // kinds 1, 2
 int pimd_launch_estimators(pimd_ctx *c);
-int pimd_launch_check_finite(pimd_ctx *c);
 int pimd_launch_nlist(pimd_ctx *c);
 int pimd_launch_gfn_forces(pimd_ctx *c);
 int pimd_launch_copy_forces_f32(pimd_ctx *c, float *d_out);

@@ -193,10 +193,9 @@ template <int H>
 int launch_node_t(pimd_ctx *c, const NodeArgs &a)
 {
     size_t smem = sizeof(NodeSmem<H>);
-    static bool attr = false;
-    if (!attr) {
+    if (!(c->attr_done & ATTR_NODE32)) {
         PIMD_CUDA_CHECK(cudaFuncSetAttribute(node_kernel<H>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr = true;
+        c->attr_done |= ATTR_NODE32;
     }
     unsigned grid = (unsigned)((c->rows + TP - 1) / TP);
     node_kernel<H><<<grid, NT, smem, c->stream>>>(a);

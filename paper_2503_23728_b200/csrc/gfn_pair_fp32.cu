@@ -222,11 +222,10 @@ template <int K, int H>
 int launch_pair_t(pimd_ctx *c, const PairArgs &a, bool head)
 {
     size_t smem = sizeof(PairSmem<K, H>);
-    static bool attr = false;
-    if (!attr) {
+    if (!(c->attr_done & ATTR_PAIR32)) {
         PIMD_CUDA_CHECK(cudaFuncSetAttribute(pair_kernel<K, H, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         PIMD_CUDA_CHECK(cudaFuncSetAttribute(pair_kernel<K, H, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr = true;
+        c->attr_done |= ATTR_PAIR32;
     }
     if (head) pair_kernel<K, H, true><<<c->num_sms, NT, smem, c->stream>>>(a);
     else pair_kernel<K, H, false><<<c->num_sms, NT, smem, c->stream>>>(a);

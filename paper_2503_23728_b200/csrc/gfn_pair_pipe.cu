@@ -105,7 +105,6 @@ struct PairArgs {
     const void *gsrc;                     // message: XE packed bf16 (x | E << 16) [rows][128] u32; head: G fp32 [rows][128]
     const float *wf2; float bf2;
     float *m_out, *carry_m, *Fraw, *carry_f;
-    const float *W2T, *Emaster;           // row-GEMM message pass: W_e2^T fp32 [k][c]; E fp32 in the node kernel's blocked layout
     unsigned char *h1_img, *meta_img;     // per tile: A2 operand image (32 KB) and Meta, written by the first pass of a force
                                           // evaluation and re-read by the later ones (same pairs, same h1)
 };
@@ -689,10 +688,13 @@ __device__ __forceinline__ void role_E_head_tc(const PairArgs &a, unsigned char 
             {
                 unsigned char *row = A3 + (q0 >> 6) * 16384;
                 const int ch0 = (q0 & 63) >> 3;
+                // fp16, not bf16: the readout sums 128 signed terms w_f2[c] act[c] that cancel, and the emulation
+                // (tests/test_bf16_emulation.py) shows a bf16 operand here alone costs 0.4-0.5 % rms of |F|; SiLU output is far inside
+                // the fp16 range (a value beyond it saturates to inf and trips the non-finite force check)
                 *(uint4 *)(row + ((ch0 ^ (c & 7)) << 4)) =
-                    make_uint4(tc::pack_bf16(v[0], v[1]), tc::pack_bf16(v[2], v[3]), tc::pack_bf16(v[4], v[5]), tc::pack_bf16(v[6], v[7]));
+                    make_uint4(tc::pack_f16(v[0], v[1]), tc::pack_f16(v[2], v[3]), tc::pack_f16(v[4], v[5]), tc::pack_f16(v[6], v[7]));
                 *(uint4 *)(row + (((ch0 + 1) ^ (c & 7)) << 4)) =
-                    make_uint4(tc::pack_bf16(v[8], v[9]), tc::pack_bf16(v[10], v[11]), tc::pack_bf16(v[12], v[13]), tc::pack_bf16(v[14], v[15]));
+                    make_uint4(tc::pack_f16(v[8], v[9]), tc::pack_f16(v[10], v[11]), tc::pack_f16(v[12], v[13]), tc::pack_f16(v[14], v[15]));
             }
         }
         tc::fence_proxy_async_smem();
@@ -754,7 +756,7 @@ __device__ __forceinline__ void role_MMA(const PairArgs &a, unsigned char *S, ui
     STATS_BEGIN
     constexpr bool TCH = HEAD && MODE == 1;      // head with the channel reduction on the tensor core
     constexpr int NA2 = TCH ? 1 : 2;             // A2 stages (the second stage's space is an A3 stage there)
-    const uint32_t idesc = tc::make_idesc_bf16(TP, H), idesc16 = tc::make_idesc_bf16(TP, 16);
+    const uint32_t idesc = tc::make_idesc_bf16(TP, H), idesc16 = tc::make_idesc_f16(TP, 16);   // readout product: fp16 operands
     const uint32_t sW1 = tc::smem_u32(S + OFF_W1), sW2 = tc::smem_u32(S + OFF_W2);
     const uint32_t sA1 = tc::smem_u32(S + OFF_A1), sA2 = tc::smem_u32(S + OFF_A2);
     tc::mbar_wait(&bar[W_FULL], 0);
@@ -814,7 +816,6 @@ __device__ __forceinline__ void role_MMA(const PairArgs &a, unsigned char *S, ui
 // ---- role G: gathered rows (512 B each) -> ring slots by TMA bulk copies.  Warp g feeds the two 16-pair slots of
 // quarter tile g, one copy per lane (the copy instruction issues from the uniform datapath, one lane at a time).  A slot
 // is refilled as soon as the E warps release it, i.e. while they work on the quarter's other slot.
-template <int SLOT_THREADS>   // threads on the slot-consumed barrier: the consumers + this warp
 __device__ __forceinline__ void role_G(const PairArgs &a, unsigned char *S, uint64_t *bar, int n_my, int qt, int lane)
 {
     STATS_BEGIN
@@ -828,8 +829,7 @@ __device__ __forceinline__ void role_G(const PairArgs &a, unsigned char *S, uint
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
             if (it > 0) {                                    // the consumers have read the slot
-                if (SLOT_THREADS > 0) WAITED(tc::named_bar_sync(NB_SLOT + qt * 2 + h, SLOT_THREADS));
-                else WAITED(tc::mbar_wait(&bar[qt * 2 + h], (it & 1) ^ 1));       // (row-GEMM kernel: mbarriers 0-7, one arrival per tile)
+                WAITED(tc::named_bar_sync(NB_SLOT + qt * 2 + h, 160));   // the 128 consumers + this warp
             }
             if (lane == 16 * h) tc::mbar_arrive_expect_tx(&bar[XE_FULL + qt * 2 + h], 8192);
             __syncwarp();
@@ -954,7 +954,7 @@ __global__ void __launch_bounds__(Warps<HEAD, MODE>::THREADS, 1) pair_pipe_kerne
     } else if (warp == WL::MMA) {
         role_MMA<HEAD, MODE>(a, S, bar, tmem, n_my, lane);
     } else if (warp >= WL::G0 && warp < WL::G0 + 4) {
-        role_G<160>(a, S, bar, n_my, warp - WL::G0, lane);
+        role_G(a, S, bar, n_my, warp - WL::G0, lane);
     } else if (warp == WL::SL) {
         if (MODE == 0) role_S(a, S, bar, n_my, lane);
         else role_L<(HEAD ? 1 : 2)>(a, S, bar, n_my, lane);
@@ -964,327 +964,6 @@ __global__ void __launch_bounds__(Warps<HEAD, MODE>::THREADS, 1) pair_pipe_kerne
     if (warp == WL::MMA) tc::tmem_dealloc(tmem, 512);
 }
 
-// =====================================================================================================================
-// Message pass of the LATER layers as one GEMM per CSR row (S:G3, G5), all on the tensor core:
-//   m_i[c] = agg_norm ( sum_k W_e2[c][k] T_i[c][k]  +  (b[c] + E_i[c]) s_i[c]  +  t_i[c] ),
-//   T_i[c][k] = sum_j (c_ij x_j[c]) h1_ij[k],   s_i[c] = sum_j c_ij x_j[c],   t_i[c] = sum_j c_ij (E_j x_j)[c]
-// i.e. e0 = W_e2 h1 is never formed per pair: the contraction over the PAIRS of a row runs first (operands with the pair
-// index as the contraction dimension: "MN-major" UMMA operands, for which the h1 operand image of the first pass is
-// already in the right shared-memory form), and W_e2 is applied once per row by the epilogue (fp32, one register per k).
-// s and t are products of the same A operands with a block of ones.  The node kernel delivers x and y = E (.) x as two
-// bf16 rows per atom.  Roles (one persistent CTA per SM, 128-pair tiles, 16-pair K blocks):
-//   LT, LM 2 warps : TMA bulk copies of the tile's h1 image (B operand, 32 KB, two stages) and of the meta records (four ahead)
-//   G   4 warps  : TMA tile::gather4 copies of the gathered rows (x_j | y_j, 512 B per pair) into an 8-slot staging ring
-//   R   8 warps  : warp kb owns K block kb of every tile: staging -> A block (scale by c_ij as bf16x2, 128-byte swizzle, zero the
-//                  pairs outside the row segment; a block that straddles row boundaries is written once per segment), then it
-//                  ISSUES the block's products T += x'^T h1, s += x'^T 1, t += y'^T 1 into one of three TMEM accumulators
-//                  (160 columns).  The eight warps issue in block order through a token chain of named barriers, so the
-//                  accumulation order is fixed.  A row segment ends at a row boundary or at the end of the tile.
-//   E   4 warps  : thread = channel = TMEM lane: the 128 columns of T against W_e2[c][:] held in registers, + s, t terms;
-//                  direct store or carry slot (granule = tile).
-// Experimental (PIMD_MSG_ROWGEMM=1): correct and reproducible, slower than the default pipeline; DESIGN.md section 11 says why.
-namespace mg {
-constexpr int NA = 8;                        // A-block slots of 8 KB, one per K block of a tile: x' (2 x 2 KB halves) | y' (2 x 2 KB halves)
-constexpr int NACC = 3;                      // TMEM accumulators of 160 columns: T 0-127, s 128-143, t 144-159
-constexpr int ACC_COLS = 160;
-constexpr int OFF_AB = 0;                    // (the weight and A1 regions of the first-pass carve are free here)
-constexpr int OFF_ONES = OFF_AB + NA * 8192; // 2 KB of bf16 1.0
-constexpr int OFF_INFO = OFF_ONES + 2048;    // NACC x {row, granule}
-static_assert(OFF_INFO + NACC * 8 <= OFF_A2, "row-GEMM carve overlaps the h1 tiles");
-enum { SLOT_EMPTY = 0 /* 8 */, ACC_FULL = 12 /* 3 */, AB_EMPTY = 32 /* 8 */, ACC_EMPTY = 40 /* 3 */ };
-enum { NB_EP = 2, NB_TOKEN = 8 /* + block: 8-15 (bar.sync blocks in hardware and wakes up at once; an mbarrier wait does not) */ };
-// warps: E 0-3, R 4-11, G 12-15, LT (h1 tiles) 16, LM (meta records) 17, idle 18-19 (whole warpgroups for setmaxnreg)
-constexpr int W_E = 0, W_R = 4, W_G = 12, W_LT = 16, W_LM = 17, THREADS = 640;
-
-__device__ __forceinline__ int row_of(int rk) { return rk < 0 ? -1 : (rk & 0x1FFFFFFF); }
-
-__device__ __forceinline__ uint64_t desc_mn(uint32_t addr, uint32_t lbo, uint32_t sbo)
-{
-    // MN-major, 128-byte swizzle: LBO = bytes between 64-element atoms along M/N, SBO = bytes between 8-row groups along K
-    return (uint64_t)((addr >> 4) & 0x3FFF) | ((uint64_t)((lbo >> 4) & 0x3FFF) << 16) | ((uint64_t)((sbo >> 4) & 0x3FFF) << 32) |
-           ((uint64_t)1 << 46) | ((uint64_t)2 << 61);
-}
-
-__device__ __forceinline__ uint32_t scale_bf16x2(uint32_t v, __nv_bfloat162 w)
-{
-    __nv_bfloat162 t = __hmul2(*reinterpret_cast<__nv_bfloat162 *>(&v), w);
-    return *reinterpret_cast<uint32_t *>(&t);
-}
-
-// start flags of the 128 pairs of a tile (bit = pair starts a row segment; pair 0 always does): whole warp
-__device__ __forceinline__ void tile_starts(const Meta &M, int lane, unsigned (&st)[4])
-{
-#pragma unroll
-    for (int q = 0; q < 4; ++q) {
-        const int p = q * 32 + lane;
-        const int r = row_of(M.rowk[p]);
-        const int rp = (p == 0) ? -3 : row_of(M.rowk[p - 1]);
-        st[q] = __ballot_sync(FULL, r != rp);
-    }
-}
-__device__ __forceinline__ unsigned block_bits(const uint32_t (&st)[4], int kb)
-{
-    const int q = kb >> 1;
-    const unsigned w = (q == 0) ? st[0] : (q == 1) ? st[1] : (q == 2) ? st[2] : st[3];      // (no dynamic indexing: registers)
-    return (w >> ((kb & 1) * 16)) & 0xFFFFu;
-}
-
-// number of start flags at pairs 0 .. pos of the tile
-__device__ __forceinline__ int starts_upto(const uint32_t (&st)[4], int pos)
-{
-    const int q = pos >> 5;
-    const uint32_t m = (2u << (pos & 31)) - 1u;              // bits 0 .. pos & 31  (pos & 31 == 31: 2u << 31 wraps to 0, m = all ones)
-    int n = 0;
-#pragma unroll
-    for (int i = 0; i < 4; ++i) n += (i < q) ? __popc(st[i]) : (i == q) ? __popc(st[i] & m) : 0;
-    return n;
-}
-
-// ---- role R: warp kb owns K block kb of every tile: it restages the block (A operand slot kb) AND issues the block's
-// products.  The eight warps issue in block order through a token chain (mbarrier TOKEN[kb], passed on after the issue),
-// so the accumulation order within a row is fixed (bitwise reproducible) although eight threads issue; everything else
-// (restaging, waits for the gathered rows) runs in parallel.  The warp that issues the last product of a row segment
-// closes it (commit -> ACC_FULL: the products of a segment form one accumulation chain, so the last completes last).
-// lane = (pair r_lo of a group of four, 16-byte chunk j of each of the four 128-byte row segments x lo, x hi, y lo, y hi)
-__device__ __forceinline__ void role_R(const PairArgs &a, unsigned char *S, uint64_t *bar, uint32_t tmem, int n_my, int kb, int lane)
-{
-    STATS_BEGIN
-    const int r_lo = lane >> 3, j = lane & 7;
-    const uint32_t idesc_T = tc::make_idesc_bf16(128, 128) | (1u << 15) | (1u << 16);   // A and B MN-major
-    const uint32_t idesc_1 = tc::make_idesc_bf16(128, 16) | (1u << 15) | (1u << 16);
-    const uint64_t ones = desc_mn(tc::smem_u32(S + OFF_ONES), 1024, 1024);
-    const uint64_t ax = desc_mn(tc::smem_u32(S + OFF_AB + kb * 8192), 2048, 1024), ay = ax + 256;
-    int2 *info = (int2 *)(S + OFF_INFO);
-    int use = 0;                                             // A blocks this warp has produced (all in slot kb)
-    int nseg_base = 0;                                       // row segments (with output) of the earlier tiles
-    for (int it = 0; it < n_my; ++it) {
-        const int s = it & 1;
-        const Meta &M = meta_of(S, it);
-        const int gran = (int)((int64_t)blockIdx.x + (int64_t)it * gridDim.x);      // granule = tile
-        WAITED(tc::mbar_wait(&bar[META_FULL + (it & (NM - 1))], (it / NM) & 1));
-        uint32_t st[4];
-        tile_starts(M, lane, st);
-        const uint32_t starts = block_bits(st, kb);
-        const bool next_starts = (kb == 7) || (block_bits(st, (kb + 1) & 7) & 1u);
-        uint32_t bnd = starts & ~1u;                         // row boundaries INSIDE the block
-        const int nseg_tile = __popc(st[0]) + __popc(st[1]) + __popc(st[2]) + __popc(st[3]) - (M.rowk[TP - 1] < 0 ? 1 : 0);
-        float wv[4];
-#pragma unroll
-        for (int rr = 0; rr < 4; ++rr) wv[rr] = M.w[kb * 16 + rr * 4 + r_lo];
-        WAITEDK(1, tc::mbar_wait(&bar[XE_FULL + kb], it & 1));           // gathered rows of this block have landed
-        const unsigned char *src = S + OFF_RING + kb * 8192 + r_lo * 512 + j * 16;
-        const uint64_t bdesc = desc_mn(tc::smem_u32(S + OFF_A2 + s * 32768 + kb * 2048), 16384, 1024);
-        int lo = 0;
-        bool have_token = false;
-#pragma unroll 1
-        while (true) {                                       // one A block per row segment that the block touches
-            const int hi = bnd ? (__ffs(bnd) - 1) : 16;
-            WAITEDK(2, tc::mbar_wait_spin(&bar[AB_EMPTY + kb], (use & 1) ^ 1));    // own products of the last A block have read the slot
-            ++use;
-            unsigned char *dst = S + OFF_AB + kb * 8192;
-#pragma unroll
-            for (int rr = 0; rr < 4; ++rr) {
-                const int r = rr * 4 + r_lo;
-                const __nv_bfloat162 w2 = __float2bfloat162_rn((r >= lo && r < hi) ? wv[rr] : 0.f);   // pairs of other rows: zero
-                unsigned char *d = dst + (r >> 3) * 1024 + (r & 7) * 128 + ((j ^ (r & 7)) << 4);
-#pragma unroll
-                for (int i = 0; i < 4; ++i) {
-                    uint4 v = *(const uint4 *)(src + rr * 2048 + i * 128);
-                    v.x = scale_bf16x2(v.x, w2); v.y = scale_bf16x2(v.y, w2);
-                    v.z = scale_bf16x2(v.z, w2); v.w = scale_bf16x2(v.w, w2);
-                    *(uint4 *)(d + i * 2048) = v;
-                }
-            }
-            tc::fence_proxy_async_smem();
-            __syncwarp();
-            if (!have_token) {
-                WAITED(tc::mbar_wait_spin(&bar[A2_FULL + s], (it >> 1) & 1));     // h1 rows of the tile
-                // token: every product of the earlier blocks (and tiles) has been issued
-                if (kb > 0 || it > 0) tc::named_bar_sync(NB_TOKEN + kb, 64);
-                have_token = true;
-            }
-            const int row = row_of(M.rowk[kb * 16 + lo]);
-            const bool seg_start = (lo > 0) || (starts & 1u);
-            const int seg = nseg_base + starts_upto(st, kb * 16 + lo) - 1;
-            const int acc = seg % NACC;
-            if (row >= 0 && seg_start) WAITED(tc::mbar_wait_spin(&bar[ACC_EMPTY + acc], ((seg / NACC) & 1) ^ 1));
-            tc::tc_fence_after_sync();
-            const bool closes = (row >= 0) && (bnd != 0u || next_starts);
-            if (lane == 0) {
-                if (row >= 0) {
-                    const uint32_t d = tmem + acc * ACC_COLS;
-                    const uint32_t accum = seg_start ? 0u : 1u;
-                    tc::mma_bf16_ss(d, ax, bdesc, idesc_T, accum);
-                    tc::mma_bf16_ss(d + 128, ax, ones, idesc_1, accum);
-                    tc::mma_bf16_ss(d + 144, ay, ones, idesc_1, accum);
-                }
-                tc::mma_commit(&bar[AB_EMPTY + kb]);
-                if (closes) {
-                    info[acc] = make_int2(row, gran);
-                    tc::mma_commit(&bar[ACC_FULL + acc]);    // the segment's accumulation chains end with these products
-                    tc::mbar_arrive(&bar[ACC_FULL + acc]);   // releases the info record
-                }
-            }
-            __syncwarp();
-            if (!bnd) break;
-            bnd &= bnd - 1;
-            lo = hi;
-        }
-        if (kb < 7 || it + 1 < n_my) tc::named_bar_arrive(NB_TOKEN + ((kb + 1) & 7), 64);   // next block (or block 0 of the next tile) may issue
-        if (lane == 0) {
-            tc::mma_commit(&bar[A2_EMPTY + s]);              // h1 tile free once the products of all eight blocks have completed
-            tc::mbar_arrive(&bar[META_EMPTY + (it & (NM - 1))]);
-            tc::mbar_arrive(&bar[SLOT_EMPTY + kb]);          // staging slot consumed
-        }
-        __syncwarp();
-        nseg_base += nseg_tile;
-    }
-    if (kb == 7) {                                           // end marker for role E (this warp issues last)
-        const int acc = nseg_base % NACC;
-        WAITED(tc::mbar_wait(&bar[ACC_EMPTY + acc], ((nseg_base / NACC) & 1) ^ 1));
-        if (lane == 0) {
-            info[acc] = make_int2(-2, 0);
-            tc::mbar_arrive(&bar[ACC_FULL + acc]);
-            tc::mbar_arrive(&bar[ACC_FULL + acc]);
-        }
-        __syncwarp();
-    }
-    STATS_END("R")
-}
-
-// ---- role LT: the h1 image of the first pass, tile by tile (B operand, two stages)
-__device__ __forceinline__ void role_LT(const PairArgs &a, unsigned char *S, uint64_t *bar, int n_my, int lane)
-{
-    for (int it = 0; it < n_my; ++it) {
-        const int s = it & 1;
-        const int64_t tile = (int64_t)blockIdx.x + (int64_t)it * gridDim.x;
-        tc::mbar_wait(&bar[A2_EMPTY + s], ((it >> 1) & 1) ^ 1);
-        if (lane == 0) {
-            tc::mbar_arrive_expect_tx(&bar[A2_FULL + s], 32768);
-            tc::bulk_g2s(S + OFF_A2 + s * 32768, a.h1_img + tile * 32768, 32768, &bar[A2_FULL + s]);
-        }
-        __syncwarp();
-    }
-}
-// ---- role LM: meta records, up to NM tiles ahead (the gathers and the restaging start from them)
-__device__ __forceinline__ void role_LM(const PairArgs &a, unsigned char *S, uint64_t *bar, int n_my, int lane)
-{
-    for (int it = 0; it < n_my; ++it) {
-        const int m = it & (NM - 1);
-        const int64_t tile = (int64_t)blockIdx.x + (int64_t)it * gridDim.x;
-        tc::mbar_wait(&bar[META_EMPTY + m], ((it / NM) & 1) ^ 1);
-        if (lane == 0) {
-            tc::mbar_arrive_expect_tx(&bar[META_FULL + m], (uint32_t)sizeof(Meta));
-            tc::bulk_g2s(&meta_of(S, it), a.meta_img + tile * (int64_t)sizeof(Meta), (uint32_t)sizeof(Meta), &bar[META_FULL + m]);
-        }
-        __syncwarp();
-    }
-}
-
-// ---- role E: thread = channel c = TMEM lane c
-__device__ __forceinline__ void role_E(const PairArgs &a, unsigned char *S, uint64_t *bar, uint32_t tmem, int c, int lane)
-{
-    STATS_BEGIN
-    const bool poller = (c >> 5) == 2;
-    float w2[H];
-#pragma unroll
-    for (int k = 0; k < H; ++k) w2[k] = __ldg(a.W2T + (size_t)k * H + c);
-    const float b2c = ((const float *)(S + OFF_BIAS))[H + c];
-    const uint32_t lane_field = (uint32_t)(c & ~31) << 16;
-    const int2 *info = (const int2 *)(S + OFF_INFO);
-    for (int n = 0;; ++n) {
-        const int acc = n % NACC;
-        if (poller) WAITED(tc::mbar_wait_spin(&bar[ACC_FULL + acc], (n / NACC) & 1));
-        WAITED(tc::named_bar_sync(NB_EP, 128));
-        tc::tc_fence_after_sync();
-        const int2 inf = info[acc];
-        const int row = inf.x;
-        if (row == -2) break;
-        // E_i (fp32 master, blocked [tile][c/4][row][4]) and the extent of the row: in flight during the contraction
-        const float Ei = __ldg(a.Emaster + ((size_t)(row >> 7) * (H / 4) + (c >> 2)) * 512 + (size_t)(row & 127) * 4 + (c & 3));
-        const int rs = __ldg(a.row_ptr + row), re = __ldg(a.row_ptr + row + 1);
-        const uint32_t td = tmem + acc * ACC_COLS + lane_field;
-        float t0 = 0.f, t1 = 0.f, t2 = 0.f, t3 = 0.f;
-#pragma unroll
-        for (int c2 = 0; c2 < 4; ++c2) {
-            uint32_t r0[16], r1[16];
-            tc::tmem_ld16_nowait(td + c2 * 32, r0);
-            tc::tmem_ld16_nowait(td + c2 * 32 + 16, r1);
-            tc::tmem_ld_wait();
-#pragma unroll
-            for (int e = 0; e < 16; e += 4) {
-                t0 = fmaf(w2[c2 * 32 + e], __uint_as_float(r0[e]), t0);
-                t1 = fmaf(w2[c2 * 32 + e + 1], __uint_as_float(r0[e + 1]), t1);
-                t2 = fmaf(w2[c2 * 32 + e + 2], __uint_as_float(r0[e + 2]), t2);
-                t3 = fmaf(w2[c2 * 32 + e + 3], __uint_as_float(r0[e + 3]), t3);
-            }
-#pragma unroll
-            for (int e = 0; e < 16; e += 4) {
-                t0 = fmaf(w2[c2 * 32 + 16 + e], __uint_as_float(r1[e]), t0);
-                t1 = fmaf(w2[c2 * 32 + 16 + e + 1], __uint_as_float(r1[e + 1]), t1);
-                t2 = fmaf(w2[c2 * 32 + 16 + e + 2], __uint_as_float(r1[e + 2]), t2);
-                t3 = fmaf(w2[c2 * 32 + 16 + e + 3], __uint_as_float(r1[e + 3]), t3);
-            }
-        }
-        const float sx = tc::tmem_ld1(td + 128), sy = tc::tmem_ld1(td + 144);
-        tc::tc_fence_before_sync();
-        __syncwarp();
-        if (lane == 0) tc::mbar_arrive(&bar[ACC_EMPTY + acc]);       // accumulator drained
-        const float mval = a.wscale * (((t0 + t1) + (t2 + t3)) + fmaf(b2c + Ei, sx, sy));
-        const int64_t g0 = (int64_t)inf.y * TP;
-        float *dst = (rs >= g0 && re <= g0 + TP) ? a.m_out + (size_t)row * H + c
-                                                 : a.carry_m + ((size_t)inf.y * 2 + (rs < g0 ? 0 : 1)) * H + c;
-        *dst = mval;
-    }
-    STATS_END("Eg")
-}
-
-__global__ void __launch_bounds__(THREADS, 1) msg_rowgemm_kernel(const __grid_constant__ PairArgs a)
-{
-    extern __shared__ __align__(1024) unsigned char smem_raw[];
-    unsigned char *S = smem_raw + ((1024u - (tc::smem_u32(smem_raw) & 1023u)) & 1023u);
-    uint64_t *bar = (uint64_t *)(S + OFF_BAR);
-    uint32_t *tmem_slot = (uint32_t *)(S + OFF_TMEM);
-    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int64_t n_pairs = a.row_ptr[a.rows];
-    const int n_my = n_my_tiles(n_pairs);
-    if (tid == 0) {
-        for (int s = 0; s < NA; ++s) { tc::mbar_init(&bar[SLOT_EMPTY + s], 1); tc::mbar_init(&bar[AB_EMPTY + s], 1); }
-        for (int s = 0; s < NACC; ++s) { tc::mbar_init(&bar[ACC_FULL + s], 2); tc::mbar_init(&bar[ACC_EMPTY + s], 4); }
-        for (int s = 0; s < 2; ++s) { tc::mbar_init(&bar[A2_FULL + s], 1); tc::mbar_init(&bar[A2_EMPTY + s], 8); }
-        for (int s = 0; s < 2 * NSLOT; ++s) tc::mbar_init(&bar[XE_FULL + s], 1);
-        for (int s = 0; s < NM; ++s) { tc::mbar_init(&bar[META_FULL + s], 1); tc::mbar_init(&bar[META_EMPTY + s], 8); }
-        tc::fence_mbar_init();
-    }
-    if (warp == W_LT) tc::tmem_alloc(tmem_slot, 512);
-    for (int i = tid; i < 1024; i += THREADS) ((uint16_t *)(S + OFF_ONES))[i] = 0x3F80;     // bf16 1.0
-    for (int i = tid; i < H; i += THREADS) ((float *)(S + OFF_BIAS))[H + i] = a.b2[i];
-    tc::fence_proxy_async_smem();
-    tc::tc_fence_before_sync();
-    __syncthreads();
-    tc::tc_fence_after_sync();
-    const uint32_t tmem = *tmem_slot;
-    // register re-balancing between warpgroups: the epilogue keeps a row of W_e2 in registers
-    if (warp < 4) asm volatile("setmaxnreg.inc.sync.aligned.u32 208;");
-    else if (warp < 12) asm volatile("setmaxnreg.dec.sync.aligned.u32 72;");
-    else if (warp < 16) asm volatile("setmaxnreg.dec.sync.aligned.u32 48;");
-    else asm volatile("setmaxnreg.dec.sync.aligned.u32 64;");   // (registers released: 6144 + 6144 + 4096 >= 14336 taken by E; the pool is the CTA's own)
-    if (warp < W_R) {
-        role_E(a, S, bar, tmem, tid, lane);
-    } else if (warp < W_G) {
-        role_R(a, S, bar, tmem, n_my, warp - W_R, lane);
-    } else if (warp < W_LT) {
-        gfn_pipe::role_G<0>(a, S, bar, n_my, warp - W_G, lane);
-    } else if (warp == W_LT) {
-        role_LT(a, S, bar, n_my, lane);
-    } else if (warp == W_LM) {
-        role_LM(a, S, bar, n_my, lane);
-    }
-    tc::tc_fence_before_sync();
-    __syncthreads();
-    if (warp == W_LT) tc::tmem_dealloc(tmem, 512);
-}
-}  // namespace mg
 
 int launch_pair_pipe(pimd_ctx *c, bool head, bool first)
 {
@@ -1301,23 +980,19 @@ int launch_pair_pipe(pimd_ctx *c, bool head, bool first)
     a.m_out = c->mfeat; a.carry_m = c->carry_m; a.Fraw = c->Fraw; a.carry_f = c->carry_f;
     a.h1_img = c->h1_img; a.meta_img = c->meta_img;
     a.gmap = head ? c->tmap_g : c->tmap_xe;
-    a.W2T = c->net.We2T; a.Emaster = c->Efeat;
     const size_t smem = SMEM_BYTES + 1024;
-    static bool attr = false;
-    if (!attr) {
+    if (!(c->attr_done & ATTR_PIPE)) {
         PIMD_CUDA_CHECK(cudaFuncSetAttribute(pair_pipe_kernel<false, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         PIMD_CUDA_CHECK(cudaFuncSetAttribute(pair_pipe_kernel<false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         PIMD_CUDA_CHECK(cudaFuncSetAttribute(pair_pipe_kernel<true, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         PIMD_CUDA_CHECK(cudaFuncSetAttribute(pair_pipe_kernel<true, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        PIMD_CUDA_CHECK(cudaFuncSetAttribute(mg::msg_rowgemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr = true;
+        c->attr_done |= ATTR_PIPE;
     }
     if (head) {
         if (first) pair_pipe_kernel<true, 0><<<c->num_sms, Warps<true, 0>::THREADS, smem, c->stream>>>(a);
         else pair_pipe_kernel<true, 1><<<c->num_sms, Warps<true, 1>::THREADS, smem, c->stream>>>(a);
     } else {
         if (first) pair_pipe_kernel<false, 0><<<c->num_sms, Warps<false, 0>::THREADS, smem, c->stream>>>(a);
-        else if (c->msg_rowgemm) mg::msg_rowgemm_kernel<<<c->num_sms, mg::THREADS, smem, c->stream>>>(a);
         else pair_pipe_kernel<false, 1><<<c->num_sms, Warps<false, 1>::THREADS, smem, c->stream>>>(a);
     }
     c->launches++;

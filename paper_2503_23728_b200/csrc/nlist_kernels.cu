@@ -1,12 +1,12 @@
 // nlist_kernels.cu -- per-bead-system periodic cell list -> CSR pair list (rows a1-a3 of SURVEY 8(a)).
 //
-// bin (wrapped fraction -> cell) -> counting sort (histogram, per-system exclusive scan, scatter of
-// atom index + fp64 position into cell order) -> one CTA per cell stages its 3x3x3 stencil in shared memory, a warp per
-// home atom counts the hits and parks them in a fixed-stride scratch row -> row_ptr scan -> fill with an in-shared-memory rank sort
-// so that every CSR row lists j ascending.  The inclusion test is
-// the fp64 sequence of S:L3 written with explicit round-to-nearest intrinsics (no FMA contraction), so
-// the list is bit-identical to the oracle's.  Integer atomics only order the scatter inside a cell;
-// the sorted rows make the CSR deterministic.
+// bin (wrapped fraction -> cell) -> counting sort (histogram, per-system exclusive scan, scatter of atom index + fp64
+// position into cell order) -> one CTA per cell stages its de-duplicated 3x3x3 stencil in shared memory (fp32 coordinates
+// relative to the cell's first atom); a lane is a home atom, the four warps share the candidates; an fp32 estimate of d^2
+// settles every candidate outside a 1e-3 band around r_c^2 and the exact fp64 sequence of S:L3 (explicit round-to-nearest
+// intrinsics, no FMA contraction) decides inside it, so the list is bit-identical to the oracle's; hits are parked in a
+// fixed-stride scratch row -> row_ptr scan -> fill through a per-warp bitmask over the atoms of the system, which emits
+// every CSR row in ascending j without a sort.  Integer atomics only order the scratch; the CSR is deterministic.
 #include "common.cuh"
 
 namespace {
@@ -122,31 +122,6 @@ __device__ __forceinline__ bool within_cutoff(const double qi[3], const double *
     }
     double d2 = __dadd_rn(__dadd_rn(__dmul_rn(d[0], d[0]), __dmul_rn(d[1], d[1])), __dmul_rn(d[2], d[2]));
     return d2 < a.rc2;
-}
-
-// Same decision as within_cutoff, but most candidates are settled by an fp32 estimate of d^2: it differs from the
-// exact value by a relative error far below the 1e-3 band (fp64 difference rounded once to fp32; the image shift may
-// differ from the exact one only when |dx| ~ L/2 >= r_c, which lands outside the band or inside it, never on the
-// wrong side).  Only candidates inside the band evaluate the exact S:L3 sequence, so the list stays bit-exact.
-__device__ __forceinline__ bool within_cutoff_fast(const double qi[3], const double *__restrict__ qj, const NlArgs &a)
-{
-    float d2 = 0.f;
-#pragma unroll
-    for (int ax = 0; ax < 3; ++ax) {
-        float dx = (float)(qj[ax] - qi[ax]);
-        if (a.periodic) dx = fmaf(-a.boxf[ax], rintf(dx * a.inv_boxf[ax]), dx);
-        d2 = fmaf(dx, dx, d2);
-    }
-    if (d2 > a.rc2_hi) return false;
-    if (d2 < a.rc2_lo) return true;
-    return within_cutoff(qi, qj, a);
-}
-
-// fp32 pre-filter + exact S:L3 test, candidate position given as three doubles
-__device__ __forceinline__ bool within_cutoff_fast3(const double qi[3], double xj, double yj, double zj, const NlArgs &a)
-{
-    const double qj[3] = {xj, yj, zj};
-    return within_cutoff_fast(qi, qj, a);
 }
 
 // One CTA per (bead-system, cell).  The atoms of the cell's de-duplicated 3x3x3 stencil are staged in shared memory
@@ -342,29 +317,8 @@ __global__ void scan_rows_add_kernel(NlArgs a)
     if (row < a.rows) a.d.row_ptr[row] += a.d.block_sums[row >> 10];
 }
 
-__global__ void __launch_bounds__(256) fill_kernel(NlArgs a)
-{
-    __shared__ int sbuf[8][PIMD_MAX_NBR];
-    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    int64_t row = (int64_t)blockIdx.x * 8 + w;
-    if (row >= a.rows) return;
-    if (a.d.row_ptr[a.rows] == 0) return;   // empty or overflowed list
-    int *buf = sbuf[w];
-    const int n = a.d.nnz[row];
-    const int *hits = a.d.hits + row * a.hit_stride;
-    for (int e = lane; e < n; e += 32) buf[e] = hits[e];
-    __syncwarp();
-    const int64_t base = a.d.row_ptr[row];
-    for (int e = lane; e < n; e += 32) {   // rank sort: j values in a row are distinct (box >= 2 r_c)
-        int v = buf[e], rank = 0;
-        for (int t = 0; t < n; ++t) rank += (buf[t] < v);
-        a.d.col[base + rank] = v;
-        a.d.pair_row[base + rank] = (int)row;
-    }
-}
-
-// Same result as fill_kernel without the O(n^2) rank sort: the row's hits set bits in a per-warp bitmask over the atoms of
-// the bead-system (shared memory, N/32 words), and the set bits are emitted in ascending order.  Used when N <= 32768.
+// CSR fill with ascending rows and no sort: the row's hits set bits in a per-warp bitmask over the atoms of the bead-system
+// (shared memory, N/32 words), and the set bits are emitted in ascending order.  N <= 32768 (checked by pimd_create).
 __global__ void __launch_bounds__(256) fill_bitmask_kernel(NlArgs a, int nw)
 {
     extern __shared__ unsigned smask[];       // [8][nw]
@@ -429,8 +383,7 @@ int pimd_launch_nlist(pimd_ctx *c)
     scan_block_sums_kernel<<<1, 1024, 0, c->stream>>>(a, nblk);
     scan_rows_add_kernel<<<gthr, 256, 0, c->stream>>>(a);
     const int nw = (c->N + 31) / 32;
-    if (nw <= 1024) fill_bitmask_kernel<<<gwarp, 256, (size_t)8 * nw * sizeof(unsigned), c->stream>>>(a, nw);
-    else fill_kernel<<<gwarp, 256, 0, c->stream>>>(a);
+    fill_bitmask_kernel<<<gwarp, 256, (size_t)8 * nw * sizeof(unsigned), c->stream>>>(a, nw);
     c->launches += 8;
     PIMD_CUDA_CHECK(cudaGetLastError());
     return 0;

@@ -199,10 +199,9 @@ int launch_nm(pimd_ctx *c, uint32_t t)
 {
     NmArgs a = make_args(c);
     size_t smem = (size_t)4 * c->P * a.TC * sizeof(double);
-    static bool attr_set[3] = {false, false, false};
-    if (!attr_set[MODE]) {
+    if (!(c->attr_done & (ATTR_NM << MODE))) {
         PIMD_CUDA_CHECK(cudaFuncSetAttribute(nm_kernel<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-        attr_set[MODE] = true;
+        c->attr_done |= (ATTR_NM << MODE);
     }
     dim3 grid((3 * c->N + a.TC - 1) / a.TC, c->R), block(a.TC, NM_TY);
     nm_kernel<MODE><<<grid, block, smem, c->stream>>>(a, t);

@@ -112,6 +112,7 @@ int compute_layout(int N, int R, int P, const double box[3], const pimd_net_para
             pimd_set_error("invalid network description");
             return PIMD_ERR_ARG;
         }
+        if (N > 32768) { pimd_set_error("n_atoms = %d > 32768 per bead-system is not supported by the neighbour-list fill", N); return PIMD_ERR_ARG; }
         H = net->hidden;
         double expect;
         if (periodic) {
@@ -170,7 +171,7 @@ int compute_layout(int N, int R, int P, const double box[3], const pimd_net_para
         L->pair_row = take(cur, sizeof(int) * L->pair_cap);
         L->weights = take(cur, sizeof(float) * L->n_wfloats);
         L->wimg = take(cur, 5 * 16384 + 4096);   // bf16 UMMA images: W_e1 (16 KB), W_e2 (32 KB), W_f1 W_e2 (32 KB)
-        L->wimg_node = take(cur, (size_t)(net->n_layers > 0 ? net->n_layers : 1) * 5 * 32768);
+        L->wimg_node = take(cur, (size_t)(net->n_layers > 0 ? net->n_layers : 1) * 20 * 16384);   // 20 half-images (16 KB) per layer: gfn_node_tc.cu
         L->xs0 = take(cur, sizeof(float) * (size_t)net->n_species * H);
         if (net->gemm_dtype == 1 && net->n_rbf == 64 && H == 128) {   // tile images of the tcgen05 pair pipeline
             const size_t n_tiles = (size_t)(L->pair_cap / 128 + 1);
@@ -200,6 +201,30 @@ uint16_t f32_to_bf16_rne(float f)
     return (uint16_t)(u >> 16);
 }
 
+// IEEE binary16, round to nearest even (finite inputs well inside the range; used for the readout weights w_f2)
+uint16_t f32_to_f16_rne(float f)
+{
+    uint32_t u;
+    memcpy(&u, &f, 4);
+    const uint32_t sign = (u >> 16) & 0x8000u;
+    const int32_t e = (int32_t)((u >> 23) & 0xFF) - 127 + 15;
+    uint32_t m = u & 0x7FFFFFu;
+    if (e >= 31) return (uint16_t)(sign | 0x7C00u);                      // overflow -> inf
+    if (e <= 0) {                                                        // subnormal or zero
+        if (e < -10) return (uint16_t)sign;
+        m |= 0x800000u;
+        const int shift = 14 - e;
+        uint32_t r = m >> shift;
+        const uint32_t rem = m & ((1u << shift) - 1u), half = 1u << (shift - 1);
+        if (rem > half || (rem == half && (r & 1u))) ++r;
+        return (uint16_t)(sign | r);
+    }
+    uint32_t r = ((uint32_t)e << 10) | (m >> 13);
+    const uint32_t rem = m & 0x1FFFu;
+    if (rem > 0x1000u || (rem == 0x1000u && (r & 1u))) ++r;              // carries into the exponent correctly
+    return (uint16_t)(sign | r);
+}
+
 // bf16 image of a row-major [n_rows][n_k] matrix as UMMA K-major operand blocks of 64 k (128-byte rows, 16-byte
 // chunks XOR-swizzled by row & 7), block kb at byte offset kb * n_rows * 128
 void build_umma_image(const float *W, int n_rows, int n_k, float scale, uint16_t *img)
@@ -210,6 +235,23 @@ void build_umma_image(const float *W, int n_rows, int n_k, float scale, uint16_t
                 for (int e = 0; e < 8; ++e)
                     img[(size_t)kb * n_rows * 64 + (size_t)n * 64 + ((c ^ (n & 7)) * 8) + e] =
                         f32_to_bf16_rne(scale * W[(size_t)n * n_k + kb * 64 + c * 8 + e]);
+}
+
+// the same image for W = hi + lo as a bf16 pair: hi = bf16(scale W), lo = bf16(scale W - hi)  (split-precision products of the
+// atom-wise layers, gfn_node_tc.cu)
+void build_umma_image_split(const float *W, int n_rows, int n_k, float scale, uint16_t *img_hi, uint16_t *img_lo)
+{
+    std::vector<float> hi((size_t)n_rows * n_k), lo((size_t)n_rows * n_k);
+    for (size_t i = 0; i < hi.size(); ++i) {
+        const float v = scale * W[i];
+        const uint32_t hb = (uint32_t)f32_to_bf16_rne(v) << 16;
+        float hf;
+        memcpy(&hf, &hb, 4);
+        hi[i] = hf;
+        lo[i] = v - hf;
+    }
+    build_umma_image(hi.data(), n_rows, n_k, 1.0f, img_hi);
+    build_umma_image(lo.data(), n_rows, n_k, 1.0f, img_lo);
 }
 
 // derived, transposed fp32 weights in the order the kernels use (S:G0 is the input order)
@@ -280,6 +322,18 @@ int check_device_error(pimd_ctx *c)
     return 0;
 }
 
+// every entry point runs on the context's device, whatever device is current in the calling thread
+int enter(pimd_ctx *c)
+{
+    int dev = -1;
+    if (cudaGetDevice(&dev) == cudaSuccess && dev == c->device) return 0;
+    PIMD_CUDA_CHECK(cudaSetDevice(c->device));
+    return 0;
+}
+
+// the Philox counter holds the step as one 32-bit word (S:N4)
+constexpr int64_t PIMD_MAX_STEP = 4294967295LL;
+
 int compute_forces(pimd_ctx *c)
 {
     int rc;
@@ -329,9 +383,10 @@ extern "C" int pimd_create(pimd_ctx **out, int n_atoms, int n_replicas, const in
     }
     if (((uintptr_t)d_workspace) % 256 != 0) { pimd_set_error("workspace must be 256-byte aligned"); return PIMD_ERR_ARG; }
     const int N = n_atoms, R = n_replicas;
+    if (net->n_species < 1) { pimd_set_error("n_species = %d (masses_amu has one entry per species)", net->n_species); return PIMD_ERR_ARG; }
     for (int i = 0; i < N; ++i)
-        if (species[i] < 0 || (net->kind == 0 && species[i] >= net->n_species)) {
-            pimd_set_error("species[%d] = %d out of range", i, species[i]);
+        if (species[i] < 0 || species[i] >= net->n_species) {
+            pimd_set_error("species[%d] = %d out of range [0, %d)", i, species[i], net->n_species);
             return PIMD_ERR_ARG;
         }
     if (net->kind == 0) {
@@ -351,7 +406,8 @@ extern "C" int pimd_create(pimd_ctx **out, int n_atoms, int n_replicas, const in
     c->harmonic_omega = net->harmonic_omega;
     c->stream = (cudaStream_t)cuda_stream;
     int dev = 0;
-    cudaError_t e = cudaGetDevice(&dev);
+    cudaError_t e = cudaGetDevice(&dev);          // the device current at creation owns the workspace and the stream
+    c->device = dev;
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, dev);
     if (e != cudaSuccess) {
         pimd_set_error("no CUDA device: %s", cudaGetErrorString(e));
@@ -425,10 +481,6 @@ extern "C" int pimd_create(pimd_ctx **out, int n_atoms, int n_replicas, const in
         RawNet raw;
         build_weights(net, wd, offs, Wfe, raw);
         c->use_tc = (net->gemm_dtype == 1 && net->n_rbf == 64 && net->hidden == 128) ? 1 : 0;
-        {
-            const char *e = getenv("PIMD_MSG_ROWGEMM");      // experimental formulation of the later message passes (off by default)
-            c->msg_rowgemm = (c->use_tc && e && e[0] == '1') ? 1 : 0;
-        }
         c->wimg_e1 = (uint16_t *)(ws + L.wimg); c->wimg_e2 = c->wimg_e1 + 8192; c->wimg_fe = c->wimg_e2 + 16384;
         if (c->use_tc) {
             wimg.resize(5 * 8192 + 2048);
@@ -440,7 +492,13 @@ extern "C" int pimd_create(pimd_ctx **out, int n_atoms, int n_replicas, const in
             {   // w_f2 on 16 identical rows: B operand of the head's 128x16x128 readout product
                 std::vector<float> rep((size_t)16 * H);
                 for (int r = 0; r < 16; ++r) for (int k = 0; k < H; ++k) rep[(size_t)r * H + k] = raw.wf2[k];
-                build_umma_image(rep.data(), 16, H, 1.0f, wimg.data() + 5 * 8192);
+                uint16_t *img = wimg.data() + 5 * 8192;      // same layout as build_umma_image, fp16 elements (the head's act operand is fp16)
+                for (int kb = 0; kb < H / 64; ++kb)
+                    for (int n = 0; n < 16; ++n)
+                        for (int cch = 0; cch < 8; ++cch)
+                            for (int e = 0; e < 8; ++e)
+                                img[(size_t)kb * 16 * 64 + (size_t)n * 64 + ((cch ^ (n & 7)) * 8) + e] =
+                                    f32_to_f16_rne(rep[(size_t)n * H + kb * 64 + cch * 8 + e]);
             }
             c->wimg_wf2 = c->wimg_e1 + 5 * 8192;
             CREATE_CHECK(cudaMemcpyAsync(c->wimg_e1, wimg.data(), sizeof(uint16_t) * wimg.size(), cudaMemcpyHostToDevice, st));
@@ -469,14 +527,16 @@ extern "C" int pimd_create(pimd_ctx **out, int n_atoms, int n_replicas, const in
             c->h1_img = (unsigned char *)(ws + L.h1_img); c->meta_img = (unsigned char *)(ws + L.meta_img);
             for (int k = 0; k < H && k < 128; ++k) c->h_be1_half[k] = 0.5f * raw.be1[k];
             const int Ln = net->n_layers;
-            wimg_node.resize((size_t)(Ln > 0 ? Ln : 1) * 5 * 16384);
+            // per layer 20 half-images of 8192 bf16 in the order a tile consumes them: (W_vn/2, W_vm/2, W_v2, W_a) as hi | lo
+            // (each two K blocks), then W_s^{l+1} hi (and its lo, unused) or, in the last layer, W_f1 hi | lo
+            wimg_node.resize((size_t)(Ln > 0 ? Ln : 1) * 20 * 8192);
             for (int l = 0; l < Ln; ++l) {
-                uint16_t *img = wimg_node.data() + (size_t)l * 5 * 16384;
-                build_umma_image(raw.layer[l].Wvn, H, H, 0.5f, img);
-                build_umma_image(raw.layer[l].Wvm, H, H, 0.5f, img + 16384);
-                build_umma_image(raw.layer[l].Wv2, H, H, 1.0f, img + 2 * 16384);
-                build_umma_image(raw.layer[l].Wa, H, H, 1.0f, img + 3 * 16384);
-                build_umma_image(l + 1 < Ln ? raw.layer[l + 1].Ws : raw.Wf1, H, H, 1.0f, img + 4 * 16384);
+                uint16_t *img = wimg_node.data() + (size_t)l * 20 * 8192;
+                build_umma_image_split(raw.layer[l].Wvn, H, H, 0.5f, img, img + 16384);
+                build_umma_image_split(raw.layer[l].Wvm, H, H, 0.5f, img + 2 * 16384, img + 3 * 16384);
+                build_umma_image_split(raw.layer[l].Wv2, H, H, 1.0f, img + 4 * 16384, img + 5 * 16384);
+                build_umma_image_split(raw.layer[l].Wa, H, H, 1.0f, img + 6 * 16384, img + 7 * 16384);
+                build_umma_image_split(l + 1 < Ln ? raw.layer[l + 1].Ws : raw.Wf1, H, H, 1.0f, img + 8 * 16384, img + 9 * 16384);
             }
             xs0.assign((size_t)net->n_species * H, 0.f);
             if (Ln > 0)
@@ -521,6 +581,7 @@ extern "C" int pimd_create(pimd_ctx **out, int n_atoms, int n_replicas, const in
 extern "C" void pimd_destroy(pimd_ctx *c)
 {
     if (!c) return;
+    (void)enter(c);
     cudaStreamSynchronize(c->stream);
     if (c->prof) {
         c->prof->clear();
@@ -533,7 +594,9 @@ extern "C" void pimd_destroy(pimd_ctx *c)
 extern "C" int pimd_step(pimd_ctx *c, int n)
 {
     if (!c || n < 0) { pimd_set_error("invalid argument"); return PIMD_ERR_ARG; }
+    if (c->step + n > PIMD_MAX_STEP) { pimd_set_error("step counter would exceed 2^32 - 1 (the noise counter holds 32 bits)"); return PIMD_ERR_ARG; }
     int rc;
+    if ((rc = enter(c))) return rc;
     if (!c->forces_valid && (rc = compute_forces(c))) return rc;
     for (int s = 0; s < n; ++s) {
         const uint32_t t = (uint32_t)c->step;
@@ -555,6 +618,7 @@ extern "C" int pimd_forces(pimd_ctx *c, float *d_out)
 {
     if (!c || !d_out) { pimd_set_error("null argument"); return PIMD_ERR_ARG; }
     int rc;
+    if ((rc = enter(c))) return rc;
     if ((rc = compute_forces(c))) return rc;
     return pimd_launch_copy_forces_f32(c, d_out);
 }
@@ -563,6 +627,7 @@ extern "C" int pimd_estimators(pimd_ctx *c, pimd_estimators_t *h_out)
 {
     if (!c || !h_out) { pimd_set_error("null argument"); return PIMD_ERR_ARG; }
     int rc;
+    if ((rc = enter(c))) return rc;
     if (!c->forces_valid && (rc = compute_forces(c))) return rc;
     if ((rc = pimd_launch_estimators(c))) return rc;
     std::vector<double> tmp((size_t)c->R * 8);
@@ -578,6 +643,7 @@ extern "C" int pimd_estimators(pimd_ctx *c, pimd_estimators_t *h_out)
 extern "C" int pimd_get_state(pimd_ctx *c, double *d_q, double *d_p, int64_t *step)
 {
     if (!c) { pimd_set_error("null context"); return PIMD_ERR_ARG; }
+    if (int rc = enter(c)) return rc;
     const size_t bytes = sizeof(double) * (size_t)c->rows * 3;
     if (d_q) PIMD_CUDA_CHECK(cudaMemcpyAsync(d_q, c->q, bytes, cudaMemcpyDeviceToDevice, c->stream));
     if (d_p) PIMD_CUDA_CHECK(cudaMemcpyAsync(d_p, c->p, bytes, cudaMemcpyDeviceToDevice, c->stream));
@@ -588,6 +654,8 @@ extern "C" int pimd_get_state(pimd_ctx *c, double *d_q, double *d_p, int64_t *st
 extern "C" int pimd_set_state(pimd_ctx *c, const double *d_q, const double *d_p, int64_t step)
 {
     if (!c) { pimd_set_error("null context"); return PIMD_ERR_ARG; }
+    if (step < 0 || step > PIMD_MAX_STEP) { pimd_set_error("step %lld outside [0, 2^32 - 1] (the noise counter holds 32 bits)", (long long)step); return PIMD_ERR_ARG; }
+    if (int rc = enter(c)) return rc;
     const size_t bytes = sizeof(double) * (size_t)c->rows * 3;
     if (d_q) PIMD_CUDA_CHECK(cudaMemcpyAsync(c->q, d_q, bytes, cudaMemcpyDeviceToDevice, c->stream));
     if (d_p) PIMD_CUDA_CHECK(cudaMemcpyAsync(c->p, d_p, bytes, cudaMemcpyDeviceToDevice, c->stream));
@@ -600,6 +668,7 @@ extern "C" int pimd_get_forces_cached(pimd_ctx *c, double *d_F)
 {
     if (!c || !d_F) { pimd_set_error("null argument"); return PIMD_ERR_ARG; }
     int rc;
+    if ((rc = enter(c))) return rc;
     if (!c->forces_valid && (rc = compute_forces(c))) return rc;
     PIMD_CUDA_CHECK(cudaMemcpyAsync(d_F, c->F, sizeof(double) * (size_t)c->rows * 3, cudaMemcpyDeviceToDevice, c->stream));
     return 0;
@@ -608,6 +677,7 @@ extern "C" int pimd_get_forces_cached(pimd_ctx *c, double *d_F)
 extern "C" int pimd_set_forces_cached(pimd_ctx *c, const double *d_F)
 {
     if (!c || !d_F) { pimd_set_error("null argument"); return PIMD_ERR_ARG; }
+    if (int rc = enter(c)) return rc;
     PIMD_CUDA_CHECK(cudaMemcpyAsync(c->F, d_F, sizeof(double) * (size_t)c->rows * 3, cudaMemcpyDeviceToDevice, c->stream));
     c->forces_valid = 1;
     return 0;
@@ -618,6 +688,7 @@ extern "C" int pimd_nlist(pimd_ctx *c, int32_t *d_row_ptr, int32_t *d_col, int64
     if (!c || !d_row_ptr || !d_col || !h_n_pairs) { pimd_set_error("null argument"); return PIMD_ERR_ARG; }
     if (c->kind != 0) { pimd_set_error("no neighbour list for this potential kind"); return PIMD_ERR_ARG; }
     int rc;
+    if ((rc = enter(c))) return rc;
     if ((rc = pimd_launch_nlist(c))) return rc;
     int n = 0;
     PIMD_CUDA_CHECK(cudaMemcpyAsync(&n, c->nl.row_ptr + c->rows, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
@@ -633,6 +704,7 @@ extern "C" int pimd_nlist(pimd_ctx *c, int32_t *d_row_ptr, int32_t *d_col, int64
 extern "C" int pimd_sync(pimd_ctx *c)
 {
     if (!c) { pimd_set_error("null context"); return PIMD_ERR_ARG; }
+    if (int rc = enter(c)) return rc;
     return check_device_error(c);
 }
 

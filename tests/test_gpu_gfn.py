@@ -8,12 +8,12 @@ import pytest
 
 import oracle
 import pimd_inputs as pi
-from gpu_util import make_pair, pair_from_workload, spread_beads, gpu_state, assert_forces_close
+from gpu_util import make_pair, pair_from_workload, spread_beads, gpu_state, assert_forces_close, assert_forces_bf16_spec
 
 pytestmark = pytest.mark.gpu
 
 RTOL32, ATOL32 = 1e-4, 1e-4
-RTOL16 = 2e-2
+# bf16 configs: |dF_i|_2 <= 2e-2 max(|F_i|_2, rms|F|) per atom (gpu_util.assert_forces_bf16_spec)
 
 
 def _forces_pair(gpu, ref):
@@ -54,14 +54,16 @@ def test_small_systems_tensor_core_path(cuda_device, L):
         gpu, ref = make_pair(sp, x, box, P, 300.0, 0.25, 1.0, 0, spec)
         spread_beads(gpu, ref, scale=0.05)
         Fg, Fr = _forces_pair(gpu, ref)
-        # With random weights F_i is the small remainder of signed terms that cancel (readout channels, then
-        # neighbours): bf16 operand rounding (2^-9 relative per operand) moves it by about 2^-9 of the SUM OF THE
-        # MAGNITUDES of those terms, whatever |F_i| is.  Bound: one bf16 ulp (2^-8) of that sum.
+        # north_star form, per bead-system; these random-weight clusters are the hard case (F_i is the small remainder of
+        # signed terms that cancel: sum |terms| ~ 10^2 |F_i|), which is why the atom-wise products run split-precision
+        for rr in range(Fg.shape[0]):
+            for k in range(Fg.shape[1]):
+                assert_forces_bf16_spec(Fg[rr, k], Fr[rr, k], f"L{L} N{n_at} replica {rr} bead {k}")
+        # complement: against the sum of the MAGNITUDES of the terms of F_i the error is below 2^-10 (measured 2^-12)
         gross = ref.force_gross()
         assert gross.max() > 1e-3 and np.all(np.linalg.norm(Fr, axis=-1) <= gross + 1e-12)
         err = np.abs(Fg - Fr).max(axis=-1)
-        assert np.all(err <= 2.0 ** -8 * gross + 1e-6), (L, n_at, (err / (gross + 1e-30)).max())
-        assert np.sqrt((err ** 2).mean()) <= 2.0 ** -10 * np.sqrt((gross ** 2).mean())  # rms well inside the bound
+        assert np.all(err <= 2.0 ** -10 * gross + 1e-6), (L, n_at, (err / (gross + 1e-30)).max())
         if box[0] == 0:
             assert np.all(Fg[:, :, 5] == 0.0)
 
@@ -76,24 +78,25 @@ def test_fp32_workload_forces(cuda_device, name):
     assert_forces_close(Fg, Fr, RTOL32, ATOL32, name)
 
 
-@pytest.mark.parametrize("name,beads", [("ice512", [0, 13, 31]), ("water4096", [7])])
+@pytest.mark.parametrize("name,beads", [("ice512", list(range(32))), ("water4096", [7, 20])])
 def test_full_size_forces_on_sampled_beads(cuda_device, name, beads):
-    """Full workload in the launch configuration bench.py times; the oracle evaluates sampled
-    bead-systems one by one (forces of a bead depend only on that bead's positions)."""
+    """Full workload in the launch configuration bench.py times; the oracle evaluates bead-systems one by one (forces of
+    a bead depend only on that bead's positions): all 32 beads of the headline config, two of the largest one."""
     import paper_2503_23728_b200 as pb
     w = pi.make_workload(name)
+    assert w.net.gemm_dtype == 1
     gpu = pb.PIMD.from_workload(w)
     q, p, st = gpu_state(gpu)
     q = q + 0.03 * np.random.default_rng(3).standard_normal(q.shape)
     gpu.set_state(q, p, st)
     Fg = gpu.forces().cpu().numpy().astype(np.float64)
-    rtol = RTOL16 if w.net.gemm_dtype == 1 else RTOL32
-    atol = 2e-2 if w.net.gemm_dtype == 1 else ATOL32
+    worst, rms = 0.0, 0.0
     for k in beads:
         ref = oracle.RefPIMD(w.species, w.masses_amu, q[0, k][None], w.box, 1, w.T, w.dt, -1.0, 0,
                              oracle.RefNet.from_spec(w.net))
-        Fr = ref.forces()[0, 0]
-        assert_forces_close(Fg[0, k], Fr, rtol, atol, f"{name} bead {k}")
+        mx, rr = assert_forces_bf16_spec(Fg[0, k], ref.forces()[0, 0], f"{name} bead {k}")
+        worst, rms = max(worst, mx), max(rms, rr)
+    assert rms <= 5e-3, rms          # norm-wise: rms|dF| / rms|F| (measured 1e-3)
     assert np.isfinite(Fg).all()
     assert np.abs(Fg.sum(axis=2)).max() < 5e-2
 
@@ -197,26 +200,3 @@ def test_tensor_core_path_is_bitwise_deterministic(cuda_device):
     a = gpu.forces().clone()
     for _ in range(3):
         assert torch.equal(a, gpu.forces())
-
-
-def test_row_gemm_message_pass_parity_and_determinism(cuda_device, monkeypatch):
-    """Experimental formulation of the later message passes (one GEMM per CSR row with the pair index as the contraction
-    dimension, W_e2 applied per row in fp32; PIMD_MSG_ROWGEMM=1): same bound as the default path,
-    and the token chain fixes the accumulation order (identical bits every time)."""
-    import torch
-    monkeypatch.setenv("PIMD_MSG_ROWGEMM", "1")
-    rng = np.random.default_rng(31)
-    for box, n_at, P in [(np.zeros(3), 23, 3), (np.array([12.5, 13.0, 12.2]), 700, 2)]:
-        x = rng.uniform(0, 1, (1, n_at, 3)) * (box if box[0] > 0 else 4.5)
-        sp = rng.integers(0, 3, n_at).astype(np.int32)
-        spec = _biased_spec(64, 128, 3, 3.0, 1.0 / 12.0, 0.2)
-        spec.gemm_dtype = 1
-        gpu, ref = make_pair(sp, x, box, P, 300.0, 0.25, 1.0, 0, spec)
-        spread_beads(gpu, ref, scale=0.05)
-        a = gpu.forces().clone()
-        Fg, Fr = a.cpu().numpy().astype(np.float64), ref.forces()
-        gross = ref.force_gross()
-        err = np.abs(Fg - Fr).max(axis=-1)
-        assert np.all(err <= 2.0 ** -8 * gross + 1e-6), (n_at, (err / (gross + 1e-30)).max())
-        for _ in range(3):
-            assert torch.equal(a, gpu.forces())

@@ -92,3 +92,28 @@ def test_invalid_arguments(cuda_device):
     w.net.weights = w.net.weights[:-1]
     with pytest.raises(pb.PimdError):
         pb.PIMD.from_workload(w)
+
+
+def test_pile_friction_constants_on_gpu(cuda_device):
+    """PILE-L friction pinned against closed forms, not against the oracle (which could share a mistake): one O A O step with
+    F = 0 from q = 0 and a large deterministic mode momentum gives E[p~_k'] / p~_k = exp(-gamma_k dt) cos(omega_k dt) with
+    gamma_k = 2 omega_k (k >= 1) and gamma_0 given in ps^-1."""
+    import oracle
+    from oracle import KB_EV, HBAR_EVFS, AMU_INTERNAL
+    import paper_2503_23728_b200 as pb
+    P, T, dt, gamma_ps, N, amp = 6, 300.0, 0.7, 80.0, 4096, 100.0
+    sig = np.sqrt(pi.MASSES_AMU[0] * AMU_INTERNAL * KB_EV * T * P)
+    C = oracle.nm_matrix(P)      # the matrix convention N2 (pinned by C C^T = I and the ring diagonalisation)
+    pt = np.full((1, P, N, 3), amp * sig)
+    p = np.einsum("jk,rkia->rjia", C, pt)
+    gpu = pb.PIMD(np.zeros(N, np.int32), pi.MASSES_AMU, np.zeros((1, N, 3)), np.zeros(3), P, T, dt, gamma_ps, 5, _spec(2))
+    gpu.set_state(np.zeros_like(p), p, 0)
+    gpu.step(1)
+    _, p1, _ = gpu_state(gpu)
+    got = (np.einsum("jk,rjia->rkia", C, p1) / pt)[0].reshape(P, -1).mean(axis=1)
+    wk = 2 * (P * KB_EV * T / HBAR_EVFS) * np.sin(np.arange(P) * np.pi / P)
+    gam = 2.0 * wk
+    gam[0] = gamma_ps * 1e-3
+    want = np.exp(-gam * dt) * np.cos(wk * dt)
+    tol = 3 * np.sqrt(2.0) / amp / np.sqrt(3 * N)
+    assert np.all(np.abs(got - want) < tol), (got, want, tol)

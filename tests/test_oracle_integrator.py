@@ -198,3 +198,84 @@ def test_qho_estimators_reach_finite_P_energy():
         assert abs(e - target) / target < 0.005, (e, target)
         assert abs(e - exact) / exact > 0.02  # distinguishes finite-P from P->inf (4.6 % apart)
     assert abs(acc[4] - T) / T < 0.03  # centroid temperature
+
+
+# ---- PILE-L friction (PAPER.md L426 names the thermostat): c1_k = exp(-gamma_k dt/2), gamma_k = 2 omega_k for
+# k >= 1, gamma_0 = the input in ps^-1.  The variance pins above hold for ANY c1 in (0, 1); these three do not.
+def pile_mode_ratio_setup(P, T, N, amp=100.0):
+    """q = 0 and a large deterministic mode momentum p~_k = amp * sqrt(m/beta_P) on every (atom, dim, mode): (q, p, sigma)."""
+    masses = np.array([1.008, 12.011, 15.999])
+    sig = np.sqrt(masses[0] * AMU_INTERNAL * KB_EV * T * P)
+    C = oracle.nm_matrix(P)
+    pt = np.full((1, P, N, 3), amp * sig)
+    p = np.einsum("jk,rkia->rjia", C, pt)
+    return np.zeros((1, P, N, 3)), p, pt, C
+
+
+def pile_expected_ratio(P, T, dt, gamma_ps):
+    """E[p~_k(after one O A O step with F = 0, q~ = 0)] / p~_k = c1_k^2 cos(omega_k dt)."""
+    wP = P * KB_EV * T / HBAR_EVFS
+    wk = 2 * wP * np.sin(np.arange(P) * np.pi / P)
+    gam = 2.0 * wk
+    gam[0] = gamma_ps * 1e-3            # ps^-1 -> fs^-1
+    return np.exp(-gam * dt) * np.cos(wk * dt)
+
+
+def test_pile_friction_one_step_mean_ratio():
+    P, T, dt, gamma_ps, N = 6, 300.0, 0.7, 80.0, 4096
+    q, p, pt, C = pile_mode_ratio_setup(P, T, N)
+    sim = RefPIMD(np.zeros(N, np.int32), np.array([1.008, 12.011, 15.999]), np.zeros((1, N, 3)), np.zeros(3), P, T, dt,
+                  gamma_ps, 5, RefNet(kind=2))
+    sim.set_state(q, p, 0)
+    sim.step(1)
+    _, p1, _ = sim.get_state()
+    ratio = (np.einsum("jk,rjia->rkia", C, p1) / pt)[0].reshape(P, -1)
+    want = pile_expected_ratio(P, T, dt, gamma_ps)
+    # noise per sample <= sqrt(2)/amp; 3 sigma of the mean over 3N samples
+    tol = 3 * np.sqrt(2.0) / 100.0 / np.sqrt(3 * N)
+    got = ratio.mean(axis=1)
+    assert np.all(np.abs(got - want) < tol), (got, want, tol)
+    # the alternatives a plausible mistake would give are far outside: gamma_k = omega_k, gamma_0 off by 1000x
+    wP = P * KB_EV * T / HBAR_EVFS
+    w1 = 2 * wP * np.sin(np.pi / P)
+    assert abs(np.exp(-w1 * dt) * np.cos(w1 * dt) - want[1]) > 100 * tol
+    assert abs(np.exp(-gamma_ps * dt) - want[0]) > 100 * tol and abs(np.exp(-gamma_ps * 1e-6 * dt) - want[0]) > 100 * tol
+
+
+def test_pile_internal_modes_are_critically_damped():
+    """gamma_k = 2 omega_k is critical damping of the free ring-polymer mode: <q~_k(t)> = q0 (1 + w t) exp(-w t), no overshoot
+    (closed form of the damped oscillator, independent of the integrator's own constants; small dt)."""
+    P, T, dt, N, k = 8, 300.0, 0.05, 3000, 1
+    masses = np.array([1.008, 12.011, 15.999])
+    C = oracle.nm_matrix(P)
+    wk = 2 * (P * KB_EV * T / HBAR_EVFS) * np.sin(k * np.pi / P)
+    sig_q = np.sqrt(KB_EV * T * P / (masses[0] * AMU_INTERNAL)) / wk        # thermal width of the mode
+    q0 = 200.0 * sig_q
+    q = np.zeros((1, P, N, 3)); q[0, :, :, :] = (q0 * C[:, k])[:, None, None]
+    sim = RefPIMD(np.zeros(N, np.int32), masses, np.zeros((1, N, 3)), np.zeros(3), P, T, dt, 1.0, 9, RefNet(kind=2))
+    sim.set_state(q, np.zeros_like(q), 0)
+    t = 0.0
+    for _ in range(4):
+        sim.step(60)
+        t += 60 * dt
+        qn, _, _ = sim.get_state()
+        got = np.einsum("j,jia->ia", C[:, k], qn[0]).mean() / q0
+        want = (1.0 + wk * t) * np.exp(-wk * t)
+        under = np.exp(-0.5 * wk * t) * (np.cos(np.sqrt(0.75) * wk * t) + np.sin(np.sqrt(0.75) * wk * t) / np.sqrt(3.0))  # gamma = omega
+        assert abs(got - want) < 2e-3, (t, got, want)
+        assert abs(under - want) > 0.02
+
+
+def test_centroid_friction_is_in_inverse_picoseconds():
+    """P = 1, free particle: Ornstein-Uhlenbeck mean decay <p(t)> = p0 exp(-gamma t) with gamma given in ps^-1 (OBABO with
+    F = 0 reproduces it exactly at the step boundaries)."""
+    T, dt, gamma_ps, N = 300.0, 2.0, 25.0, 4096
+    masses = np.array([1.008, 12.011, 15.999])
+    sig = np.sqrt(masses[0] * AMU_INTERNAL * KB_EV * T)
+    p = np.full((1, 1, N, 3), 100.0 * sig)
+    sim = RefPIMD(np.zeros(N, np.int32), masses, np.zeros((1, N, 3)), np.zeros(3), 1, T, dt, gamma_ps, 2, RefNet(kind=2))
+    sim.set_state(np.zeros_like(p), p, 0)
+    sim.step(20)                                   # t = 40 fs = 0.04 ps: exp(-1)
+    _, p1, _ = sim.get_state()
+    got = (p1 / p).mean()
+    assert abs(got - np.exp(-gamma_ps * 1e-3 * 20 * dt)) < 3 * 1.0 / 100.0 / np.sqrt(3 * N) + 1e-12, got
