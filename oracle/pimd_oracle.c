@@ -74,6 +74,8 @@ typedef struct {
     double *C;         /* [P][P], C[j*P+k], bead j, mode k */
     double *omega_k;   /* [P] */
     int forces_valid;
+    int transform;  /* 0 normal modes (N2), 1 staging, 2 primitive (no transformation, explicit spring forces) */
+    int thermostat; /* 0 PILE-L / white-noise Langevin, 1 PILE-G (global velocity rescaling of the free mode) */
 } ref_ctx;
 
 /* ------------------------------------------------------------------ */
@@ -503,6 +505,219 @@ static void step_A(ref_ctx *c)
         }
 }
 
+
+/* ------------------------------------------------------------------ */
+/* integrator variants: staging transformation, PILE-G, primitive                                   */
+/* P:L52 "the normal mode or staging transformation is employed to decouple the evolution of individual beads";    */
+/* P:L114 "For primitive PIMD, inter-bead harmonic coupling potentials are incorporated as pluggable energy terms" */
+/* ------------------------------------------------------------------ */
+/* Staging variables (Tuckerman, Berne, Martyna, Klein 1993), beads j = 0..P-1 with q_P = q_0:
+ *   u_0 = q_0,   u_j = q_j - (j q_{j+1} + q_0) / (j + 1)   for j = 1..P-1
+ * Staging masses: lam_0 = 1 (no spring), lam_j = (j+1)/j for j >= 1, so that
+ *   sum_j 1/2 m w_P^2 (q_j - q_{j+1})^2 = sum_{j>=1} 1/2 m lam_j w_P^2 u_j^2,
+ * and with kinetic masses m lam_j every staging mode j >= 1 oscillates at w_P; u_0 moves freely with mass m.   */
+static void stage_fwd(const double *q, double *u, int P)
+{
+    u[0] = q[0];
+    for (int j = 1; j < P; ++j) {
+        double qn = (j + 1 < P) ? q[j + 1] : q[0];
+        u[j] = q[j] - ((double)j * qn + q[0]) / (double)(j + 1);
+    }
+}
+/* inverse, from the top bead down: q_0 = u_0; q_j = u_j + j/(j+1) q_{j+1} + u_0/(j+1) */
+static void stage_inv(const double *u, double *q, int P)
+{
+    q[0] = u[0];
+    for (int j = P - 1; j >= 1; --j) {
+        double qn = (j + 1 < P) ? q[j + 1] : q[0];
+        q[j] = u[j] + ((double)j / (double)(j + 1)) * qn + u[0] / (double)(j + 1);
+    }
+}
+/* chain rule dV/du from dV/dq (the same map takes bead momenta p_q to staging momenta p_u):
+ *   f_u0 = sum_j f_qj;   f_uj = f_qj + (j-1)/j f_u(j-1)  for j >= 1 */
+static void stage_force(const double *fq, double *fu, int P)
+{
+    double s = 0.0;
+    for (int j = 0; j < P; ++j) s += fq[j];
+    fu[0] = s;
+    for (int j = 1; j < P; ++j) fu[j] = fq[j] + ((j > 1) ? ((double)(j - 1) / (double)j) * fu[j - 1] : 0.0);
+}
+/* canonical bead momenta from staging momenta, p_qj = sum_k (du_k/dq_j) p_uk, read off the definition of u:
+ *   p_q0 = p_u0 - sum_{k>=1} p_uk/(k+1) - (P-1)/P p_u(P-1)   (the last term: q_P = q_0 inside u_{P-1}; P >= 2)
+ *   p_qj = p_uj - (j-1)/j p_u(j-1)                            for j >= 1 */
+static void stage_mom_to_bead(const double *pu, double *pq, int P)
+{
+    double s = pu[0];
+    for (int k = 1; k < P; ++k) s -= pu[k] / (double)(k + 1);
+    if (P >= 2) s -= ((double)(P - 1) / (double)P) * pu[P - 1];
+    pq[0] = s;
+    for (int j = 1; j < P; ++j) pq[j] = pu[j] - ((j > 1) ? ((double)(j - 1) / (double)j) * pu[j - 1] : 0.0);
+}
+static double stage_lam(int j) { return j == 0 ? 1.0 : (double)(j + 1) / (double)j; }
+
+/* gather / scatter one (r, i, a) column of P beads */
+static void col_get(const ref_ctx *c, const double *v, int r, int i, int a, double *out)
+{
+    for (int j = 0; j < c->P; ++j) out[j] = v[idx4(c, r, j, i, a)];
+}
+static void col_put(const ref_ctx *c, double *v, int r, int i, int a, const double *in)
+{
+    for (int j = 0; j < c->P; ++j) v[idx4(c, r, j, i, a)] = in[j];
+}
+
+/* The state array p always holds canonical BEAD momenta p_q (conjugate to q).  Mode momenta of one column: */
+static void mom_to_modes(const ref_ctx *c, int r, int i, int a, double *pm)
+{
+    double pq[1024];
+    if (c->transform == 0) { to_modes(c, c->p, r, i, a, pm); return; }
+    col_get(c, c->p, r, i, a, pq);
+    if (c->transform == 1) stage_force(pq, pm, c->P);
+    else memcpy(pm, pq, sizeof(double) * c->P);
+}
+static void mom_from_modes(ref_ctx *c, int r, int i, int a, const double *pm)
+{
+    double pq[1024];
+    if (c->transform == 0) { from_modes(c, pm, r, i, a, c->p); return; }
+    if (c->transform == 1) stage_mom_to_bead(pm, pq, c->P);
+    else memcpy(pq, pm, sizeof(double) * c->P);
+    col_put(c, c->p, r, i, a, pq);
+}
+/* mass factor, free-ring frequency and PILE friction of mode k */
+static double mode_lam(const ref_ctx *c, int k) { return c->transform == 1 ? stage_lam(k) : 1.0; }
+static double mode_omega(const ref_ctx *c, int k)
+{
+    if (c->transform == 0) return c->omega_k[k];
+    if (c->transform == 1) return k == 0 ? 0.0 : c->P * KB_EV * c->T / HBAR_EVFS;
+    return 0.0; /* primitive: springs are explicit forces, every bead flies freely in A */
+}
+static double mode_gamma(const ref_ctx *c, int k)
+{
+    if (c->transform == 2) return c->gamma_fs; /* white-noise Langevin on every bead */
+    return (k == 0) ? c->gamma_fs : 2.0 * mode_omega(c, k); /* PILE: critical damping of the free-ring mode */
+}
+
+/* O(dt/2) for any transform / thermostat.  PILE-G (Ceriotti, Parrinello, Markland, Manolopoulos 2010, sec. II.D with the
+ * stochastic velocity rescaling of Bussi, Donadio, Parrinello 2007): the free mode (k = 0) of ALL atoms of a replica is scaled by
+ *   alpha^2 = c + (1-c) (R1^2 + S) / (2 beta_P K) + 2 R1 sqrt(c (1-c) / (2 beta_P K)),   c = exp(-gamma dt/2),
+ *   sign(alpha) = sign(R1 + sqrt(2 beta_P K c / (1-c))),
+ * K = kinetic energy of the free modes, R1 and S = the first normal and the sum of the squares of the other 3N-1 normals
+ * of the SAME counter-based stream PILE-L would use for mode 0 (atom, r*P+0, step, tag): R1 = (atom 0, x). */
+static void step_O_general(ref_ctx *c, uint32_t t, uint32_t tag)
+{
+    const int P = c->P;
+    const double bP = beta_P(c), hdt = 0.5 * c->dt;
+    for (int r = 0; r < c->R; ++r) {
+        double alpha = 1.0;
+        if (c->thermostat == 1) {
+            double K = 0.0, R1 = 0.0, S = 0.0;
+            for (int i = 0; i < c->N; ++i) {
+                double xi[3];
+                ref_normal3(c->seed, (uint32_t)i, (uint32_t)(r * P + 0), t, tag, xi);
+                for (int a = 0; a < 3; ++a) {
+                    double pm[1024];
+                    mom_to_modes(c, r, i, a, pm);
+                    K += pm[0] * pm[0] / (2.0 * c->mass[i] * mode_lam(c, 0));
+                    if (i == 0 && a == 0) R1 = xi[a]; else S += xi[a] * xi[a];
+                }
+            }
+            double c1 = exp(-c->gamma_fs * hdt);
+            if (K > 0.0) {
+                double a2 = c1 + (1.0 - c1) * (R1 * R1 + S) / (2.0 * bP * K) + 2.0 * R1 * sqrt(c1 * (1.0 - c1) / (2.0 * bP * K));
+                double sgn = (R1 + sqrt(2.0 * bP * K * c1 / (1.0 - c1)) >= 0.0) ? 1.0 : -1.0;
+                alpha = sgn * sqrt(a2 > 0.0 ? a2 : 0.0);
+            }
+        }
+#pragma omp parallel for schedule(static)
+        for (int i = 0; i < c->N; ++i) {
+            for (int a = 0; a < 3; ++a) {
+                double pm[1024];
+                mom_to_modes(c, r, i, a, pm);
+                for (int k = 0; k < P; ++k) {
+                    if (k == 0 && c->thermostat == 1) { pm[0] *= alpha; continue; }
+                    double gam = mode_gamma(c, k);
+                    double c1 = exp(-gam * hdt), c2 = sqrt(1.0 - c1 * c1);
+                    double xi[3];
+                    ref_normal3(c->seed, (uint32_t)i, (uint32_t)(r * P + k), t, tag, xi);
+                    pm[k] = c1 * pm[k] + sqrt(c->mass[i] * mode_lam(c, k) / bP) * c2 * xi[a];
+                }
+                mom_from_modes(c, r, i, a, pm);
+            }
+        }
+    }
+}
+
+/* B(dt/2) for the primitive variant: physical force plus the explicit ring springs -m w_P^2 (2 q_j - q_{j-1} - q_{j+1}) */
+static void step_B_primitive(ref_ctx *c)
+{
+    const int P = c->P;
+    const double hdt = 0.5 * c->dt, wP = P * KB_EV * c->T / HBAR_EVFS;
+    for (int r = 0; r < c->R; ++r)
+        for (int i = 0; i < c->N; ++i)
+            for (int a = 0; a < 3; ++a)
+                for (int j = 0; j < P; ++j) {
+                    double qj = c->q[idx4(c, r, j, i, a)];
+                    double qm = c->q[idx4(c, r, (j + P - 1) % P, i, a)], qp = c->q[idx4(c, r, (j + 1) % P, i, a)];
+                    double fs = -c->mass[i] * wP * wP * ((qj - qm) + (qj - qp));
+                    c->p[idx4(c, r, j, i, a)] += hdt * (c->F[idx4(c, r, j, i, a)] + fs);
+                }
+}
+
+/* A(dt): exact propagation of every mode under its own free-ring Hamiltonian p^2/(2 m lam) + 1/2 m lam w^2 u^2 */
+static void step_A_general(ref_ctx *c)
+{
+    const int P = c->P;
+    const double dt = c->dt;
+#pragma omp parallel for collapse(2) schedule(static)
+    for (int r = 0; r < c->R; ++r)
+        for (int i = 0; i < c->N; ++i)
+            for (int a = 0; a < 3; ++a) {
+                double qb[1024], um[1024], pm[1024];
+                col_get(c, c->q, r, i, a, qb);
+                if (c->transform == 1) stage_fwd(qb, um, P); else memcpy(um, qb, sizeof(double) * P);
+                mom_to_modes(c, r, i, a, pm);
+                for (int k = 0; k < P; ++k) {
+                    double mu = c->mass[i] * mode_lam(c, k), w = mode_omega(c, k);
+                    if (w == 0.0) {
+                        um[k] = um[k] + dt * pm[k] / mu;
+                    } else {
+                        double cs = cos(w * dt), sn = sin(w * dt);
+                        double pn = cs * pm[k] - mu * w * sn * um[k];
+                        double un = sn / (mu * w) * pm[k] + cs * um[k];
+                        pm[k] = pn; um[k] = un;
+                    }
+                }
+                if (c->transform == 1) stage_inv(um, qb, P); else memcpy(qb, um, sizeof(double) * P);
+                col_put(c, c->q, r, i, a, qb);
+                mom_from_modes(c, r, i, a, pm);
+            }
+}
+
+/* N5 in the chosen representation: mode momenta ~ N(0, m lam_k / beta_P), tag 2 */
+static void init_momenta_general(ref_ctx *c)
+{
+    const double bP = beta_P(c);
+    for (int r = 0; r < c->R; ++r)
+        for (int i = 0; i < c->N; ++i) {
+            double pm[3][1024];
+            for (int k = 0; k < c->P; ++k) {
+                double xi[3];
+                ref_normal3(c->seed, (uint32_t)i, (uint32_t)(r * c->P + k), 0u, 2u, xi);
+                for (int a = 0; a < 3; ++a) pm[a][k] = sqrt(c->mass[i] * mode_lam(c, k) / bP) * xi[a];
+            }
+            for (int a = 0; a < 3; ++a) mom_from_modes(c, r, i, a, pm[a]);
+        }
+}
+
+/* Choose the integrator variant; to be called before the first step (it redraws the initial momenta, N5). */
+int ref_set_integrator(ref_ctx *c, int transform, int thermostat)
+{
+    if (!c || transform < 0 || transform > 2 || thermostat < 0 || thermostat > 1 || c->step != 0) return -1;
+    if (thermostat == 1 && transform == 2) return -1; /* PILE-G needs a free (centroid-like) mode */
+    c->transform = transform; c->thermostat = thermostat;
+    init_momenta_general(c);
+    return 0;
+}
+
 int ref_step(ref_ctx *c, int n)
 {
     if (!c || n < 0) return -1;
@@ -512,13 +727,23 @@ int ref_step(ref_ctx *c, int n)
     if (rc) return rc;
     for (int s = 0; s < n; ++s) {
         uint32_t t = (uint32_t)c->step;
-        if (c->gamma_fs >= 0.0) step_O(c, t, 0u);
-        step_B(c);
-        step_A(c);
-        rc = compute_forces(c);
-        if (rc) return rc;
-        step_B(c);
-        if (c->gamma_fs >= 0.0) step_O(c, t, 1u);
+        if (c->transform == 0 && c->thermostat == 0) { /* N3: normal modes + PILE-L */
+            if (c->gamma_fs >= 0.0) step_O(c, t, 0u);
+            step_B(c);
+            step_A(c);
+            rc = compute_forces(c);
+            if (rc) return rc;
+            step_B(c);
+            if (c->gamma_fs >= 0.0) step_O(c, t, 1u);
+        } else { /* same O B A [forces] B O splitting, other representation / thermostat (8(f)4) */
+            if (c->gamma_fs >= 0.0) step_O_general(c, t, 0u);
+            if (c->transform == 2) step_B_primitive(c); else step_B(c);
+            step_A_general(c);
+            rc = compute_forces(c);
+            if (rc) return rc;
+            if (c->transform == 2) step_B_primitive(c); else step_B(c);
+            if (c->gamma_fs >= 0.0) step_O_general(c, t, 1u);
+        }
         c->step += 1;
     }
     return 0;
@@ -717,7 +942,9 @@ int ref_estimators(ref_ctx *c, ref_estimators_t *out)
             for (int k = 0; k < P; ++k)
                 for (int a = 0; a < 3; ++a) {
                     qbar[a] += c->q[idx4(c, r, k, i, a)];
-                    pc[a] += c->C[k * P + 0] * c->p[idx4(c, r, k, i, a)];
+                    /* momentum of the free mode: p~_0 = sum_j p_j / sqrt(P) (normal modes; same normalisation for primitive),
+                       p_u0 = sum_j p_j (staging, whose free mode has mass m instead of the ring's P m / P) */
+                    pc[a] += (c->transform == 1 ? 1.0 : c->C[k * P + 0]) * c->p[idx4(c, r, k, i, a)];
                 }
             for (int a = 0; a < 3; ++a) qbar[a] /= P;
             for (int k = 0; k < P; ++k) {
@@ -741,6 +968,21 @@ int ref_estimators(ref_ctx *c, ref_estimators_t *out)
         out[r].t_centroid = tc / (3.0 * N * KB_EV * P);
     }
     return 0;
+}
+
+/* test access to the staging maps of one column (P values each) */
+void ref_stage_fwd(const double *q, double *u, int P) { stage_fwd(q, u, P); }
+void ref_stage_inv(const double *u, double *q, int P) { stage_inv(u, q, P); }
+void ref_stage_force(const double *fq, double *fu, int P) { stage_force(fq, fu, P); }
+void ref_stage_mom_to_bead(const double *pu, double *pq, int P) { stage_mom_to_bead(pu, pq, P); }
+
+void ref_set_num_threads(int n)
+{
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
 }
 
 int ref_num_threads(void)
