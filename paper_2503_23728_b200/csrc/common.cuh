@@ -15,7 +15,6 @@
 
 #define PIMD_MAX_P 256
 #define PIMD_MAX_NBR 512               // neighbours per atom the fill kernel can sort
-#define PIMD_MAX_PART 1024             // row ranges (CTAs of the persistent pair kernels)
 
 // device error word bits
 #define PIMD_FLAG_PAIRS 1
@@ -56,9 +55,6 @@ struct NlistDev {
     int *col;                          // [pair_cap] local atom index j
     int *pair_row;                     // [pair_cap] global row i
     int64_t pair_cap;
-    int pad16;                         // 1: every row padded to a multiple of 16 pair slots (col = -1 in the padding); tcgen05 path
-    int *part;                         // [n_part + 1] row ranges of about equal slot counts, one per CTA of the pair kernels (or null)
-    int n_part;
 };
 
 struct pimd_ctx {
@@ -96,9 +92,8 @@ struct pimd_ctx {
     float *xs0;                        // [S][H] W_s^0 Emb[s]
     float h_be1_half[128];             // HOST copy of b_e1 / 2 (passed to the pair kernels as kernel parameters)
     unsigned char *h1_img, *meta_img;  // [pair_cap/128 + 1] tile images kept between the pair passes of one evaluation (tc path)
-    uint16_t *XY;                      // [rows][2 H] bf16 (x | y = E x) gathered by the message pass (aliases xfeat)
-    CUtensorMap tmap_xy;               // XY as [rows][256 bf16], box 64 x 1, 128-byte swizzle: tile::gather4 lands in the UMMA operand layout
-    CUtensorMap tmap_g;                // G as [rows][128 x 32 bit], box = one row (head)
+    uint32_t *XE;                      // [rows][H] packed bf16 (x | E << 16) gathered by the pair kernels (aliases xfeat)
+    CUtensorMap tmap_xe, tmap_g;       // 2-D tensor maps [rows][128 x 32 bit] of XE and G for TMA tile::gather4 (four gathered rows per copy)
     float *nfeat, *xfeat, *mfeat, *Efeat, *Gfeat;   // [rows][H]
     float *carry_m;                    // [n_gran_m][2][H]
     float *carry_f;                    // [n_gran_f][2][4]
@@ -116,7 +111,7 @@ struct ProfScope {
     ProfScope(pimd_ctx *ctx, int kind) : c(ctx) { if (c->prof) pimd_prof_begin(c, kind); }
     ~ProfScope() { if (c->prof) pimd_prof_end(c); }
 };
-enum { ATTR_PAIR32 = 1, ATTR_NODE32 = 2, ATTR_PIPE = 4, ATTR_NODETC = 8, ATTR_MSGROW = 16, ATTR_NM = 256 /* << MODE */ };
+enum { ATTR_PAIR32 = 1, ATTR_NODE32 = 2, ATTR_PIPE = 4, ATTR_NODETC = 8, ATTR_NM = 256 /* << MODE */ };
 enum { PROF_NM = 0, PROF_NLIST = 1, PROF_PAIR = 2, PROF_NODE = 3, PROF_HEAD = 4, PROF_OTHER = 5 };
 
 void pimd_set_error(const char *fmt, ...);
@@ -137,7 +132,6 @@ int pimd_launch_nm_post(pimd_ctx *c, uint32_t t);
 int pimd_launch_simple_forces(pimd_ctx *c);          // kinds 1, 2
 int pimd_launch_estimators(pimd_ctx *c);
 int pimd_launch_nlist(pimd_ctx *c);
-int pimd_launch_nlist_export(pimd_ctx *c, int *d_row_ptr, int *d_col, int64_t col_capacity);   // compact CSR of the list just built
 int pimd_launch_gfn_forces(pimd_ctx *c);
 int pimd_launch_copy_forces_f32(pimd_ctx *c, float *d_out);
 size_t pimd_gfn_smem_bytes(int K, int H);

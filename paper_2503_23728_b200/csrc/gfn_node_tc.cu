@@ -15,9 +15,9 @@
 // a single product, because x is gathered as bf16 by the message pass anyway.  The tensor pipe has the time (the kernel is
 // bound by its HBM reads and writes); shared memory does not hold ten 32 KB weight images, so the weight images stream
 // from L2 through a ring of 16 KB slots (TMA bulk copies, one producer warp), 18 (20 in the last layer) slots per tile.
-// The message pass (gfn_msg_row.cu) gathers, per pair slot, the row [x_j | y_j] with y_j = E_j x_j (channel-wise) as the A operand
-// of its row contraction: that table is written here as bf16, 512 B per atom (XY[row][0..127] = x, [128..255] = y; y is the fp32
-// product rounded once).  G stays fp32: G_i + G_j enters the force readout directly, with no averaging over neighbours behind it.
+// The pair kernels gather x_j, E_j per directed pair in the message passes: that copy is written as packed bf16
+// (XE[row][c] = x | E << 16) so that one 32-bit load serves both and the L2 gather traffic halves.  G stays fp32:
+// G_i + G_j enters the force readout directly, with no averaging over neighbours behind it.
 // SiLU(x) = h tanh(h) + h with h = x/2: the 1/2 is folded (exactly) into the W_vn, W_vm images and b_v1.
 #include "common.cuh"
 #include "tc_ptx.cuh"
@@ -38,12 +38,13 @@ constexpr int SEQ_MID = 18, SEQ_LAST = 20, IMG_PER_LAYER = 20;
 
 struct Args {
     int64_t rows;
-    int N, last, n_tiles;
+    int N, last, gran_m, n_tiles;
+    const int *row_ptr;
     const uint16_t *Wimg;          // this layer's IMG_PER_LAYER half-images, SLOT bytes each
     const float *bv1, *bv2, *ba;
     float *n, *E;
-    const float *m;                // [rows][H] messages of this layer (whole rows: the row contraction leaves no partial sums)
-    uint16_t *XY;                  // [rows][2 H] bf16: x | y = E x
+    const float *m, *carry_m;
+    uint32_t *XE;
     float *G;
 };
 
@@ -137,6 +138,7 @@ __global__ void __launch_bounds__(NTH, 1) node_tc_kernel(const __grid_constant__
     uint64_t *bar_full = (uint64_t *)(S + OFF_BAR), *bar_empty = bar_full + NS, *mbar_mma = bar_empty + NS;
     uint32_t *tmem_slot = (uint32_t *)(mbar_mma + 1);
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int n_pairs = a.row_ptr[a.rows];
     const int n_seq = a.last ? SEQ_LAST : SEQ_MID;
 
     if (tid == 0) {
@@ -177,7 +179,9 @@ __global__ void __launch_bounds__(NTH, 1) node_tc_kernel(const __grid_constant__
 
     for (int tile = blockIdx.x; tile < a.n_tiles; tile += gridDim.x) {
         const int64_t row0 = (int64_t)tile * TR;
-        // ---- operands n, m (fp32 in HBM) -> bf16 hi/lo swizzled tiles
+        // ---- operands n, m (fp32 in HBM) -> bf16 hi/lo swizzled tiles; m: one warp per row, coalesced 512-byte reads.
+        // m_i is assembled in fixed order from the direct row or the carry slots (tail slot of the first granule, head
+        // slots of the rest).  All loads of four rows are issued before the first use: the phase is latency-bound.
         {
             // n: the masters are tile-blocked ([c / 4][row][4 floats]), so with thread = row a warp reads 512 contiguous bytes
             // per instruction; eight loads in flight per thread (columns cgrp * 32 .. + 31), issued before everything else
@@ -191,16 +195,49 @@ __global__ void __launch_bounds__(NTH, 1) node_tc_kernel(const __grid_constant__
 #pragma unroll
                 for (int i = 0; i < 8; ++i) store_operand4(A0h, A0l, nr, cgrp * 32 + i * 4, nv8[i]);
             }
-            // m: one warp per row, coalesced 512-byte reads; all eight loads of a warp are issued before the first use
             const int k = lane * 4, wrow = tid >> 5;
-            float4 mv[8];
+            int rs[8], re[8];
 #pragma unroll
             for (int it = 0; it < 8; ++it) {
                 const int64_t row = row0 + wrow + it * 16;
-                mv[it] = (row < a.rows) ? __ldg((const float4 *)(a.m + (size_t)row * H + k)) : make_float4(0.f, 0.f, 0.f, 0.f);
+                const bool ok = row < a.rows && n_pairs > 0;
+                rs[it] = ok ? __ldg(a.row_ptr + row) : 0;
+                re[it] = ok ? __ldg(a.row_ptr + row + 1) : 0;
             }
 #pragma unroll
-            for (int it = 0; it < 8; ++it) store_operand4(A1h, A1l, wrow + it * 16, k, mv[it]);
+            for (int it0 = 0; it0 < 8; it0 += 4) {
+                float4 pc[4][4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const int it = it0 + j;
+                    const int64_t row = row0 + wrow + it * 16;
+                    const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
+                    pc[j][0] = pc[j][1] = pc[j][2] = pc[j][3] = z;
+                    if (re[it] > rs[it]) {       // warp-uniform
+                        const int g0 = rs[it] / a.gran_m, g1 = (re[it] - 1) / a.gran_m;
+                        if (g0 == g1) pc[j][0] = __ldg((const float4 *)(a.m + (size_t)row * H + k));
+                        else pc[j][0] = __ldg((const float4 *)(a.carry_m + ((size_t)g0 * 2 + 1) * H + k));
+#pragma unroll
+                        for (int t = 1; t < 4; ++t)
+                            if (g0 + t <= g1) pc[j][t] = __ldg((const float4 *)(a.carry_m + ((size_t)(g0 + t) * 2) * H + k));
+                    }
+                }
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const int it = it0 + j, rr = wrow + it * 16;
+                    float4 mv = pc[j][0];
+#pragma unroll
+                    for (int t = 1; t < 4; ++t) { mv.x += pc[j][t].x; mv.y += pc[j][t].y; mv.z += pc[j][t].z; mv.w += pc[j][t].w; }
+                    if (re[it] > rs[it]) {       // rows with more than four granules (very long rows): the rest, in order
+                        const int g0 = rs[it] / a.gran_m, g1 = (re[it] - 1) / a.gran_m;
+                        for (int gg = g0 + 4; gg <= g1; ++gg) {
+                            const float4 t4 = __ldg((const float4 *)(a.carry_m + ((size_t)gg * 2) * H + k));
+                            mv.x += t4.x; mv.y += t4.y; mv.z += t4.z; mv.w += t4.w;
+                        }
+                    }
+                    store_operand4(A1h, A1l, rr, k, mv);
+                }
+            }
         }
         tc::fence_proxy_async_smem();
         tc::named_bar_sync(NB_COMPUTE, NTC);
@@ -281,7 +318,7 @@ __global__ void __launch_bounds__(NTH, 1) node_tc_kernel(const __grid_constant__
         tc::mbar_wait(mbar_mma, par);
         par ^= 1;
         tc::tc_fence_after_sync();
-        // ---- E <- E + D0 + b_a ; XY = (x | y = E x) bf16, or E -> A1 for G = W_f1 E
+        // ---- E <- E + D0 + b_a ; XE = (x, E) packed bf16, or E -> A1 for G = W_f1 E
 #pragma unroll
         for (int j = 0; j < 2; ++j) {
             const int c0 = g * 32 + j * 16;
@@ -304,30 +341,24 @@ __global__ void __launch_bounds__(NTH, 1) node_tc_kernel(const __grid_constant__
                 // A thread owns a row, so a direct store is 16 bytes per lane at a 512-byte stride (32 sectors per
                 // instruction).  The warp's 32 x 128-byte block goes through shared memory instead (the operand tiles
                 // are free now; 16-byte chunks XOR-swizzled by row & 7) and leaves as whole 128-byte lines below.
-                // staged row (128 B): chunks 0-3 = x of the warp's 32 columns, chunks 4-7 = y = E x of the same columns
                 unsigned char *xs = A0h + warp * 4096 + lane * 128;
 #pragma unroll
-                for (int e8 = 0; e8 < 2; ++e8) {
-                    const int o = e8 * 8;
-                    *(uint4 *)(xs + (((j * 2 + e8) ^ (lane & 7)) << 4)) =
-                        make_uint4(tc::pack_bf16(v[o], v[o + 1]), tc::pack_bf16(v[o + 2], v[o + 3]),
-                                   tc::pack_bf16(v[o + 4], v[o + 5]), tc::pack_bf16(v[o + 6], v[o + 7]));
-                    *(uint4 *)(xs + (((4 + j * 2 + e8) ^ (lane & 7)) << 4)) =
-                        make_uint4(tc::pack_bf16(ee[o] * v[o], ee[o + 1] * v[o + 1]), tc::pack_bf16(ee[o + 2] * v[o + 2], ee[o + 3] * v[o + 3]),
-                                   tc::pack_bf16(ee[o + 4] * v[o + 4], ee[o + 5] * v[o + 5]), tc::pack_bf16(ee[o + 6] * v[o + 6], ee[o + 7] * v[o + 7]));
-                }
+                for (int e4 = 0; e4 < 4; ++e4)
+                    *(uint4 *)(xs + (((j * 4 + e4) ^ (lane & 7)) << 4)) =
+                        make_uint4(tc::pack_bf16(v[e4 * 4], ee[e4 * 4]), tc::pack_bf16(v[e4 * 4 + 1], ee[e4 * 4 + 1]),
+                                   tc::pack_bf16(v[e4 * 4 + 2], ee[e4 * 4 + 2]), tc::pack_bf16(v[e4 * 4 + 3], ee[e4 * 4 + 3]));
             } else {
                 store_operand16(A1h, A1l, r, c0, ee);
             }
         }
-        if (!a.last) {             // the warp's XY block: 4 rows x (64 bytes of x + 64 bytes of y) per store instruction
+        if (!a.last) {             // the warp's XE block: 4 rows x 128 bytes per store instruction
             __syncwarp();
 #pragma unroll
             for (int it = 0; it < 8; ++it) {
                 const int rr = it * 4 + (lane >> 3), ch = lane & 7;
                 const uint4 w4 = *(const uint4 *)(A0h + warp * 4096 + rr * 128 + ((ch ^ (rr & 7)) << 4));
                 const int64_t orow = row0 + q * 32 + rr;
-                if (orow < a.rows) *(uint4 *)(a.XY + (size_t)orow * (2 * H) + (ch >> 2) * H + g * 32 + (ch & 3) * 8) = w4;
+                if (orow < a.rows) *(uint4 *)(a.XE + (size_t)orow * H + g * 32 + ch * 4) = w4;
             }
         }
         if (a.last) {
@@ -372,7 +403,7 @@ __global__ void __launch_bounds__(NTH, 1) node_tc_kernel(const __grid_constant__
 // layer-0 inputs: n = Emb[species], E = 0, x = W_s^0 n (one vector per species, formed on the host) -> XE
 __global__ void node_init_tc_kernel(int64_t rows, int N, const int *__restrict__ species, const float *__restrict__ Emb,
                                     const float *__restrict__ xs0, float *__restrict__ n, float *__restrict__ E,
-                                    uint16_t *__restrict__ XY)
+                                    uint32_t *__restrict__ XE)
 {
     const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;      // over the rows rounded up to whole tiles
     {   // tile-blocked masters: consecutive threads = consecutive rows of one 4-column group (16 contiguous bytes each)
@@ -386,13 +417,13 @@ __global__ void node_init_tc_kernel(int64_t rows, int N, const int *__restrict__
             *(float4 *)(E + o) = make_float4(0.f, 0.f, 0.f, 0.f);
         }
     }
-    // row-major XY (x | y = E x = 0 in layer 0): consecutive threads = consecutive 8-byte pieces of one 512-byte row
+    // row-major XE: consecutive threads = consecutive columns of one row
     if (idx >= rows * (H / 4)) return;
     const int64_t row = idx >> 5;
     const int c0 = (int)(idx & 31) * 4;
     const float4 xv = __ldg((const float4 *)(xs0 + (size_t)species[row % N] * H + c0));
-    *(uint2 *)(XY + (size_t)row * (2 * H) + c0) = make_uint2(tc::pack_bf16(xv.x, xv.y), tc::pack_bf16(xv.z, xv.w));
-    *(uint2 *)(XY + (size_t)row * (2 * H) + H + c0) = make_uint2(0u, 0u);
+    *(uint4 *)(XE + (size_t)row * H + c0) =
+        make_uint4(tc::pack_bf16(xv.x, 0.f), tc::pack_bf16(xv.y, 0.f), tc::pack_bf16(xv.z, 0.f), tc::pack_bf16(xv.w, 0.f));
 }
 
 int launch_node_tc(pimd_ctx *c, int mode, int layer)
@@ -401,19 +432,20 @@ int launch_node_tc(pimd_ctx *c, int mode, int layer)
     if (mode == 0) {
         const int64_t work = (c->rows + 127) / 128 * 128 * (H / 4);
         node_init_tc_kernel<<<(unsigned)((work + 255) / 256), 256, 0, c->stream>>>(c->rows, c->N, c->species, n.Emb, c->xs0,
-                                                                                 c->nfeat, c->Efeat, c->XY);
+                                                                                 c->nfeat, c->Efeat, c->XE);
         c->launches++;
         PIMD_CUDA_CHECK(cudaGetLastError());
         return 0;
     }
     const GfnLayerW &w = n.layer[layer];
     Args a;
-    a.rows = c->rows; a.N = c->N; a.last = (layer == n.L - 1);
+    a.rows = c->rows; a.N = c->N; a.last = (layer == n.L - 1); a.gran_m = c->gran_m;
     a.n_tiles = (int)((c->rows + TR - 1) / TR);
+    a.row_ptr = c->nl.row_ptr;
     a.Wimg = c->wimg_node + (size_t)layer * IMG_PER_LAYER * (SLOT / 2);
     a.bv1 = w.bv1; a.bv2 = w.bv2; a.ba = w.ba;
-    a.n = c->nfeat; a.E = c->Efeat; a.m = c->mfeat;
-    a.XY = c->XY; a.G = c->Gfeat;
+    a.n = c->nfeat; a.E = c->Efeat; a.m = c->mfeat; a.carry_m = c->carry_m;
+    a.XE = c->XE; a.G = c->Gfeat;
     const size_t smem = SMEM_BYTES + 1024;
     if (!(c->attr_done & ATTR_NODETC)) {
         PIMD_CUDA_CHECK(cudaFuncSetAttribute(node_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));

@@ -236,12 +236,11 @@ int launch_pair_t(pimd_ctx *c, const PairArgs &a, bool head)
 
 }  // namespace gfn
 namespace gfn_pipe { int launch_pair_pipe(pimd_ctx *c, bool head, bool first); }
-namespace gfn_row { int launch_msg_row(pimd_ctx *c, bool first); }
 namespace gfn {
 
 int launch_pair(pimd_ctx *c, int layer, bool head)
 {
-    if (c->use_tc) return head ? gfn_pipe::launch_pair_pipe(c, true, true) : gfn_row::launch_msg_row(c, layer == 0);   // layer 0: E = 0
+    if (c->use_tc) return gfn_pipe::launch_pair_pipe(c, head, layer == 0);   // layer 0 = first pair pass of this evaluation
     PairArgs a;
     a.N = c->N; a.periodic = c->periodic;
     for (int k = 0; k < 3; ++k) a.box[k] = c->box[k];

@@ -191,11 +191,7 @@ __device__ __forceinline__ void role_P(const PairArgs &a, unsigned char *S, uint
         float w = 0.f, ux = 0.f, uy = 0.f, uz = 0.f, dist = 0.f;
         int prev_row = -1;
         if (lane == 0 && (p & (GP - 1)) != 0 && pg - 1 < n_pairs) prev_row = __ldg(a.pair_row + pg - 1);
-        if (row >= 0 && cj < 0) {                 // padding slot of a row (pad16 lists): weight 0, any finite gathered row
-            jrow = row;
-            const int rs = __ldg(a.row_ptr + row), re = __ldg(a.row_ptr + row + 1);
-            kind = seg_kind(rs, re, pg & ~(int64_t)(GP - 1), GP);
-        } else if (row >= 0) {
+        if (row >= 0) {
             const int sys = row / a.N;
             jrow = sys * a.N + cj;
             const int rs = __ldg(a.row_ptr + row), re = __ldg(a.row_ptr + row + 1);
@@ -979,11 +975,11 @@ int launch_pair_pipe(pimd_ctx *c, bool head, bool first)
     a.W1img = c->wimg_e1; a.W2img = head ? c->wimg_fe : c->wimg_e2; a.Wf2img = c->wimg_wf2;
     for (int k = 0; k < H; ++k) a.b1h[k] = c->h_be1_half[k];
     a.b2 = head ? c->net.bfe : c->net.be2;
-    a.gsrc = (const void *)c->Gfeat;
+    a.gsrc = head ? (const void *)c->Gfeat : (const void *)c->XE;
     a.wf2 = c->net.wf2; a.bf2 = c->net.bf2;
     a.m_out = c->mfeat; a.carry_m = c->carry_m; a.Fraw = c->Fraw; a.carry_f = c->carry_f;
     a.h1_img = c->h1_img; a.meta_img = c->meta_img;
-    a.gmap = c->tmap_g;
+    a.gmap = head ? c->tmap_g : c->tmap_xe;
     const size_t smem = SMEM_BYTES + 1024;
     if (!(c->attr_done & ATTR_PIPE)) {
         PIMD_CUDA_CHECK(cudaFuncSetAttribute(pair_pipe_kernel<false, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));

@@ -279,15 +279,12 @@ __global__ void __launch_bounds__(COUNT_THREADS) count_cell_kernel(NlArgs a)
     }
 }
 
-// row_ptr: three-kernel exclusive scan over rows (1024 rows per block).  With pad16 (tcgen05 path) every row is padded to a
-// multiple of 16 pair slots: a row is then a whole number of K blocks of the row-aligned tensor-core contraction (gfn_msg_row.cu).
-__device__ __forceinline__ int padded(int n, int pad16) { return pad16 ? ((n + 15) & ~15) : n; }
-
+// row_ptr: three-kernel exclusive scan over rows (1024 rows per block)
 __global__ void __launch_bounds__(1024) scan_rows_local_kernel(NlArgs a)
 {
     __shared__ int tot;
     int64_t row = (int64_t)blockIdx.x * 1024 + threadIdx.x;
-    int v = (row < a.rows) ? padded(a.d.nnz[row], a.d.pad16) : 0;
+    int v = (row < a.rows) ? a.d.nnz[row] : 0;
     int ex = block_exclusive_scan(v, &tot);
     if (row < a.rows) a.d.row_ptr[row] = ex;
     if (threadIdx.x == 0) a.d.block_sums[blockIdx.x] = tot;
@@ -314,28 +311,10 @@ __global__ void __launch_bounds__(1024) scan_block_sums_kernel(NlArgs a, int nbl
     }
 }
 
-// adds the block offsets; with a partition table (tcgen05 path) it also cuts the rows into n_part contiguous ranges of about
-// equal slot counts: part[b] = first row whose first slot is at or beyond b * total / n_part (whole rows per CTA)
 __global__ void scan_rows_add_kernel(NlArgs a)
 {
     int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (row >= a.rows) return;
-    const int rp = a.d.row_ptr[row] + a.d.block_sums[row >> 10];
-    a.d.row_ptr[row] = rp;
-    if (!a.d.part) return;
-    const int G = a.d.n_part;
-    const long long total = a.d.row_ptr[a.rows];
-    if (row == 0) { a.d.part[0] = 0; a.d.part[G] = (int)a.rows; }
-    if (total == 0) { if (row == 0) for (int b = 1; b < G; ++b) a.d.part[b] = (int)a.rows; return; }
-    // boundaries b with rp_prev < target_b <= rp, target_b = floor(total b / G)  (row 0: 0 < target_b <= rp never holds, rp = 0)
-    const long long prev = (row == 0) ? -1 : (long long)rp - padded(a.d.nnz[row - 1], a.d.pad16);
-    int b = (int)(((prev + 1) * G + total - 1) / total);          // smallest b with total b / G >= prev + 1  (b >= 1 as prev >= 0)
-    if (b < 1) b = 1;
-    for (; b < G && (total * b) / G <= rp; ++b)
-        if ((total * b) / G > prev) a.d.part[b] = (int)row;
-    if (row == a.rows - 1) {                                      // boundaries beyond the last row's first slot
-        for (int bb = 1; bb < G; ++bb) if ((total * bb) / G > rp) a.d.part[bb] = (int)a.rows;
-    }
+    if (row < a.rows) a.d.row_ptr[row] += a.d.block_sums[row >> 10];
 }
 
 // CSR fill with ascending rows and no sort: the row's hits set bits in a per-warp bitmask over the atoms of the bead-system
@@ -375,31 +354,14 @@ __global__ void __launch_bounds__(256) fill_bitmask_kernel(NlArgs a, int nw)
             bits &= bits - 1;
         }
     }
-    const int np = padded(n, a.d.pad16);
-    for (int e = lane; e < np; e += 32) {                                   // coalesced, outside the divergent loop
-        a.d.pair_row[base + e] = (int)row;
-        if (e >= n) a.d.col[base + e] = -1;                                 // padding slots: no neighbour (weight 0 downstream)
-    }
-}
-
-// pimd_nlist export of a padded list: the compact CSR (row_ptr_out = exclusive scan of the true counts, done by the scan
-// kernels into the caller's buffer) and the columns without the padding slots.  One warp per row.
-__global__ void __launch_bounds__(256) compact_cols_kernel(NlArgs a, const int *__restrict__ row_ptr_out, int *__restrict__ col_out,
-                                                           int64_t col_capacity)
-{
-    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int64_t row = (int64_t)blockIdx.x * 8 + w;
-    if (row >= a.rows) return;
-    if (row_ptr_out[a.rows] > col_capacity) return;
-    const int n = a.d.nnz[row];
-    const int64_t src = a.d.row_ptr[row], dst = row_ptr_out[row];
-    for (int e = lane; e < n; e += 32) col_out[dst + e] = a.d.col[src + e];
+    for (int e = lane; e < n; e += 32) a.d.pair_row[base + e] = (int)row;   // coalesced, outside the divergent loop
 }
 
 }  // namespace
 
-static void fill_args(pimd_ctx *c, NlArgs &a)
+int pimd_launch_nlist(pimd_ctx *c)
 {
+    NlArgs a;
     a.N = c->N; a.nsys = c->R * c->P; a.periodic = c->periodic; a.rows = c->rows;
     for (int k = 0; k < 3; ++k) { a.box[k] = c->box[k]; a.nc[k] = c->nl.ncell[k]; }
     a.rc2 = (double)c->net.r_cut * (double)c->net.r_cut;
@@ -407,12 +369,6 @@ static void fill_args(pimd_ctx *c, NlArgs &a)
     a.rc2_lo = (float)(a.rc2 * (1.0 - 1e-3)); a.rc2_hi = (float)(a.rc2 * (1.0 + 1e-3));
     for (int k = 0; k < 3; ++k) { a.boxf[k] = (float)c->box[k]; a.inv_boxf[k] = c->periodic ? (float)(1.0 / c->box[k]) : 0.f; }
     a.hit_stride = c->nl.hit_stride;
-}
-
-int pimd_launch_nlist(pimd_ctx *c)
-{
-    NlArgs a;
-    fill_args(c, a);
     const int64_t rows = c->rows;
     const unsigned gthr = (unsigned)((rows + 255) / 256), gwarp = (unsigned)((rows + 7) / 8);
     const int nblk = (int)((rows + 1023) / 1024);
@@ -429,26 +385,6 @@ int pimd_launch_nlist(pimd_ctx *c)
     const int nw = (c->N + 31) / 32;
     fill_bitmask_kernel<<<gwarp, 256, (size_t)8 * nw * sizeof(unsigned), c->stream>>>(a, nw);
     c->launches += 8;
-    PIMD_CUDA_CHECK(cudaGetLastError());
-    return 0;
-}
-
-// compact CSR for pimd_nlist: row_ptr = exclusive scan of the true counts (the scan kernels, aimed at the caller's buffer),
-// columns copied without the padding slots.  For an unpadded list this is a plain copy through the same kernels.
-int pimd_launch_nlist_export(pimd_ctx *c, int *d_row_ptr, int *d_col, int64_t col_capacity)
-{
-    NlArgs a;
-    fill_args(c, a);
-    NlArgs b = a;                      // scan of the true counts into the caller's row_ptr; no partition table
-    b.d.pad16 = 0; b.d.part = nullptr; b.d.row_ptr = d_row_ptr;
-    const int64_t rows = c->rows;
-    const unsigned gthr = (unsigned)((rows + 255) / 256), gwarp = (unsigned)((rows + 7) / 8);
-    const int nblk = (int)((rows + 1023) / 1024);
-    scan_rows_local_kernel<<<nblk, 1024, 0, c->stream>>>(b);
-    scan_block_sums_kernel<<<1, 1024, 0, c->stream>>>(b, nblk);
-    scan_rows_add_kernel<<<gthr, 256, 0, c->stream>>>(b);
-    compact_cols_kernel<<<gwarp, 256, 0, c->stream>>>(a, d_row_ptr, d_col, col_capacity);
-    c->launches += 4;
     PIMD_CUDA_CHECK(cudaGetLastError());
     return 0;
 }

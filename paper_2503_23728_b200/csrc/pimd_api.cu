@@ -60,7 +60,7 @@ namespace {
 
 struct Layout {
     size_t q, p, F, species, mass, C, CT, omega, err, est_partial, est_out;
-    size_t cell_id, cell_count, cell_start, cell_cursor, sorted_atom, sorted_q, nnz, hits, row_ptr, block_sums, col, pair_row, part;
+    size_t cell_id, cell_count, cell_start, cell_cursor, sorted_atom, sorted_q, nnz, hits, row_ptr, block_sums, col, pair_row;
     size_t wimg, wimg_node, xs0, h1_img, meta_img, weights, nfeat, xfeat, mfeat, Efeat, Gfeat, carry_m, carry_f, Fraw;
     size_t total;
     int ncell[3], nct;
@@ -133,7 +133,6 @@ int compute_layout(int N, int R, int P, const double box[3], const pimd_net_para
         if (cap_row > N - 1) cap_row = N - 1;
         if (cap_row > PIMD_MAX_NBR) cap_row = PIMD_MAX_NBR;
         if (cap_row < 1) cap_row = 1;
-        if (net->gemm_dtype == 1 && net->n_rbf == 64 && H == 128) cap_row = (cap_row + 15) / 16 * 16;   // rows padded to whole K blocks (pad16)
         L->pair_cap = (rows * cap_row + 255) / 256 * 256;
         if (L->pair_cap > 2000000000LL) { pimd_set_error("pair capacity exceeds int32 range"); return PIMD_ERR_ARG; }
         // pairs per message-reduction granule: TP * H / NT in the fp32 kernel, a quarter tile in the tcgen05 pipeline
@@ -170,7 +169,6 @@ int compute_layout(int N, int R, int P, const double box[3], const pimd_net_para
         L->block_sums = take(cur, sizeof(int) * ((rows + 1023) / 1024 + 1));
         L->col = take(cur, sizeof(int) * L->pair_cap);
         L->pair_row = take(cur, sizeof(int) * L->pair_cap);
-        L->part = take(cur, sizeof(int) * (PIMD_MAX_PART + 1));
         L->weights = take(cur, sizeof(float) * L->n_wfloats);
         L->wimg = take(cur, 5 * 16384 + 4096);   // bf16 UMMA images: W_e1 (16 KB), W_e2 (32 KB), W_f1 W_e2 (32 KB)
         L->wimg_node = take(cur, (size_t)(net->n_layers > 0 ? net->n_layers : 1) * 20 * 16384);   // 20 half-images (16 KB) per layer: gfn_node_tc.cu
@@ -473,7 +471,6 @@ extern "C" int pimd_create(pimd_ctx **out, int n_atoms, int n_replicas, const in
         nl.sorted_atom = (int *)(ws + L.sorted_atom); nl.sorted_q = (double *)(ws + L.sorted_q);
         nl.nnz = (int *)(ws + L.nnz); nl.hits = (int *)(ws + L.hits); nl.hit_stride = L.hit_stride; nl.row_ptr = (int *)(ws + L.row_ptr); nl.block_sums = (int *)(ws + L.block_sums);
         nl.col = (int *)(ws + L.col); nl.pair_row = (int *)(ws + L.pair_row); nl.pair_cap = L.pair_cap;
-        nl.pad16 = 0; nl.part = nullptr; nl.n_part = 0;
         c->weights_dev = (float *)(ws + L.weights);
         c->nfeat = (float *)(ws + L.nfeat); c->xfeat = (float *)(ws + L.xfeat); c->mfeat = (float *)(ws + L.mfeat);
         c->Efeat = (float *)(ws + L.Efeat); c->Gfeat = (float *)(ws + L.Gfeat);
@@ -507,10 +504,8 @@ extern "C" int pimd_create(pimd_ctx **out, int n_atoms, int n_replicas, const in
             CREATE_CHECK(cudaMemcpyAsync(c->wimg_e1, wimg.data(), sizeof(uint16_t) * wimg.size(), cudaMemcpyHostToDevice, st));
             // atom-wise layers: five images per layer; SiLU's 1/2 folded into W_vn, W_vm
             c->wimg_node = (uint16_t *)(ws + L.wimg_node); c->xs0 = (float *)(ws + L.xs0);
-            c->XY = (uint16_t *)c->xfeat;
-            // rows padded to whole K blocks of 16 slots, and a row partition with one range per CTA of the pair kernels
-            nl.pad16 = 1; nl.part = (int *)(ws + L.part); nl.n_part = c->num_sms < PIMD_MAX_PART ? c->num_sms : PIMD_MAX_PART;
-            {   // tensor maps of the two gathered tables (rows of 512 B; used with tile::gather4)
+            c->XE = (uint32_t *)c->xfeat;
+            {   // tensor maps of the two gathered tables (rows of 512 B; box = one row; used with tile::gather4)
                 typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
                                               const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
                                               CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -518,21 +513,16 @@ extern "C" int pimd_create(pimd_ctx **out, int n_atoms, int n_replicas, const in
                 cudaDriverEntryPointQueryResult qres;
                 CREATE_CHECK(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
                 if (!fn || qres != cudaDriverEntryPointSuccess) { pimd_set_error("cuTensorMapEncodeTiled is not available in this driver"); delete c; return PIMD_ERR_CUDA; }
+                const cuuint64_t gdim[2] = {128, (cuuint64_t)c->rows};
                 const cuuint64_t gstr[1] = {512};
-                const cuuint32_t estr[2] = {1, 1};
-                // G: fp32 rows, box = one whole row, no swizzle (read by threads)
-                const cuuint64_t gdim_g[2] = {128, (cuuint64_t)c->rows};
-                const cuuint32_t box_g[2] = {128, 1};
-                CUresult rc = ((encode_fn)fn)(&c->tmap_g, CU_TENSOR_MAP_DATA_TYPE_UINT32, 2, c->Gfeat, gdim_g, gstr, box_g, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                                              CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-                // XY: bf16 rows (x | y), box = 64 columns (128 B) of one row, 128-byte swizzle: four gathered rows form half of an
-                // 8-row group of an MN-major UMMA operand (gfn_msg_row.cu)
-                const cuuint64_t gdim_xy[2] = {256, (cuuint64_t)c->rows};
-                const cuuint32_t box_xy[2] = {64, 1};
-                if (rc == CUDA_SUCCESS)
-                    rc = ((encode_fn)fn)(&c->tmap_xy, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, c->XY, gdim_xy, gstr, box_xy, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                                         CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-                if (rc != CUDA_SUCCESS) { pimd_set_error("cuTensorMapEncodeTiled failed (%d)", (int)rc); delete c; return PIMD_ERR_CUDA; }
+                const cuuint32_t box[2] = {128, 1}, estr[2] = {1, 1};
+                void *bases[2] = {c->XE, c->Gfeat};
+                CUtensorMap *maps[2] = {&c->tmap_xe, &c->tmap_g};
+                for (int t = 0; t < 2; ++t) {
+                    const CUresult rc = ((encode_fn)fn)(maps[t], CU_TENSOR_MAP_DATA_TYPE_UINT32, 2, bases[t], gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                                        CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                    if (rc != CUDA_SUCCESS) { pimd_set_error("cuTensorMapEncodeTiled failed (%d)", (int)rc); delete c; return PIMD_ERR_CUDA; }
+                }
             }
             c->h1_img = (unsigned char *)(ws + L.h1_img); c->meta_img = (unsigned char *)(ws + L.meta_img);
             for (int k = 0; k < H && k < 128; ++k) c->h_be1_half[k] = 0.5f * raw.be1[k];
@@ -700,12 +690,14 @@ extern "C" int pimd_nlist(pimd_ctx *c, int32_t *d_row_ptr, int32_t *d_col, int64
     int rc;
     if ((rc = enter(c))) return rc;
     if ((rc = pimd_launch_nlist(c))) return rc;
-    if ((rc = pimd_launch_nlist_export(c, d_row_ptr, d_col, col_capacity))) return rc;   // compact CSR (internal rows may be padded)
     int n = 0;
-    PIMD_CUDA_CHECK(cudaMemcpyAsync(&n, d_row_ptr + c->rows, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    PIMD_CUDA_CHECK(cudaMemcpyAsync(&n, c->nl.row_ptr + c->rows, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
     if ((rc = check_device_error(c))) return rc;
     *h_n_pairs = n;
     if (n > col_capacity) { pimd_set_error("col_capacity %lld < %d pairs", (long long)col_capacity, n); return PIMD_ERR_PAIRS; }
+    PIMD_CUDA_CHECK(cudaMemcpyAsync(d_row_ptr, c->nl.row_ptr, sizeof(int) * (c->rows + 1), cudaMemcpyDeviceToDevice, c->stream));
+    PIMD_CUDA_CHECK(cudaMemcpyAsync(d_col, c->nl.col, sizeof(int) * (size_t)n, cudaMemcpyDeviceToDevice, c->stream));
+    PIMD_CUDA_CHECK(cudaStreamSynchronize(c->stream));
     return 0;
 }
 
