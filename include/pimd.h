@@ -100,6 +100,20 @@ int pimd_create(pimd_ctx **out, int n_atoms, int n_replicas, const int32_t *spec
                 double gamma_centroid_per_ps, uint64_t seed, const pimd_net_params *net, void *d_workspace,
                 size_t workspace_bytes, void *cuda_stream);
 
+/* Integrator variant, to be chosen before the first step (the initial momenta are redrawn in the chosen representation, S:N5).
+ *   transform   0 normal modes (default; S:N2)
+ *               1 staging transformation ("the normal mode or staging transformation is employed to decouple the
+ *                 evolution of individual beads"): u_0 = q_0, u_j = q_j - (j q_{j+1} + q_0)/(j+1); staging masses m (j+1)/j,
+ *                 every staging mode j >= 1 is propagated exactly at w_P, u_0 moves freely
+ *               2 primitive ("inter-bead harmonic coupling potentials are incorporated as pluggable energy terms"):
+ *                 no transformation; the ring springs are explicit forces in the B half-steps, beads fly freely in A
+ *   thermostat  0 PILE-L: Langevin on every mode, friction gamma on the free mode, 2 w_k on the others
+ *                 (with transform 2: white-noise Langevin with gamma on every bead)
+ *               1 PILE-G: the free mode of all atoms of a replica is rescaled by one stochastic factor (global velocity
+ *                 rescaling with time constant 1/gamma); the other modes as PILE-L.  Not available with transform 2.
+ * Returns PIMD_ERR_ARG after the first step or for an unsupported combination.  Synchronises. */
+int pimd_set_integrator(pimd_ctx *ctx, int transform, int thermostat);
+
 /* n steps of O(dt/2) B(dt/2) A(dt) [neighbour list, forces] B(dt/2) O(dt/2) (S:N3).
  * Asynchronous on the stream; no host synchronisation. */
 int pimd_step(pimd_ctx *ctx, int n);

@@ -673,7 +673,9 @@ static void step_A_general(ref_ctx *c)
             for (int a = 0; a < 3; ++a) {
                 double qb[1024], um[1024], pm[1024];
                 col_get(c, c->q, r, i, a, qb);
-                if (c->transform == 1) stage_fwd(qb, um, P); else memcpy(um, qb, sizeof(double) * P);
+                if (c->transform == 0) to_modes(c, c->q, r, i, a, um);
+                else if (c->transform == 1) stage_fwd(qb, um, P);
+                else memcpy(um, qb, sizeof(double) * P);
                 mom_to_modes(c, r, i, a, pm);
                 for (int k = 0; k < P; ++k) {
                     double mu = c->mass[i] * mode_lam(c, k), w = mode_omega(c, k);
@@ -686,8 +688,11 @@ static void step_A_general(ref_ctx *c)
                         pm[k] = pn; um[k] = un;
                     }
                 }
-                if (c->transform == 1) stage_inv(um, qb, P); else memcpy(qb, um, sizeof(double) * P);
-                col_put(c, c->q, r, i, a, qb);
+                if (c->transform == 0) from_modes(c, um, r, i, a, c->q);
+                else {
+                    if (c->transform == 1) stage_inv(um, qb, P); else memcpy(qb, um, sizeof(double) * P);
+                    col_put(c, c->q, r, i, a, qb);
+                }
                 mom_from_modes(c, r, i, a, pm);
             }
 }

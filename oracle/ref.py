@@ -52,6 +52,10 @@ def lib():
         L.ref_destroy.argtypes = [C.c_void_p]
         L.ref_destroy.restype = None
         L.ref_step.argtypes = [C.c_void_p, C.c_int]
+        L.ref_set_integrator.argtypes = [C.c_void_p, C.c_int, C.c_int]
+        for f in (L.ref_stage_fwd, L.ref_stage_inv, L.ref_stage_force, L.ref_stage_mom_to_bead):
+            f.argtypes = [dp, dp, C.c_int]
+            f.restype = None
         L.ref_forces.argtypes = [C.c_void_p, dp]
         L.ref_force_gross.argtypes = [C.c_void_p, dp]
         L.ref_get_state.argtypes = [C.c_void_p, dp, dp, C.POINTER(C.c_int64)]
@@ -67,6 +71,15 @@ def lib():
 
 def _dp(a):
     return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def stage_map(name, v):
+    """One of the oracle's four staging maps ('fwd' q->u, 'inv' u->q, 'force' f_q->f_u (also p_q->p_u), 'mom_to_bead' p_u->p_q)
+    applied to a vector of P bead values."""
+    v = np.ascontiguousarray(v, dtype=np.float64)
+    out = np.zeros_like(v)
+    getattr(lib(), "ref_stage_" + name)(_dp(v), _dp(out), int(v.size))
+    return out
 
 
 def _ip(a):
@@ -181,6 +194,15 @@ class RefPIMD:
 
     def __del__(self):
         self.close()
+
+    TRANSFORMS = {"normal_modes": 0, "staging": 1, "primitive": 2}
+    THERMOSTATS = {"pile_l": 0, "pile_g": 1}
+
+    def set_integrator(self, transform="normal_modes", thermostat="pile_l"):
+        """SURVEY 8(f)4 variants; before the first step (redraws the initial momenta in the chosen representation)."""
+        rc = lib().ref_set_integrator(self._h, self.TRANSFORMS[transform], self.THERMOSTATS[thermostat])
+        if rc != 0:
+            raise RuntimeError(f"ref_set_integrator failed: {rc}")
 
     def step(self, n=1):
         rc = lib().ref_step(self._h, int(n))

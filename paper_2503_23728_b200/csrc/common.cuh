@@ -77,8 +77,12 @@ struct pimd_ctx {
     double *q, *p, *F;                 // [rows][3]
     int *species;                      // [N]
     double *mass;                      // [N] internal units
-    double *Cmat, *CmatT;              // [P][P]: C[j*P+k]; CT[k*P+j]
-    double *omega_k;                   // [P]
+    int transform, thermostat;         // integrator variant (pimd_set_integrator): 0 normal modes | 1 staging | 2 primitive; 0 PILE-L | 1 PILE-G
+    double *Cmat, *CmatT;              // [P][P]: C[j*P+k]; CT[k*P+j]   (normal-mode matrix, S:N2)
+    double *Tq_fwd, *Tq_inv, *Tp_fwd, *Tp_inv;   // [P][P] bead <-> mode maps of coordinates and momenta in use
+    double *Tstage;                    // [4][P][P] the staging maps (used when transform == 1)
+    double *omega_k, *lam_k, *gam_k;   // [P] mode frequency, mass factor, friction
+    double *pileg_partial, *pileg_alpha;   // [R][64][2], [R]
     int *err;                          // [4] device error word
     double *est_partial;               // [R][EST_BLOCKS][8]
     double *est_out;                   // [R][8]

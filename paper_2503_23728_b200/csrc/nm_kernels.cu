@@ -1,9 +1,15 @@
-// nm_kernels.cu -- ring-polymer normal-mode integrator kernels (rows a8-a11 of SURVEY 8(a)).
+// nm_kernels.cu -- ring-polymer integrator kernels (rows a8-a11 of SURVEY 8(a); variants of 8(f)4).
 //
 // pimd_nm: one CTA owns TC (atom,dim) columns of one replica and all P beads of them, staged in
 // shared memory as [P][TC] fp64 slabs; global accesses are coalesced over the column index
-// (contiguous inside a bead).  The P x P orthogonal transform (S:N2) is applied slab-wise;
-// PILE-L noise is Philox4x32-10 + Box-Muller keyed by (seed; atom, r*P+mode, step, tag) (S:N4).
+// (contiguous inside a bead).  The bead <-> mode maps are applied slab-wise as P x P matrices:
+//   normal modes (S:N2, the default)  u = C^T q, p_u = C^T p            (orthogonal: the inverse maps are C)
+//   staging                   u = F q,  p_u = F^-T p            (F from the definition of the staging variables)
+//   primitive                identity; the ring springs are explicit forces in the B step
+// with per-mode mass factors, frequencies and frictions set up by the host (pimd_api.cu).
+// Thermostats: PILE-L (S:N3): Langevin on every mode; PILE-G: the free mode of all atoms of a replica is
+// rescaled by one stochastic factor alpha (global velocity rescaling), computed by a fixed-order reduction.
+// Noise is Philox4x32-10 + Box-Muller keyed by (seed; atom, r*P+mode, step, tag) (S:N4).
 // HBM-bound: ~(q,p read+write, F read) 8-byte words per bead-atom-dim per step.
 #include "common.cuh"
 #include <math.h>
@@ -14,9 +20,14 @@ constexpr int NM_TY = 8;
 
 struct NmArgs {
     int N, R, P, TC;
+    int transform, thermostat;   // 0 normal modes | 1 staging | 2 primitive;  0 PILE-L | 1 PILE-G
     double dt, gamma_fs, kT_P;   // kT_P = k_B T P = 1/beta_P
+    double omega_P;              // P k_B T / hbar (explicit springs of the primitive variant)
     unsigned long long seed;
-    const double *C, *CT, *omega_k, *mass;
+    const double *Tq_fwd, *Tq_inv, *Tp_fwd, *Tp_inv;   // [P][P]: u = Tq_fwd q, q = Tq_inv u, p_u = Tp_fwd p, p = Tp_inv p_u
+    const double *lam, *omega_k, *gam_k;               // [P]: mode mass factor, free-ring frequency, friction (fs^-1)
+    const double *mass;
+    const double *alpha;         // [R] PILE-G scale of the free mode for this half-step
     double *q, *p;
     const double *F;
     int *err;
@@ -81,13 +92,21 @@ __device__ __forceinline__ void pile_O(const NmArgs &a, double *pt, int r, int c
     const int c = threadIdx.x;
     const int atom = col / 3, dim = col - 3 * atom;
     const double hdt = 0.5 * a.dt;
-    const double sig = sqrt(a.mass[atom] * a.kT_P);
     for (int k = threadIdx.y; k < a.P; k += NM_TY) {
-        double gam = (k == 0) ? a.gamma_fs : 2.0 * a.omega_k[k];
-        double c1 = exp(-gam * hdt), c2 = sqrt(1.0 - c1 * c1);
+        if (k == 0 && a.thermostat == 1) { pt[c] = a.alpha[r] * pt[c]; continue; }   // PILE-G: one factor for the replica's free modes
+        const double sig = sqrt(a.mass[atom] * a.lam[k] * a.kT_P);
+        double c1 = exp(-a.gam_k[k] * hdt), c2 = sqrt(1.0 - c1 * c1);
         double xi = normal_component(a.seed, (uint32_t)atom, (uint32_t)(r * a.P + k), t, tag, dim);
         pt[k * a.TC + c] = c1 * pt[k * a.TC + c] + sig * c2 * xi;
     }
+}
+
+// B(dt/2) of the primitive variant adds the explicit ring springs -m w_P^2 ((q_j - q_{j-1}) + (q_j - q_{j+1}))
+__device__ __forceinline__ double spring_force(const NmArgs &a, const double *bQ, int j, int c, double mi)
+{
+    const int P = a.P, jm = (j + P - 1) % P, jp = (j + 1) % P;
+    const double qj = bQ[j * a.TC + c];
+    return -mi * a.omega_P * a.omega_P * ((qj - bQ[jm * a.TC + c]) + (qj - bQ[jp * a.TC + c]));
 }
 
 // mode: 0 = pre (O,B,A), 1 = post (B,O), 2 = initial momenta (S:N5)
@@ -108,11 +127,10 @@ __global__ void __launch_bounds__(32 * NM_TY) nm_kernel(NmArgs a, uint32_t t)
 
     if (MODE == 2) {
         const int atom = colc / 3, dim = colc - 3 * atom;
-        const double sig = sqrt(a.mass[atom] * a.kT_P);
         for (int k = threadIdx.y; k < P; k += NM_TY)
-            bT[k * TC + c] = sig * normal_component(a.seed, (uint32_t)atom, (uint32_t)(r * P + k), 0u, 2u, dim);
+            bT[k * TC + c] = sqrt(a.mass[atom] * a.lam[k] * a.kT_P) * normal_component(a.seed, (uint32_t)atom, (uint32_t)(r * P + k), 0u, 2u, dim);
         __syncthreads();
-        xform(a.C, bT, bP, P, TC);
+        xform(a.Tp_inv, bT, bP, P, TC);
         __syncthreads();
         if (live)
             for (int j = threadIdx.y; j < P; j += NM_TY) a.p[base + (size_t)j * ncol] = bP[j * TC + c];
@@ -120,23 +138,29 @@ __global__ void __launch_bounds__(32 * NM_TY) nm_kernel(NmArgs a, uint32_t t)
     }
 
     bool bad = false;
+    const bool prim = a.transform == 2;
+    const double mi = a.mass[colc / 3];
+    if (MODE == 0 || prim) {
+        for (int j = threadIdx.y; j < P; j += NM_TY) bQ[j * TC + c] = live ? a.q[base + (size_t)j * ncol] : 0.0;
+        if (MODE == 1) __syncthreads();   // the spring force below reads the neighbouring beads
+    }
     for (int j = threadIdx.y; j < P; j += NM_TY) {
         double pv = live ? a.p[base + (size_t)j * ncol] : 0.0;
         if (MODE == 1) {  // B(dt/2) first
             double f = live ? a.F[base + (size_t)j * ncol] : 0.0;
             bad |= !isfinite(f);
+            if (prim) f += spring_force(a, bQ, j, c, mi);
             pv += hdt * f;
         }
         bP[j * TC + c] = pv;
-        if (MODE == 0) bQ[j * TC + c] = live ? a.q[base + (size_t)j * ncol] : 0.0;
     }
     __syncthreads();
     if (thermo) {
-        xform(a.CT, bP, bT, P, TC);
+        xform(a.Tp_fwd, bP, bT, P, TC);
         __syncthreads();
         pile_O(a, bT, r, colc, t, MODE == 0 ? 0u : 1u);
         __syncthreads();
-        xform(a.C, bT, bP, P, TC);
+        xform(a.Tp_inv, bT, bP, P, TC);
         __syncthreads();
     }
     if (MODE == 1) {
@@ -145,34 +169,35 @@ __global__ void __launch_bounds__(32 * NM_TY) nm_kernel(NmArgs a, uint32_t t)
         if (bad) atomicOr(a.err, PIMD_FLAG_NAN);
         return;
     }
-    // MODE 0: B(dt/2), then A(dt) exact in normal modes
+    // MODE 0: B(dt/2), then A(dt): every mode is propagated exactly under p^2 / (2 m lam) + 1/2 m lam w^2 u^2
     for (int j = threadIdx.y; j < P; j += NM_TY) {
         double f = live ? a.F[base + (size_t)j * ncol] : 0.0;
+        if (prim) f += spring_force(a, bQ, j, c, mi);
         bP[j * TC + c] += hdt * f;
     }
     __syncthreads();
-    xform(a.CT, bQ, bQ2, P, TC);
-    xform(a.CT, bP, bT, P, TC);
+    xform(a.Tq_fwd, bQ, bQ2, P, TC);
+    xform(a.Tp_fwd, bP, bT, P, TC);
     __syncthreads();
     {
-        const double mi = a.mass[colc / 3];
         for (int k = threadIdx.y; k < P; k += NM_TY) {
             double qt = bQ2[k * TC + c], pt = bT[k * TC + c];
-            if (k == 0) {
-                qt = qt + a.dt * pt / mi;
+            const double mu = mi * a.lam[k], w = a.omega_k[k];
+            if (w == 0.0) {
+                qt = qt + a.dt * pt / mu;
             } else {
-                double w = a.omega_k[k], sn, cs;
+                double sn, cs;
                 sincos(w * a.dt, &sn, &cs);
-                double pn = cs * pt - mi * w * sn * qt;
-                double qn = sn / (mi * w) * pt + cs * qt;
+                double pn = cs * pt - mu * w * sn * qt;
+                double qn = sn / (mu * w) * pt + cs * qt;
                 pt = pn; qt = qn;
             }
             bQ2[k * TC + c] = qt; bT[k * TC + c] = pt;
         }
     }
     __syncthreads();
-    xform(a.C, bQ2, bQ, P, TC);
-    xform(a.C, bT, bP, P, TC);
+    xform(a.Tq_inv, bQ2, bQ, P, TC);
+    xform(a.Tp_inv, bT, bP, P, TC);
     __syncthreads();
     if (live)
         for (int j = threadIdx.y; j < P; j += NM_TY) {
@@ -184,12 +209,70 @@ __global__ void __launch_bounds__(32 * NM_TY) nm_kernel(NmArgs a, uint32_t t)
     if (bad) atomicOr(a.err, PIMD_FLAG_NAN);
 }
 
+// PILE-G (global thermostat on the free modes of a replica): per replica, the kinetic energy K of the free
+// modes (k = 0) of all atoms, and the noise sums R1 (first normal: atom 0, x) and S (squares of the other 3N - 1 normals of
+// the stream PILE-L would use for mode 0).  Partial sums per block in a fixed order, then one thread per replica:
+//   alpha^2 = c + (1 - c) (R1^2 + S) / (2 beta_P K) + 2 R1 sqrt(c (1 - c) / (2 beta_P K)),  c = exp(-gamma dt / 2),
+//   sign(alpha) = sign(R1 + sqrt(2 beta_P K c / (1 - c)))           (stochastic velocity rescaling, exact for the half-step)
+constexpr int PG_BLOCKS = 64, PG_THREADS = 128;
+
+__global__ void __launch_bounds__(PG_THREADS) pileg_partial_kernel(NmArgs a, uint32_t t, uint32_t tag, int after_B, double *__restrict__ partial)
+{
+    __shared__ double red[2][PG_THREADS];
+    const int r = blockIdx.y, P = a.P, ncol = 3 * a.N;
+    const double hdt = 0.5 * a.dt;
+    double K = 0.0, S = 0.0;
+    for (int col = blockIdx.x * PG_THREADS + threadIdx.x; col < ncol; col += PG_BLOCKS * PG_THREADS) {
+        const int atom = col / 3, dim = col - 3 * atom;
+        const size_t base = (size_t)r * P * ncol + col;
+        double pm = 0.0;
+        for (int j = 0; j < P; ++j) {
+            double pv = a.p[base + (size_t)j * ncol];
+            if (after_B) pv += hdt * a.F[base + (size_t)j * ncol];
+            pm += a.Tp_fwd[j] * pv;          // row 0 of the momentum map: the free mode
+        }
+        K += pm * pm / (2.0 * a.mass[atom] * a.lam[0]);
+        if (col > 0) {
+            const double xi = normal_component(a.seed, (uint32_t)atom, (uint32_t)(r * P), t, tag, dim);
+            S += xi * xi;
+        }
+    }
+    red[0][threadIdx.x] = K; red[1][threadIdx.x] = S;
+    __syncthreads();
+    for (int s = PG_THREADS / 2; s > 0; s >>= 1) {
+        if (threadIdx.x < s) { red[0][threadIdx.x] += red[0][threadIdx.x + s]; red[1][threadIdx.x] += red[1][threadIdx.x + s]; }
+        __syncthreads();
+    }
+    if (threadIdx.x < 2) partial[((size_t)r * PG_BLOCKS + blockIdx.x) * 2 + threadIdx.x] = red[threadIdx.x][0];
+}
+
+__global__ void pileg_final_kernel(NmArgs a, uint32_t t, uint32_t tag, const double *__restrict__ partial, double *__restrict__ alpha)
+{
+    const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= a.R) return;
+    double K = 0.0, S = 0.0;
+    for (int b = 0; b < PG_BLOCKS; ++b) { K += partial[((size_t)r * PG_BLOCKS + b) * 2]; S += partial[((size_t)r * PG_BLOCKS + b) * 2 + 1]; }
+    const double R1 = normal_component(a.seed, 0u, (uint32_t)(r * a.P), t, tag, 0);
+    const double c1 = exp(-a.gamma_fs * 0.5 * a.dt), bP = 1.0 / a.kT_P;
+    double al = 1.0;
+    if (K > 0.0) {
+        const double a2 = c1 + (1.0 - c1) * (R1 * R1 + S) / (2.0 * bP * K) + 2.0 * R1 * sqrt(c1 * (1.0 - c1) / (2.0 * bP * K));
+        const double sgn = (R1 + sqrt(2.0 * bP * K * c1 / (1.0 - c1)) >= 0.0) ? 1.0 : -1.0;
+        al = sgn * sqrt(a2 > 0.0 ? a2 : 0.0);
+    }
+    alpha[r] = al;
+}
+
 NmArgs make_args(const pimd_ctx *c)
 {
     NmArgs a;
     a.N = c->N; a.R = c->R; a.P = c->P; a.TC = (c->P <= 128) ? 32 : 16;
+    a.transform = c->transform; a.thermostat = c->thermostat;
     a.dt = c->dt; a.gamma_fs = c->gamma_fs; a.kT_P = PIMD_KB * c->T * c->P;
-    a.seed = c->seed; a.C = c->Cmat; a.CT = c->CmatT; a.omega_k = c->omega_k; a.mass = c->mass;
+    a.omega_P = c->P * PIMD_KB * c->T / PIMD_HBAR;
+    a.seed = c->seed;
+    a.Tq_fwd = c->Tq_fwd; a.Tq_inv = c->Tq_inv; a.Tp_fwd = c->Tp_fwd; a.Tp_inv = c->Tp_inv;
+    a.lam = c->lam_k; a.omega_k = c->omega_k; a.gam_k = c->gam_k; a.mass = c->mass; a.alpha = c->pileg_alpha;
     a.q = c->q; a.p = c->p; a.F = c->F; a.err = c->err;
     return a;
 }
@@ -198,6 +281,12 @@ template <int MODE>
 int launch_nm(pimd_ctx *c, uint32_t t)
 {
     NmArgs a = make_args(c);
+    if (MODE != 2 && c->thermostat == 1 && c->gamma_fs >= 0.0) {   // PILE-G: the replica's scale factor for this half-step
+        const uint32_t tag = MODE == 0 ? 0u : 1u;
+        pileg_partial_kernel<<<dim3(PG_BLOCKS, c->R), PG_THREADS, 0, c->stream>>>(a, t, tag, MODE == 1 ? 1 : 0, c->pileg_partial);
+        pileg_final_kernel<<<(c->R + 127) / 128, 128, 0, c->stream>>>(a, t, tag, c->pileg_partial, c->pileg_alpha);
+        c->launches += 2;
+    }
     size_t smem = (size_t)4 * c->P * a.TC * sizeof(double);
     if (!(c->attr_done & (ATTR_NM << MODE))) {
         PIMD_CUDA_CHECK(cudaFuncSetAttribute(nm_kernel<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));

@@ -7,6 +7,7 @@
 #include <stdio.h>
 #include <stdlib.h>
 #include <string.h>
+#include <algorithm>
 #include <vector>
 
 static thread_local char g_err[512] = "";
@@ -59,7 +60,7 @@ void pimd_prof_end(pimd_ctx *c)
 namespace {
 
 struct Layout {
-    size_t q, p, F, species, mass, C, CT, omega, err, est_partial, est_out;
+    size_t q, p, F, species, mass, C, CT, omega, lam, gam, Tstage, pileg_partial, pileg_alpha, err, est_partial, est_out;
     size_t cell_id, cell_count, cell_start, cell_cursor, sorted_atom, sorted_q, nnz, hits, row_ptr, block_sums, col, pair_row;
     size_t wimg, wimg_node, xs0, h1_img, meta_img, weights, nfeat, xfeat, mfeat, Efeat, Gfeat, carry_m, carry_f, Fraw;
     size_t total;
@@ -152,6 +153,11 @@ int compute_layout(int N, int R, int P, const double box[3], const pimd_net_para
     L->C = take(cur, sizeof(double) * P * P);
     L->CT = take(cur, sizeof(double) * P * P);
     L->omega = take(cur, sizeof(double) * P);
+    L->lam = take(cur, sizeof(double) * P);
+    L->gam = take(cur, sizeof(double) * P);
+    L->Tstage = take(cur, sizeof(double) * 4 * P * P);
+    L->pileg_partial = take(cur, sizeof(double) * (size_t)R * 64 * 2);
+    L->pileg_alpha = take(cur, sizeof(double) * (size_t)R);
     L->err = take(cur, sizeof(int) * 4);
     L->est_partial = take(cur, sizeof(double) * (size_t)R * 64 * 8);
     L->est_out = take(cur, sizeof(double) * (size_t)R * 8);
@@ -418,6 +424,10 @@ extern "C" int pimd_create(pimd_ctx **out, int n_atoms, int n_replicas, const in
     c->q = (double *)(ws + L.q); c->p = (double *)(ws + L.p); c->F = (double *)(ws + L.F);
     c->species = (int *)(ws + L.species); c->mass = (double *)(ws + L.mass);
     c->Cmat = (double *)(ws + L.C); c->CmatT = (double *)(ws + L.CT); c->omega_k = (double *)(ws + L.omega);
+    c->lam_k = (double *)(ws + L.lam); c->gam_k = (double *)(ws + L.gam); c->Tstage = (double *)(ws + L.Tstage);
+    c->pileg_partial = (double *)(ws + L.pileg_partial); c->pileg_alpha = (double *)(ws + L.pileg_alpha);
+    c->transform = 0; c->thermostat = 0;
+    c->Tq_fwd = c->CmatT; c->Tp_fwd = c->CmatT; c->Tq_inv = c->Cmat; c->Tp_inv = c->Cmat;   // normal modes: orthogonal
     c->err = (int *)(ws + L.err);
     c->est_partial = (double *)(ws + L.est_partial); c->est_out = (double *)(ws + L.est_out);
 
@@ -458,6 +468,10 @@ extern "C" int pimd_create(pimd_ctx **out, int n_atoms, int n_replicas, const in
     CREATE_CHECK(cudaMemcpyAsync(c->Cmat, Cm.data(), sizeof(double) * P * P, cudaMemcpyHostToDevice, st));
     CREATE_CHECK(cudaMemcpyAsync(c->CmatT, CT.data(), sizeof(double) * P * P, cudaMemcpyHostToDevice, st));
     CREATE_CHECK(cudaMemcpyAsync(c->omega_k, om.data(), sizeof(double) * P, cudaMemcpyHostToDevice, st));
+    std::vector<double> lam(P, 1.0), gam(P);
+    for (int k = 0; k < P; ++k) gam[k] = (k == 0) ? c->gamma_fs : 2.0 * om[k];   // PILE: critical damping of the free-ring modes (S:N3)
+    CREATE_CHECK(cudaMemcpyAsync(c->lam_k, lam.data(), sizeof(double) * P, cudaMemcpyHostToDevice, st));
+    CREATE_CHECK(cudaMemcpyAsync(c->gam_k, gam.data(), sizeof(double) * P, cudaMemcpyHostToDevice, st));
 
     std::vector<float> wd, xs0;
     std::vector<uint16_t> wimg, wimg_node;
@@ -589,6 +603,85 @@ extern "C" void pimd_destroy(pimd_ctx *c)
         delete c->prof;
     }
     delete c;
+}
+
+// Integrator variants ("normal mode or staging transformation", P:L114 primitive PIMD with the bead
+// springs as explicit forces).  The mode tables are built here, in fp64 on the host, from the DEFINITIONS:
+//   staging variables  u_0 = q_0,  u_j = q_j - (j q_{j+1} + q_0) / (j + 1), q_P = q_0  ->  matrix F;  q = F^-1 u by elimination;
+//   canonical momenta transform with the inverse transpose: p_u = F^-T p_q, p_q = F^T p_u;
+//   staging masses m (j+1)/j and frequency w_P for j >= 1 (the ring springs become sum_j 1/2 m lam_j w_P^2 u_j^2), u_0 free.
+extern "C" int pimd_set_integrator(pimd_ctx *c, int transform, int thermostat)
+{
+    if (!c) { pimd_set_error("null context"); return PIMD_ERR_ARG; }
+    if (transform < 0 || transform > 2 || thermostat < 0 || thermostat > 1) { pimd_set_error("transform in {0,1,2}, thermostat in {0,1}"); return PIMD_ERR_ARG; }
+    if (thermostat == 1 && transform == 2) { pimd_set_error("PILE-G needs a free (centroid-like) mode: not with the primitive variant"); return PIMD_ERR_ARG; }
+    if (c->step != 0) { pimd_set_error("the integrator variant is chosen before the first step"); return PIMD_ERR_ARG; }
+    int rc;
+    if ((rc = enter(c))) return rc;
+    const int P = c->P;
+    const double pi = 3.14159265358979323846264338327950288;
+    const double omega_P = P * PIMD_KB * c->T / PIMD_HBAR;
+    std::vector<double> om(P), lam(P, 1.0), gam(P);
+    if (transform == 0) {
+        for (int k = 0; k < P; ++k) { om[k] = 2.0 * omega_P * sin(k * pi / P); gam[k] = (k == 0) ? c->gamma_fs : 2.0 * om[k]; }
+        c->Tq_fwd = c->CmatT; c->Tp_fwd = c->CmatT; c->Tq_inv = c->Cmat; c->Tp_inv = c->Cmat;
+    } else if (transform == 2) {
+        // identity maps: rows of the normal-mode storage are not needed; the staging block holds I four times
+        std::vector<double> I4((size_t)4 * P * P, 0.0);
+        for (int m = 0; m < 4; ++m) for (int j = 0; j < P; ++j) I4[(size_t)m * P * P + (size_t)j * P + j] = 1.0;
+        PIMD_CUDA_CHECK(cudaMemcpyAsync(c->Tstage, I4.data(), sizeof(double) * I4.size(), cudaMemcpyHostToDevice, c->stream));
+        PIMD_CUDA_CHECK(cudaStreamSynchronize(c->stream));
+        c->Tq_fwd = c->Tstage; c->Tq_inv = c->Tstage + (size_t)P * P; c->Tp_fwd = c->Tstage + 2 * (size_t)P * P; c->Tp_inv = c->Tstage + 3 * (size_t)P * P;
+        for (int k = 0; k < P; ++k) { om[k] = 0.0; gam[k] = c->gamma_fs; }   // every bead flies freely in A; white-noise Langevin on every bead
+    } else {
+        std::vector<long double> F((size_t)P * P, 0.0L), Fi((size_t)P * P, 0.0L);
+        F[0] = 1.0L;
+        for (int j = 1; j < P; ++j) {
+            F[(size_t)j * P + j] += 1.0L;
+            F[(size_t)j * P + (j + 1) % P] -= (long double)j / (long double)(j + 1);
+            F[(size_t)j * P + 0] -= 1.0L / (long double)(j + 1);
+        }
+        {   // inverse by Gauss-Jordan elimination with partial pivoting
+            std::vector<long double> A(F);
+            for (int j = 0; j < P; ++j) Fi[(size_t)j * P + j] = 1.0L;
+            for (int col = 0; col < P; ++col) {
+                int piv = col;
+                for (int rr = col + 1; rr < P; ++rr) if (fabsl(A[(size_t)rr * P + col]) > fabsl(A[(size_t)piv * P + col])) piv = rr;
+                if (piv != col)
+                    for (int k = 0; k < P; ++k) { std::swap(A[(size_t)piv * P + k], A[(size_t)col * P + k]); std::swap(Fi[(size_t)piv * P + k], Fi[(size_t)col * P + k]); }
+                const long double d = A[(size_t)col * P + col];
+                for (int k = 0; k < P; ++k) { A[(size_t)col * P + k] /= d; Fi[(size_t)col * P + k] /= d; }
+                for (int rr = 0; rr < P; ++rr) {
+                    if (rr == col) continue;
+                    const long double f = A[(size_t)rr * P + col];
+                    if (f == 0.0L) continue;
+                    for (int k = 0; k < P; ++k) { A[(size_t)rr * P + k] -= f * A[(size_t)col * P + k]; Fi[(size_t)rr * P + k] -= f * Fi[(size_t)col * P + k]; }
+                }
+            }
+        }
+        std::vector<double> T4((size_t)4 * P * P);
+        for (int j = 0; j < P; ++j)
+            for (int k = 0; k < P; ++k) {
+                T4[(size_t)j * P + k] = (double)F[(size_t)j * P + k];                                  // u = F q
+                T4[(size_t)P * P + (size_t)j * P + k] = (double)Fi[(size_t)j * P + k];                 // q = F^-1 u
+                T4[2 * (size_t)P * P + (size_t)j * P + k] = (double)Fi[(size_t)k * P + j];             // p_u = F^-T p_q
+                T4[3 * (size_t)P * P + (size_t)j * P + k] = (double)F[(size_t)k * P + j];              // p_q = F^T p_u
+            }
+        PIMD_CUDA_CHECK(cudaMemcpyAsync(c->Tstage, T4.data(), sizeof(double) * T4.size(), cudaMemcpyHostToDevice, c->stream));
+        PIMD_CUDA_CHECK(cudaStreamSynchronize(c->stream));
+        c->Tq_fwd = c->Tstage; c->Tq_inv = c->Tstage + (size_t)P * P; c->Tp_fwd = c->Tstage + 2 * (size_t)P * P; c->Tp_inv = c->Tstage + 3 * (size_t)P * P;
+        for (int k = 0; k < P; ++k) {
+            lam[k] = (k == 0) ? 1.0 : (double)(k + 1) / (double)k;
+            om[k] = (k == 0) ? 0.0 : omega_P;
+            gam[k] = (k == 0) ? c->gamma_fs : 2.0 * omega_P;
+        }
+    }
+    PIMD_CUDA_CHECK(cudaMemcpyAsync(c->omega_k, om.data(), sizeof(double) * P, cudaMemcpyHostToDevice, c->stream));
+    PIMD_CUDA_CHECK(cudaMemcpyAsync(c->lam_k, lam.data(), sizeof(double) * P, cudaMemcpyHostToDevice, c->stream));
+    PIMD_CUDA_CHECK(cudaMemcpyAsync(c->gam_k, gam.data(), sizeof(double) * P, cudaMemcpyHostToDevice, c->stream));
+    PIMD_CUDA_CHECK(cudaStreamSynchronize(c->stream));
+    c->transform = transform; c->thermostat = thermostat;
+    return pimd_launch_init_momenta(c);   // S:N5 in the chosen representation
 }
 
 extern "C" int pimd_step(pimd_ctx *c, int n)

@@ -53,6 +53,7 @@ def load_library():
     L.pimd_create.argtypes = [C.POINTER(vp), C.c_int, C.c_int, ip, dp, dp, dp, C.c_int, C.c_double, C.c_double,
                               C.c_double, C.c_uint64, C.POINTER(NetParams), vp, C.c_size_t, vp]
     L.pimd_step.argtypes = [vp, C.c_int]
+    L.pimd_set_integrator.argtypes = [vp, C.c_int, C.c_int]
     L.pimd_forces.argtypes = [vp, vp]
     L.pimd_estimators.argtypes = [vp, C.POINTER(Estimators)]
     L.pimd_get_state.argtypes = [vp, vp, vp, C.POINTER(C.c_int64)]
@@ -143,6 +144,13 @@ class PIMD:
             pass
 
     # ---- C-ABI calls -------------------------------------------------------------------------
+    TRANSFORMS = {"normal_modes": 0, "staging": 1, "primitive": 2}
+    THERMOSTATS = {"pile_l": 0, "pile_g": 1}
+
+    def set_integrator(self, transform="normal_modes", thermostat="pile_l"):
+        """Integrator variant (before the first step): normal-mode / staging / primitive, PILE-L / PILE-G."""
+        _check(load_library().pimd_set_integrator(self._h, self.TRANSFORMS[transform], self.THERMOSTATS[thermostat]))
+
     def step(self, n=1):
         _check(load_library().pimd_step(self._h, int(n)))
 

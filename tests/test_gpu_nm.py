@@ -117,3 +117,39 @@ def test_pile_friction_constants_on_gpu(cuda_device):
     want = np.exp(-gam * dt) * np.cos(wk * dt)
     tol = 3 * np.sqrt(2.0) / amp / np.sqrt(3 * N)
     assert np.all(np.abs(got - want) < tol), (got, want, tol)
+
+
+@pytest.mark.parametrize("transform,thermostat", [("staging", "pile_l"), ("staging", "pile_g"), ("normal_modes", "pile_g"),
+                                                  ("primitive", "pile_l")])
+@pytest.mark.parametrize("P", [1, 4, 32])
+def test_integrator_variants_match_oracle(cuda_device, transform, thermostat, P):
+    """staging transformation, primitive PIMD with explicit springs, PILE-G; the
+    device builds the staging maps as matrices from the definition (F, F^-1 by elimination, inverse transposes for the momenta),
+    the oracle applies the recurrences: two derivations of the same maps."""
+    sp, pos = _system(N=11, R=3)
+    for gamma in (-1.0, 20.0):
+        if thermostat == "pile_g" and gamma < 0:
+            continue
+        gpu, ref = make_pair(sp, pos, np.zeros(3), P, 300.0, 0.25, gamma, 23, _spec(1, 0.2))
+        gpu.set_integrator(transform, thermostat); ref.set_integrator(transform, thermostat)
+        qg, pg, _ = gpu_state(gpu)
+        qr, pr, _ = ref.get_state()
+        assert np.abs(pg - pr).max() < 1e-12 * max(1.0, np.abs(pr).max())      # initial momenta in the chosen representation
+        spread_beads(gpu, ref)
+        gpu.step(40); ref.step(40)
+        qg, pg, sg = gpu_state(gpu)
+        qr, pr, sr = ref.get_state()
+        assert sg == sr == 40
+        assert np.abs(qg - qr).max() < 1e-10, (transform, thermostat, P, gamma, np.abs(qg - qr).max())
+        assert np.abs(pg - pr).max() < 1e-9 * max(1.0, np.abs(pr).max())
+
+
+def test_integrator_variant_is_chosen_before_the_first_step(cuda_device):
+    import paper_2503_23728_b200 as pb
+    sp, pos = _system()
+    gpu, ref = make_pair(sp, pos, np.zeros(3), 4, 300.0, 0.25, 1.0, 1, _spec(2))
+    with pytest.raises(pb.PimdError):
+        gpu.set_integrator("primitive", "pile_g")       # no free mode to rescale
+    gpu.step(1)
+    with pytest.raises(pb.PimdError):
+        gpu.set_integrator("staging", "pile_l")
