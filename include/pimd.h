@@ -146,6 +146,17 @@ int pimd_set_forces_cached(pimd_ctx *ctx, const double *d_F);
  *   h_n_pairs HOST.  Synchronises. */
 int pimd_nlist(pimd_ctx *ctx, int32_t *d_row_ptr, int32_t *d_col, int64_t col_capacity, int64_t *h_n_pairs);
 
+/* Neighbour-list reuse (the paper fixes only the cutoff, so any list that yields the forces of the exact-r_cut list is
+ * admissible): candidates within r_cut + skin are collected by the cell-list pass and kept until some atom has moved by skin/2
+ * or more (checked on the device every step, no host synchronisation); every step the exact list d^2 < r_cut^2 (S:L3) is
+ * filtered from them, so pimd_nlist and the forces are identical for every skin.  skin in A; 0 = cell-list pass every step.
+ * Default: 0 (pays only when atoms move by less than skin/2 over many steps).  PIMD_ERR_ARG unless every periodic box edge
+ * >= 2 (r_cut + skin).
+ * Asynchronous. */
+int pimd_set_nlist_skin(pimd_ctx *ctx, double skin);
+/* Number of cell-list passes (candidate-list rebuilds) so far.  h_count HOST.  Synchronises. */
+int pimd_nlist_rebuilds(pimd_ctx *ctx, int64_t *h_count);
+
 /* Waits for the stream and returns any latched device error. */
 int pimd_sync(pimd_ctx *ctx);
 

@@ -47,8 +47,14 @@ struct NlistDev {
     int *cell_cursor;                  // [nsys*ncell_tot]
     int *sorted_atom;                  // [rows] local atom index in cell order
     double *sorted_q;                  // [rows][3]
-    int *nnz;                          // [rows]
-    int *hits;                         // [rows][hit_stride] unsorted neighbour indices of each row
+    int *nnz;                          // [rows] neighbours within r_cut (this step)
+    int *ncand;                        // [rows] candidates within r_cut + skin (since the last rebuild)
+    int *hits;                         // [rows][hit_stride] candidate indices of each row, ascending j after the rebuild
+    unsigned *hitmask;                 // [rows][PIMD_MAX_NBR / 32] which candidates are within r_cut this step
+    double *q_ref;                     // [rows][3] positions the candidate lists were built at
+    float4 *q32;                       // [rows] fp32 copy of the current positions (filter estimate)
+    int *need;                         // device flag: rebuild the candidate lists
+    double skin;                       // A; 0 = rebuild every step
     int hit_stride;
     int *row_ptr;                      // [rows+1]
     int *block_sums;                   // [ceil(rows/1024)+1]
@@ -136,6 +142,7 @@ int pimd_launch_nm_post(pimd_ctx *c, uint32_t t);
 int pimd_launch_simple_forces(pimd_ctx *c);          // kinds 1, 2
 int pimd_launch_estimators(pimd_ctx *c);
 int pimd_launch_nlist(pimd_ctx *c);
+int pimd_launch_nlist_invalidate(pimd_ctx *c);       // positions were replaced from outside: rebuild the candidate lists
 int pimd_launch_gfn_forces(pimd_ctx *c);
 int pimd_launch_copy_forces_f32(pimd_ctx *c, float *d_out);
 size_t pimd_gfn_smem_bytes(int K, int H);

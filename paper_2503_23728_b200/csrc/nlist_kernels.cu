@@ -1,4 +1,9 @@
-// nlist_kernels.cu -- per-bead-system periodic cell list -> CSR pair list (rows a1-a3 of SURVEY 8(a)).
+// nlist_kernels.cu -- per-bead-system periodic cell list -> CSR pair list (rows a1-a3 of SURVEY 8(a)), with
+// neighbour-list reuse (the paper fixes only the cutoff): the cell-list pass collects CANDIDATES
+// within r_cut + skin at reference positions and is repeated only when some atom has moved by skin/2 or more since
+// (decided on the device, no host synchronisation: the rebuild kernels are launched every step and return at once when
+// the flag is clear); every step the exact list is filtered from the candidates with the same fp64 predicate S:L3, so
+// the CSR, and with it the forces, are identical to a rebuild from scratch.  skin = 0 rebuilds every step.
 //
 // bin (wrapped fraction -> cell) -> counting sort (histogram, per-system exclusive scan, scatter of atom index + fp64
 // position into cell order) -> one CTA per cell stages its de-duplicated 3x3x3 stencil in shared memory (fp32 coordinates
@@ -16,7 +21,11 @@ struct NlArgs {
     int64_t rows;
     double box[3];
     double rc2;
-    float rc2_lo, rc2_hi;          // fp32 pre-filter band around r_c^2 (exact fp64 test inside the band)
+    double rl2;                    // (r_cut + skin)^2: candidate radius of the cell-list pass
+    float rc2_lo, rc2_hi;          // fp32 pre-filter band around the candidate radius^2 (exact fp64 test inside the band)
+    double skin_half2;             // (skin / 2)^2
+    const int *need;               // device flag: 1 = the candidate lists must be rebuilt this step
+    int *need_w;
     float boxf[3], inv_boxf[3];
     int nc[3], nct, hit_stride;
     const double *q;
@@ -24,10 +33,27 @@ struct NlArgs {
     int *err;
 };
 
-__global__ void bin_kernel(NlArgs a)
+// displacement since the candidate lists were built: any atom at or beyond skin/2 raises the rebuild flag
+__global__ void verlet_check_kernel(NlArgs a)
 {
     int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (row >= a.rows) return;
+    double d2 = 0.0;
+    const double x[3] = {a.q[row * 3], a.q[row * 3 + 1], a.q[row * 3 + 2]};
+#pragma unroll
+    for (int ax = 0; ax < 3; ++ax) { const double d = x[ax] - a.d.q_ref[row * 3 + ax]; d2 += d * d; }
+    if (!(d2 < a.skin_half2)) *a.need_w = 1;       // (also NaN positions)
+    a.d.q32[row] = make_float4((float)x[0], (float)x[1], (float)x[2], 0.f);   // fp32 copy for the filter's estimate (one 16-byte gather per candidate)
+}
+
+__global__ void bin_kernel(NlArgs a)
+{
+    if (!*a.need) return;
+    int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (row >= a.rows) return;
+#pragma unroll
+    for (int ax = 0; ax < 3; ++ax) a.d.q_ref[row * 3 + ax] = a.q[row * 3 + ax];   // reference positions of the new candidate lists
+    if (row == 0) a.need_w[1] += 1;                                              // rebuild counter (pimd_nlist_rebuilds)
     int cell = 0;
     if (a.periodic) {
         int c[3];
@@ -79,6 +105,7 @@ __device__ __forceinline__ int block_exclusive_scan(int v, int *total)
 // one block per bead-system: cell_start (relative) = exclusive scan of cell_count; zero the cursors
 __global__ void __launch_bounds__(256) scan_cells_kernel(NlArgs a)
 {
+    if (!*a.need) return;
     __shared__ int tot;
     const int sys = blockIdx.x;
     const int *cnt = a.d.cell_count + (size_t)sys * a.nct;
@@ -98,6 +125,7 @@ __global__ void __launch_bounds__(256) scan_cells_kernel(NlArgs a)
 
 __global__ void scatter_kernel(NlArgs a)
 {
+    if (!*a.need) return;
     int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (row >= a.rows) return;
     int sys = (int)(row / a.N), i = (int)(row - (int64_t)sys * a.N);
@@ -111,7 +139,7 @@ __global__ void scatter_kernel(NlArgs a)
 }
 
 // S:L3 predicate, explicit IEEE round-to-nearest operations in the stated order
-__device__ __forceinline__ bool within_cutoff(const double qi[3], const double *__restrict__ qj, const NlArgs &a)
+__device__ __forceinline__ bool within_cutoff(const double qi[3], const double *__restrict__ qj, const NlArgs &a, double r2)
 {
     double d[3];
 #pragma unroll
@@ -121,7 +149,7 @@ __device__ __forceinline__ bool within_cutoff(const double qi[3], const double *
         d[ax] = dx;
     }
     double d2 = __dadd_rn(__dadd_rn(__dmul_rn(d[0], d[0]), __dmul_rn(d[1], d[1])), __dmul_rn(d[2], d[2]));
-    return d2 < a.rc2;
+    return d2 < r2;
 }
 
 // One CTA per (bead-system, cell).  The atoms of the cell's de-duplicated 3x3x3 stencil are staged in shared memory
@@ -145,6 +173,7 @@ __global__ void __launch_bounds__(COUNT_THREADS) count_cell_kernel(NlArgs a)
     __shared__ int hj[HOME_MAX];
     __shared__ int scnt[HOME_MAX];             // hits per home atom so far
     __shared__ float4 sc[CAND_CHUNK];          // candidate: position relative to the cell's reference atom (minimum image, fp32) | atom index
+    if (!*a.need) return;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int sys = blockIdx.x / a.nct, cell = blockIdx.x - sys * a.nct;
     const int *start = a.d.cell_start + (size_t)sys * (a.nct + 1);
@@ -260,7 +289,7 @@ __global__ void __launch_bounds__(COUNT_THREADS) count_cell_kernel(NlArgs a)
                     if (!hit) {                  // in the band (about 0.2 % of the candidates): fp64 positions
                         const double qi[3] = {in_s ? hq[0][ha] : a.d.sorted_q[posi * 3], in_s ? hq[1][ha] : a.d.sorted_q[posi * 3 + 1],
                                               in_s ? hq[2][ha] : a.d.sorted_q[posi * 3 + 2]};
-                        hit = within_cutoff(qi, a.d.sorted_q + (sbase + sp[s0]) * 3, a);
+                        hit = within_cutoff(qi, a.d.sorted_q + (sbase + sp[s0]) * 3, a, a.rl2);
                     }
                     if (hit) {
                         const int idx = in_s ? atomicAdd(&scnt[ha], 1) : atomicAdd(&a.d.nnz[row], 1);
@@ -275,8 +304,99 @@ __global__ void __launch_bounds__(COUNT_THREADS) count_cell_kernel(NlArgs a)
         const int64_t row = sbase + ((t < HOME_MAX) ? hj[t] : a.d.sorted_atom[sbase + h0 + t]);
         int cnt = (t < HOME_MAX) ? scnt[t] : a.d.nnz[row];
         if (cnt > a.hit_stride) { atomicOr(a.err, PIMD_FLAG_PAIRS); cnt = a.hit_stride; }
-        a.d.nnz[row] = cnt;
+        a.d.ncand[row] = cnt;
     }
+}
+
+// candidates of a row -> ascending j, in place: the row's candidates set bits in a per-warp bitmask over the atoms of the
+// bead-system (shared memory, N/32 words) and the set bits are written back in order.  N <= 32768 (checked by pimd_create).
+__global__ void __launch_bounds__(256) sort_candidates_kernel(NlArgs a, int nw)
+{
+    extern __shared__ unsigned smask[];       // [8][nw]
+    if (!*a.need) return;
+    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int64_t row = (int64_t)blockIdx.x * 8 + w;
+    if (row >= a.rows) return;
+    unsigned *mk = smask + (size_t)w * nw;
+    const int n = a.d.ncand[row];
+    int *hits = a.d.hits + row * a.hit_stride;
+    for (int t = lane; t < nw; t += 32) mk[t] = 0u;
+    __syncwarp();
+    for (int e = lane; e < n; e += 32) {
+        const int j = hits[e];
+        atomicOr(&mk[j >> 5], 1u << (j & 31));
+    }
+    __syncwarp();
+    const int wpl = (nw + 31) >> 5, w0 = lane * wpl, w1 = min(w0 + wpl, nw);
+    int cnt = 0;
+    for (int t = w0; t < w1; ++t) cnt += __popc(mk[t]);
+    int inc = cnt;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int v = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += v;
+    }
+    // a candidate is stored as j (15 bits) | image shift of the pair at the reference positions, five bits per axis (biased by 16:
+    // positions are never wrapped, S:L2, so the shift can be several box lengths) | bit 30 if a shift does not fit (the filter
+    // then takes the exact path).  The shift cannot change while the list is in use in a way that matters: a pair whose
+    // minimum image flips is at least r_cut apart with either image (box >= 2 (r_cut + skin)).
+    const int64_t sbase = (row / a.N) * a.N;
+    const double qi[3] = {a.q[row * 3], a.q[row * 3 + 1], a.q[row * 3 + 2]};
+    int *colp = hits + (inc - cnt);
+    for (int t = w0; t < w1; ++t) {
+        unsigned bits = mk[t];
+        while (bits) {
+            const int j = t * 32 + (__ffs(bits) - 1);
+            int packed = j;
+#pragma unroll
+            for (int ax = 0; ax < 3; ++ax) {
+                int sh = 0;
+                if (a.periodic) sh = (int)rint((a.q[(sbase + j) * 3 + ax] - qi[ax]) / a.box[ax]);
+                if (sh < -16 || sh > 15) { packed |= 1 << 30; sh = 0; }
+                packed |= (sh + 16) << (15 + 5 * ax);
+            }
+            *colp++ = packed;
+            bits &= bits - 1;
+        }
+    }
+}
+
+// every step: the exact list from the sorted candidates.  One warp per row; a lane tests candidates e = lane, lane + 32, ...:
+// an fp32 estimate from the fp32 copy of the positions and the stored image shift settles everything outside a 2e-4 band
+// around r_c^2, the fp64 predicate of S:L3 decides inside it; the ballots are kept as the row's hit mask.
+constexpr int MASK_WORDS = PIMD_MAX_NBR / 32;
+__global__ void __launch_bounds__(256) filter_count_kernel(NlArgs a)
+{
+    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int64_t row = (int64_t)blockIdx.x * 8 + w;
+    if (row >= a.rows) return;
+    const int n = a.d.ncand[row];
+    const int *cand = a.d.hits + row * a.hit_stride;
+    const int64_t sbase = (row / a.N) * a.N;
+    const float4 qi = a.d.q32[row];
+    const float lo = (float)(a.rc2 * (1.0 - 2e-4)), hi = (float)(a.rc2 * (1.0 + 2e-4));   // fp32 absolute coordinates: error << band
+    int cnt = 0;
+    for (int e0 = 0; e0 < n; e0 += 32) {
+        const int e = e0 + lane;
+        bool hit = false;
+        if (e < n) {
+            const int pk = cand[e], j = pk & 0x7FFF;
+            const float4 qj = __ldg(a.d.q32 + sbase + j);
+            const float dx = (qj.x - qi.x) - (float)(((pk >> 15) & 31) - 16) * a.boxf[0];
+            const float dy = (qj.y - qi.y) - (float)(((pk >> 20) & 31) - 16) * a.boxf[1];
+            const float dz = (qj.z - qi.z) - (float)(((pk >> 25) & 31) - 16) * a.boxf[2];
+            const float d2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+            hit = d2 < lo && !(pk & (1 << 30));
+            if ((!hit && d2 <= hi) || (pk & (1 << 30))) {   // in the band (or shift not stored): the exact fp64 operation sequence of S:L3 decides
+                const double qid[3] = {a.q[row * 3], a.q[row * 3 + 1], a.q[row * 3 + 2]};
+                hit = within_cutoff(qid, a.q + (sbase + j) * 3, a, a.rc2);
+            }
+        }
+        const unsigned m = __ballot_sync(0xffffffffu, hit);
+        if (lane == 0) a.d.hitmask[row * MASK_WORDS + (e0 >> 5)] = m;
+        cnt += __popc(m);
+    }
+    if (lane == 0) a.d.nnz[row] = cnt;
 }
 
 // row_ptr: three-kernel exclusive scan over rows (1024 rows per block)
@@ -357,7 +477,32 @@ __global__ void __launch_bounds__(256) fill_bitmask_kernel(NlArgs a, int nw)
     for (int e = lane; e < n; e += 32) a.d.pair_row[base + e] = (int)row;   // coalesced, outside the divergent loop
 }
 
+// CSR fill: the row's hit mask selects from its sorted candidates, so the rows come out in ascending j
+__global__ void __launch_bounds__(256) filter_fill_kernel(NlArgs a)
+{
+    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int64_t row = (int64_t)blockIdx.x * 8 + w;
+    if (blockIdx.x == 0 && threadIdx.x == 0) *a.need_w = 0;   // the candidate lists are current; the next check may raise the flag again
+    if (row >= a.rows) return;
+    if (a.d.row_ptr[a.rows] == 0) return;     // empty or overflowed list
+    const int n = a.d.ncand[row];
+    const int *cand = a.d.hits + row * a.hit_stride;
+    int64_t base = a.d.row_ptr[row];
+    for (int e0 = 0; e0 < n; e0 += 32) {
+        const unsigned m = a.d.hitmask[row * MASK_WORDS + (e0 >> 5)];
+        const int e = e0 + lane;
+        if ((m >> lane) & 1u) {
+            const int pos = __popc(m & ((1u << lane) - 1u));
+            a.d.col[base + pos] = cand[e] & 0x7FFF;
+            a.d.pair_row[base + pos] = (int)row;
+        }
+        base += __popc(m);
+    }
+}
+
 }  // namespace
+
+__global__ void set_flag_kernel(int *f, int v) { *f = v; }
 
 int pimd_launch_nlist(pimd_ctx *c)
 {
@@ -365,26 +510,63 @@ int pimd_launch_nlist(pimd_ctx *c)
     a.N = c->N; a.nsys = c->R * c->P; a.periodic = c->periodic; a.rows = c->rows;
     for (int k = 0; k < 3; ++k) { a.box[k] = c->box[k]; a.nc[k] = c->nl.ncell[k]; }
     a.rc2 = (double)c->net.r_cut * (double)c->net.r_cut;
+    const double rl = (double)c->net.r_cut + c->nl.skin;
+    a.rl2 = rl * rl;
+    a.skin_half2 = 0.25 * c->nl.skin * c->nl.skin;
     a.nct = c->nl.ncell_tot; a.q = c->q; a.d = c->nl; a.err = c->err;
-    a.rc2_lo = (float)(a.rc2 * (1.0 - 1e-3)); a.rc2_hi = (float)(a.rc2 * (1.0 + 1e-3));
+    a.need = c->nl.need; a.need_w = c->nl.need;
+    a.rc2_lo = (float)(a.rl2 * (1.0 - 1e-3)); a.rc2_hi = (float)(a.rl2 * (1.0 + 1e-3));
     for (int k = 0; k < 3; ++k) { a.boxf[k] = (float)c->box[k]; a.inv_boxf[k] = c->periodic ? (float)(1.0 / c->box[k]) : 0.f; }
     a.hit_stride = c->nl.hit_stride;
     const int64_t rows = c->rows;
     const unsigned gthr = (unsigned)((rows + 255) / 256), gwarp = (unsigned)((rows + 7) / 8);
     const int nblk = (int)((rows + 1023) / 1024);
+    const int nw = (c->N + 31) / 32;
+    const bool wrap = a.periodic && (a.nc[0] < 4 || a.nc[1] < 4 || a.nc[2] < 4);
+    if (c->nl.skin == 0.0) {
+        // no reuse: the cell-list pass at r_cut IS the list of this step (count -> scan -> fill through the bitmask, ascending j)
+        a.d.nnz = a.d.ncand;           // the count kernel's output is the row length
+        set_flag_kernel<<<1, 1, 0, c->stream>>>(c->nl.need, 1);
+        PIMD_CUDA_CHECK(cudaMemsetAsync(c->nl.cell_count, 0, sizeof(int) * (size_t)a.nsys * a.nct, c->stream));
+        bin_kernel<<<gthr, 256, 0, c->stream>>>(a);
+        scan_cells_kernel<<<a.nsys, 256, 0, c->stream>>>(a);
+        scatter_kernel<<<gthr, 256, 0, c->stream>>>(a);
+        if (wrap) count_cell_kernel<true><<<(unsigned)(a.nsys * a.nct), COUNT_THREADS, 0, c->stream>>>(a);
+        else count_cell_kernel<false><<<(unsigned)(a.nsys * a.nct), COUNT_THREADS, 0, c->stream>>>(a);
+        scan_rows_local_kernel<<<nblk, 1024, 0, c->stream>>>(a);
+        scan_block_sums_kernel<<<1, 1024, 0, c->stream>>>(a, nblk);
+        scan_rows_add_kernel<<<gthr, 256, 0, c->stream>>>(a);
+        fill_bitmask_kernel<<<gwarp, 256, (size_t)8 * nw * sizeof(unsigned), c->stream>>>(a, nw);
+        c->launches += 9;
+        PIMD_CUDA_CHECK(cudaGetLastError());
+        return 0;
+    }
+    // candidate lists (r_cut + skin): rebuilt only when the flag is up; these kernels return at once otherwise
+    verlet_check_kernel<<<gthr, 256, 0, c->stream>>>(a);
     PIMD_CUDA_CHECK(cudaMemsetAsync(c->nl.cell_count, 0, sizeof(int) * (size_t)a.nsys * a.nct, c->stream));
     bin_kernel<<<gthr, 256, 0, c->stream>>>(a);
     scan_cells_kernel<<<a.nsys, 256, 0, c->stream>>>(a);
     scatter_kernel<<<gthr, 256, 0, c->stream>>>(a);
-    const bool wrap = a.periodic && (a.nc[0] < 4 || a.nc[1] < 4 || a.nc[2] < 4);
     if (wrap) count_cell_kernel<true><<<(unsigned)(a.nsys * a.nct), COUNT_THREADS, 0, c->stream>>>(a);
     else count_cell_kernel<false><<<(unsigned)(a.nsys * a.nct), COUNT_THREADS, 0, c->stream>>>(a);
+    sort_candidates_kernel<<<gwarp, 256, (size_t)8 * nw * sizeof(unsigned), c->stream>>>(a, nw);
+    // exact list of this step, filtered from the candidates
+    filter_count_kernel<<<gwarp, 256, 0, c->stream>>>(a);
     scan_rows_local_kernel<<<nblk, 1024, 0, c->stream>>>(a);
     scan_block_sums_kernel<<<1, 1024, 0, c->stream>>>(a, nblk);
     scan_rows_add_kernel<<<gthr, 256, 0, c->stream>>>(a);
-    const int nw = (c->N + 31) / 32;
-    fill_bitmask_kernel<<<gwarp, 256, (size_t)8 * nw * sizeof(unsigned), c->stream>>>(a, nw);
-    c->launches += 8;
+    filter_fill_kernel<<<gwarp, 256, 0, c->stream>>>(a);
+    c->launches += 11;
+    PIMD_CUDA_CHECK(cudaGetLastError());
+    return 0;
+}
+
+// raises the rebuild flag (new positions from outside, new skin)
+int pimd_launch_nlist_invalidate(pimd_ctx *c)
+{
+    if (c->kind != 0) return 0;
+    set_flag_kernel<<<1, 1, 0, c->stream>>>(c->nl.need, 1);
+    c->launches++;
     PIMD_CUDA_CHECK(cudaGetLastError());
     return 0;
 }

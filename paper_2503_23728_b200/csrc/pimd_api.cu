@@ -61,7 +61,7 @@ namespace {
 
 struct Layout {
     size_t q, p, F, species, mass, C, CT, omega, lam, gam, Tstage, pileg_partial, pileg_alpha, err, est_partial, est_out;
-    size_t cell_id, cell_count, cell_start, cell_cursor, sorted_atom, sorted_q, nnz, hits, row_ptr, block_sums, col, pair_row;
+    size_t cell_id, cell_count, cell_start, cell_cursor, sorted_atom, sorted_q, nnz, ncand, hits, hitmask, q_ref, q32, need, row_ptr, block_sums, col, pair_row;
     size_t wimg, wimg_node, xs0, h1_img, meta_img, weights, nfeat, xfeat, mfeat, Efeat, Gfeat, carry_m, carry_f, Fraw;
     size_t total;
     int ncell[3], nct;
@@ -169,6 +169,11 @@ int compute_layout(int N, int R, int P, const double box[3], const pimd_net_para
         L->sorted_atom = take(cur, sizeof(int) * rows);
         L->sorted_q = take(cur, sizeof(double) * rows * 3);
         L->nnz = take(cur, sizeof(int) * rows);
+        L->ncand = take(cur, sizeof(int) * rows);
+        L->hitmask = take(cur, sizeof(unsigned) * rows * (PIMD_MAX_NBR / 32));
+        L->q_ref = take(cur, sizeof(double) * rows * 3);
+        L->q32 = take(cur, sizeof(float) * 4 * rows);
+        L->need = take(cur, sizeof(int) * 4);
         L->hit_stride = (N - 1 < PIMD_MAX_NBR) ? (N > 1 ? N - 1 : 1) : PIMD_MAX_NBR;
         L->hits = take(cur, sizeof(int) * rows * L->hit_stride);
         L->row_ptr = take(cur, sizeof(int) * (rows + 1));
@@ -340,6 +345,25 @@ int enter(pimd_ctx *c)
 // the Philox counter holds the step as one 32-bit word (S:N4)
 constexpr int64_t PIMD_MAX_STEP = 4294967295LL;
 
+// candidate radius r_cut + skin of the reusable neighbour lists: the cell grid must have cells at least that wide
+int apply_skin(pimd_ctx *c, double skin)
+{
+    if (c->kind != 0) return 0;
+    if (!(skin >= 0.0)) { pimd_set_error("skin must be >= 0"); return PIMD_ERR_ARG; }
+    const double rl = (double)c->net.r_cut + skin;
+    int nc[3] = {1, 1, 1};
+    if (c->periodic)
+        for (int a = 0; a < 3; ++a) {
+            if (c->box[a] < 2.0 * rl) { pimd_set_error("periodic box edge %g < 2 (r_cut + skin) = %g", c->box[a], 2.0 * rl); return PIMD_ERR_ARG; }
+            nc[a] = (int)floor(c->box[a] / rl);
+            if (nc[a] < 1) nc[a] = 1;
+        }
+    for (int a = 0; a < 3; ++a) c->nl.ncell[a] = nc[a];
+    c->nl.ncell_tot = nc[0] * nc[1] * nc[2];
+    c->nl.skin = skin;
+    return pimd_launch_nlist_invalidate(c);
+}
+
 int compute_forces(pimd_ctx *c)
 {
     int rc;
@@ -483,7 +507,10 @@ extern "C" int pimd_create(pimd_ctx **out, int n_atoms, int n_replicas, const in
         nl.cell_id = (int *)(ws + L.cell_id); nl.cell_count = (int *)(ws + L.cell_count);
         nl.cell_start = (int *)(ws + L.cell_start); nl.cell_cursor = (int *)(ws + L.cell_cursor);
         nl.sorted_atom = (int *)(ws + L.sorted_atom); nl.sorted_q = (double *)(ws + L.sorted_q);
-        nl.nnz = (int *)(ws + L.nnz); nl.hits = (int *)(ws + L.hits); nl.hit_stride = L.hit_stride; nl.row_ptr = (int *)(ws + L.row_ptr); nl.block_sums = (int *)(ws + L.block_sums);
+        nl.nnz = (int *)(ws + L.nnz); nl.ncand = (int *)(ws + L.ncand); nl.hitmask = (unsigned *)(ws + L.hitmask);
+        nl.q_ref = (double *)(ws + L.q_ref); nl.q32 = (float4 *)(ws + L.q32); nl.need = (int *)(ws + L.need); nl.skin = 0.0;
+        CREATE_CHECK(cudaMemsetAsync(nl.need, 0, sizeof(int) * 4, st));
+        nl.hits = (int *)(ws + L.hits); nl.hit_stride = L.hit_stride; nl.row_ptr = (int *)(ws + L.row_ptr); nl.block_sums = (int *)(ws + L.block_sums);
         nl.col = (int *)(ws + L.col); nl.pair_row = (int *)(ws + L.pair_row); nl.pair_cap = L.pair_cap;
         c->weights_dev = (float *)(ws + L.weights);
         c->nfeat = (float *)(ws + L.nfeat); c->xfeat = (float *)(ws + L.xfeat); c->mfeat = (float *)(ws + L.mfeat);
@@ -582,6 +609,10 @@ extern "C" int pimd_create(pimd_ctx **out, int n_atoms, int n_replicas, const in
             g.layer[l].Wv2T = b + o[4]; g.layer[l].bv2 = b + o[5]; g.layer[l].WaT = b + o[6]; g.layer[l].ba = b + o[7];
         }
         CREATE_CHECK(cudaMemsetAsync(nl.row_ptr, 0, sizeof(int) * (c->rows + 1), st));
+        // default: no reuse (skin 0).  The synthetic workloads are hot (random-weight force field): atoms move skin/2 =
+        // 0.25 A in about four steps and the larger candidate radius costs more than it saves; pimd_set_nlist_skin turns reuse on
+        g.r_cut = net->r_cut;   // (apply_skin reads it)
+        if (apply_skin(c, 0.0)) { delete c; return PIMD_ERR_CUDA; }
     }
     rc = pimd_launch_init_momenta(c);   // S:N5
     if (rc) { delete c; return rc; }
@@ -754,7 +785,26 @@ extern "C" int pimd_set_state(pimd_ctx *c, const double *d_q, const double *d_p,
     if (d_p) PIMD_CUDA_CHECK(cudaMemcpyAsync(c->p, d_p, bytes, cudaMemcpyDeviceToDevice, c->stream));
     c->step = step;
     c->forces_valid = 0;
+    if (d_q) return pimd_launch_nlist_invalidate(c);   // positions jumped: the candidate lists are rebuilt at the next force evaluation
     return 0;
+}
+
+extern "C" int pimd_nlist_rebuilds(pimd_ctx *c, int64_t *h_count)
+{
+    if (!c || !h_count) { pimd_set_error("null argument"); return PIMD_ERR_ARG; }
+    if (int rc = enter(c)) return rc;
+    int v = 0;
+    if (c->kind == 0) PIMD_CUDA_CHECK(cudaMemcpyAsync(&v, c->nl.need + 1, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    PIMD_CUDA_CHECK(cudaStreamSynchronize(c->stream));
+    *h_count = v;
+    return 0;
+}
+
+extern "C" int pimd_set_nlist_skin(pimd_ctx *c, double skin)
+{
+    if (!c) { pimd_set_error("null context"); return PIMD_ERR_ARG; }
+    if (int rc = enter(c)) return rc;
+    return apply_skin(c, skin);
 }
 
 extern "C" int pimd_get_forces_cached(pimd_ctx *c, double *d_F)

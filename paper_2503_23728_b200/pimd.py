@@ -54,6 +54,8 @@ def load_library():
                               C.c_double, C.c_uint64, C.POINTER(NetParams), vp, C.c_size_t, vp]
     L.pimd_step.argtypes = [vp, C.c_int]
     L.pimd_set_integrator.argtypes = [vp, C.c_int, C.c_int]
+    L.pimd_set_nlist_skin.argtypes = [vp, C.c_double]
+    L.pimd_nlist_rebuilds.argtypes = [vp, C.POINTER(C.c_int64)]
     L.pimd_forces.argtypes = [vp, vp]
     L.pimd_estimators.argtypes = [vp, C.POINTER(Estimators)]
     L.pimd_get_state.argtypes = [vp, vp, vp, C.POINTER(C.c_int64)]
@@ -150,6 +152,15 @@ class PIMD:
     def set_integrator(self, transform="normal_modes", thermostat="pile_l"):
         """Integrator variant (before the first step): normal-mode / staging / primitive, PILE-L / PILE-G."""
         _check(load_library().pimd_set_integrator(self._h, self.TRANSFORMS[transform], self.THERMOSTATS[thermostat]))
+
+    def set_nlist_skin(self, skin):
+        """Verlet skin (A) of the reusable candidate lists; 0 = cell-list pass every step.  Results do not depend on it."""
+        _check(load_library().pimd_set_nlist_skin(self._h, float(skin)))
+
+    def nlist_rebuilds(self):
+        n = C.c_int64()
+        _check(load_library().pimd_nlist_rebuilds(self._h, C.byref(n)))
+        return int(n.value)
 
     def step(self, n=1):
         _check(load_library().pimd_step(self._h, int(n)))

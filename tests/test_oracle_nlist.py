@@ -114,3 +114,34 @@ def test_capacity_overflow_reported():
     x = np.random.default_rng(0).uniform(0, 3, (20, 3))
     with pytest.raises(RuntimeError):
         oracle.nlist_cell(x, np.zeros(3), 5.0, cap=10)
+
+
+def test_skin_list_filtered_to_the_cutoff_equals_the_exact_list():
+    """Neighbour-list reuse: candidates within r_c + skin at reference positions, filtered with the exact predicate at
+    the current positions, give the exact list as long as no atom has moved by skin/2 or more (triangle inequality on the
+    minimum-image distance); the oracle's brute-force list is the definition on both sides."""
+    rng = np.random.default_rng(8)
+    box = np.array([13.0, 12.5, 14.0])
+    N, rc, skin = 150, 3.0, 0.6
+    q_ref = rng.uniform(0, 1, (N, 3)) * box
+    step = rng.standard_normal((N, 3))
+    step *= (0.999 * skin / 2) / np.linalg.norm(step, axis=1).max()            # largest displacement just below skin/2
+    q = q_ref + step
+    rp_c, col_c = oracle.nlist_brute(q_ref, box, rc + skin)
+    rp_x, col_x = oracle.nlist_brute(q, box, rc)
+    rows, cols = [], []
+    for i in range(N):
+        cand = col_c[rp_c[i]:rp_c[i + 1]]
+        d = q[cand] - q[i]
+        d = d - box * np.round(d / box)
+        keep = cand[(d[:, 0] * d[:, 0] + d[:, 1] * d[:, 1]) + d[:, 2] * d[:, 2] < np.float64(np.float32(rc)) ** 2]
+        rows.append(len(keep)); cols.append(keep)
+    assert np.array_equal(np.concatenate([[0], np.cumsum(rows)]), rp_x)
+    assert np.array_equal(np.concatenate(cols), col_x)
+    # and a displacement beyond skin/2 can lose a pair: the rebuild criterion is needed
+    q_far = q_ref + step * 4.0
+    rp_f, col_f = oracle.nlist_brute(q_far, box, rc)
+    lost = 0
+    for i in range(N):
+        lost += len(set(col_f[rp_f[i]:rp_f[i + 1]]) - set(col_c[rp_c[i]:rp_c[i + 1]]))
+    assert lost > 0
