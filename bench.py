@@ -33,7 +33,7 @@ import pimd_inputs as pi  # noqa: E402
 
 METRIC = "pimd_atom_bead_steps_per_s"
 UNIT = "atom*bead*steps/s"
-FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12  # 74.4: SMs x FP32 lanes x 2 (FMA) x clocks.max.sm
+FP32_NOMINAL_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12  # 74.4: SMs x FP32 lanes x 2 (FMA) x clocks.max.sm; the roofline uses the MEASURED rate
 
 
 def measured_peaks():
@@ -167,9 +167,23 @@ def cpu_baseline(w, budget_beads):
         if time.perf_counter() - t0 > 10.0 or n >= 200:
             break
     dt = time.perf_counter() - t0
-    return {"value": w.n_atoms * P_s * n / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
-            "sample": f"{n} oracle step(s) of {w.name} restricted to the first {P_s} of {w.P} bead-systems "
-                      f"({w.n_atoms} atoms each), {dt:.1f} s"}
+    out = {"value": w.n_atoms * P_s * n / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+           "sample": f"{n} oracle step(s) of {w.name} restricted to the first {P_s} of {w.P} bead-systems "
+                     f"({w.n_atoms} atoms each), {dt:.1f} s"}
+    # the same oracle on ONE thread (OMP_NUM_THREADS = 1 and = all cores), a shorter sample
+    threads = oracle.num_threads()
+    oracle.set_num_threads(1)
+    t0 = time.perf_counter()
+    n1 = 0
+    while True:
+        ref.step(1)
+        n1 += 1
+        if time.perf_counter() - t0 > 5.0 or n1 >= 200:
+            break
+    dt1 = time.perf_counter() - t0
+    oracle.set_num_threads(threads)
+    out["single_thread"] = {"value": w.n_atoms * P_s * n1 / dt1, "cores": 1, "sample": f"{n1} step(s), {dt1:.1f} s"}
+    return out
 
 
 # ------------------------------------------------------------------------------------------------
@@ -211,20 +225,30 @@ def run_ours(args):
     if rank == 0:
         sampler.start()
     l0 = sim.launch_count()
-    sim.profile(True)
     wall0 = time.perf_counter()
-    for a, b in ev:
+    for a, b in ev:                      # the timed region: the library replays its captured step (CUDA graph)
         flush.add_(1.0)
         a.record(stream)
         sim.step(1)
         b.record(stream)
     barrier()
     wall = time.perf_counter() - wall0
-    prof = sim.profile_read()
-    sim.profile(False)
     launches = sim.launch_count() - l0
     clocks = sampler.stop() if rank == 0 else None
     t_dev = sum(a.elapsed_time(b) for a, b in ev) * 1e-3
+    # the same K steps again with the library's per-class CUDA events (plain launches: events cannot be timed inside a graph):
+    # kernel_ms_per_step and the roofline's launch durations come from this pass
+    ev2 = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    sim.profile(True)
+    for a, b in ev2:
+        flush.add_(1.0)
+        a.record(stream)
+        sim.step(1)
+        b.record(stream)
+    barrier()
+    prof = sim.profile_read()
+    sim.profile(False)
+    t_prof = sum(a.elapsed_time(b) for a, b in ev2) * 1e-3
     sim.sync()
     rp1, _ = sim.nlist()
     pairs_last = int(rp1[-1].item())
@@ -281,8 +305,9 @@ def run_ours(args):
                            else "B200_PROFILING.md sustained fallback 1.4 PFLOP/s (of fallback)")
             kname = "gfn_pipe::pair_pipe_kernel (message + head passes, tcgen05)"
         else:
-            bound, peak = "alu", FP32_PEAK_TFLOPS
-            peak_source = "derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (MEASURED_PEAKS has no fp32 figure)"
+            bound, peak = "alu", pb.measure_fp32_fma_tflops(stream)
+            peak_source = (f"measured in this run: FMA-chain micro-kernel (pimd_measure_fp32_fma_tflops; nominal 148 SM x 128 lanes x 2 x "
+                           f"1.965 GHz = {FP32_NOMINAL_TFLOPS:.1f})")
             kname = "gfn::pair_kernel (message + head passes, fp32 FFMA)"
         hbm = float(mp["hbm_gbs"]) if mp and "hbm_gbs" in mp else 6650.0
         # HBM-bound kernel classes: algorithmic bytes per step / measured ms per step
@@ -309,7 +334,10 @@ def run_ours(args):
                        "rows_per_gpu": w.rows, "n_rbf": K, "hidden": H, "layers": L, "r_cut": w.net.r_cut,
                        "pairs_per_row_first": pairs_first / w.rows, "pairs_per_row_last": pairs_last / w.rows,
                        "l2": "512 MB buffer rewritten between timed steps (flush)", "parallelism": f"replicas x{world}",
-                       "timing": "sum of per-step CUDA-event intervals on the launch stream"},
+                       "timing": "sum of per-step CUDA-event intervals on the launch stream; the library replays one captured step (CUDA graph); "
+                                 "kernel_ms_per_step and the roofline durations come from a second pass of the same K steps with the library's "
+                                 "per-class events (plain launches)"},
+            "ms_per_step_profiled_pass": 1e3 * t_prof / args.steps,
             "ns_per_day": args.steps / t_dev * w.dt * 86400e-6,
             "wall_ms_per_step_incl_flush": 1e3 * wall / args.steps,
             "e2e": {"value": whole_job_value(w.rows, e2e_steps, world, t_e2e), "unit": UNIT, "h2d_bytes_per_step": state_bytes,
@@ -339,13 +367,22 @@ def run_ours(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
-    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=20, help="untimed steps before the timed window (SURVEY D5: the beads start collapsed)")
     ap.add_argument("--workload", default="ice512", choices=pi.workload_names())
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--ref-beads", type=int, default=2, help="bead-systems in the oracle's bounded sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # started as a plain `python bench.py --gpus N`: start the N ranks ourselves (one process per GPU; torch.distributed.run)
+        import socket
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+               "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        sys.exit(subprocess.call(cmd))
     if args.impl == "reference":
         if int(os.environ.get("RANK", "0")) == 0:
             run_reference(args)

@@ -169,6 +169,11 @@ int pimd_sync(pimd_ctx *ctx);
 int pimd_profile(pimd_ctx *ctx, int enable);
 int pimd_profile_read(pimd_ctx *ctx, double *h_ms, int64_t *h_launches);
 
+/* Measurement helper (no context needed): the FP32 fused-multiply-add rate of the current device in TFLOP/s, measured with a
+ * kernel of independent FMA chains (best of six launches, CUDA events on `cuda_stream`).  It is the denominator of the "alu"
+ * roofline of the fp32 pair kernel (the benchmark must measure it).  h_tflops HOST.  Synchronises. */
+int pimd_measure_fp32_fma_tflops(void *cuda_stream, double *h_tflops);
+
 /* Number of kernels the library has launched on this context so far (HOST counter). */
 int64_t pimd_launch_count(const pimd_ctx *ctx);
 

@@ -13,6 +13,7 @@ from .ref import (  # noqa: F401
     nlist_brute,
     nlist_cell,
     num_threads,
+    set_num_threads,
     KB_EV,
     HBAR_EVFS,
     AMU_INTERNAL,

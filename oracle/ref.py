@@ -65,6 +65,8 @@ def lib():
         L.ref_n_weights.argtypes = [C.c_int] * 4
         L.ref_n_weights.restype = C.c_int64
         L.ref_num_threads.restype = C.c_int
+        L.ref_set_num_threads.argtypes = [C.c_int]
+        L.ref_set_num_threads.restype = None
         _lib = L
     return _lib
 
@@ -84,6 +86,11 @@ def stage_map(name, v):
 
 def _ip(a):
     return a.ctypes.data_as(C.POINTER(C.c_int32))
+
+
+def set_num_threads(n: int) -> None:
+    """OpenMP threads of the oracle (bench.py's single-thread leg)."""
+    lib().ref_set_num_threads(int(n))
 
 
 def num_threads() -> int:

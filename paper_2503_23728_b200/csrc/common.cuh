@@ -74,7 +74,7 @@ struct pimd_ctx {
     double harmonic_omega;
     cudaStream_t stream;
     int forces_valid;
-    int64_t launches;
+    int64_t launches, launches_per_step;
     int num_sms;
     int device;                        // CUDA device the workspace and stream belong to (set current at every entry point)
     unsigned attr_done;                // per-context (= per-device) bits: opt-in shared-memory attribute set for a kernel family
@@ -90,6 +90,10 @@ struct pimd_ctx {
     double *omega_k, *lam_k, *gam_k;   // [P] mode frequency, mass factor, friction
     double *pileg_partial, *pileg_alpha;   // [R][64][2], [R]
     int *err;                          // [4] device error word
+    uint32_t *step_dev;                // device copy of the step counter (read by the noise kernels: a captured step does not depend on it)
+    cudaGraphExec_t step_graph;        // one whole step, captured at the first pimd_step (null: not captured yet)
+    int graph_state;                   // 0 not tried, 1 captured, -1 capture not available
+    int warm;                          // a step has run with plain launches (every lazy kernel attribute is set)
     double *est_partial;               // [R][EST_BLOCKS][8]
     double *est_out;                   // [R][8]
     NlistDev nl;
@@ -137,8 +141,9 @@ void pimd_set_error(const char *fmt, ...);
 
 // kernel launchers (each returns 0 or PIMD_ERR_CUDA)
 int pimd_launch_init_momenta(pimd_ctx *c);
-int pimd_launch_nm_pre(pimd_ctx *c, uint32_t t);
-int pimd_launch_nm_post(pimd_ctx *c, uint32_t t);
+int pimd_launch_nm_pre(pimd_ctx *c);                 // O B A with the noise of step *step_dev
+int pimd_launch_step_inc(pimd_ctx *c);               // *step_dev += 1
+int pimd_launch_nm_post(pimd_ctx *c);                // B O with the noise of step *step_dev - 1
 int pimd_launch_simple_forces(pimd_ctx *c);          // kinds 1, 2
 int pimd_launch_estimators(pimd_ctx *c);
 int pimd_launch_nlist(pimd_ctx *c);

@@ -110,9 +110,16 @@ __device__ __forceinline__ double spring_force(const NmArgs &a, const double *bQ
 }
 
 // mode: 0 = pre (O,B,A), 1 = post (B,O), 2 = initial momenta (S:N5)
+// The step index of the noise counter is read from device memory (t = *t_dev - t_off; null = 0), so that the launch sequence
+// of one step does not depend on the step and can be captured once as a CUDA graph and replayed.
+__device__ __forceinline__ uint32_t step_of(const uint32_t *t_dev, uint32_t t_off) { return t_dev ? *t_dev - t_off : 0u; }
+
+__global__ void step_inc_kernel(uint32_t *t_dev) { *t_dev += 1u; }
+
 template <int MODE>
-__global__ void __launch_bounds__(32 * NM_TY) nm_kernel(NmArgs a, uint32_t t)
+__global__ void __launch_bounds__(32 * NM_TY) nm_kernel(NmArgs a, const uint32_t *t_dev, uint32_t t_off)
 {
+    const uint32_t t = step_of(t_dev, t_off);
     extern __shared__ double sm[];
     const int P = a.P, TC = a.TC;
     double *bP = sm, *bT = sm + (size_t)P * TC, *bQ = bT + (size_t)P * TC, *bQ2 = bQ + (size_t)P * TC;
@@ -216,8 +223,9 @@ __global__ void __launch_bounds__(32 * NM_TY) nm_kernel(NmArgs a, uint32_t t)
 //   sign(alpha) = sign(R1 + sqrt(2 beta_P K c / (1 - c)))           (stochastic velocity rescaling, exact for the half-step)
 constexpr int PG_BLOCKS = 64, PG_THREADS = 128;
 
-__global__ void __launch_bounds__(PG_THREADS) pileg_partial_kernel(NmArgs a, uint32_t t, uint32_t tag, int after_B, double *__restrict__ partial)
+__global__ void __launch_bounds__(PG_THREADS) pileg_partial_kernel(NmArgs a, const uint32_t *t_dev, uint32_t t_off, uint32_t tag, int after_B, double *__restrict__ partial)
 {
+    const uint32_t t = step_of(t_dev, t_off);
     __shared__ double red[2][PG_THREADS];
     const int r = blockIdx.y, P = a.P, ncol = 3 * a.N;
     const double hdt = 0.5 * a.dt;
@@ -246,8 +254,9 @@ __global__ void __launch_bounds__(PG_THREADS) pileg_partial_kernel(NmArgs a, uin
     if (threadIdx.x < 2) partial[((size_t)r * PG_BLOCKS + blockIdx.x) * 2 + threadIdx.x] = red[threadIdx.x][0];
 }
 
-__global__ void pileg_final_kernel(NmArgs a, uint32_t t, uint32_t tag, const double *__restrict__ partial, double *__restrict__ alpha)
+__global__ void pileg_final_kernel(NmArgs a, const uint32_t *t_dev, uint32_t t_off, uint32_t tag, const double *__restrict__ partial, double *__restrict__ alpha)
 {
+    const uint32_t t = step_of(t_dev, t_off);
     const int r = blockIdx.x * blockDim.x + threadIdx.x;
     if (r >= a.R) return;
     double K = 0.0, S = 0.0;
@@ -278,22 +287,24 @@ NmArgs make_args(const pimd_ctx *c)
 }
 
 template <int MODE>
-int launch_nm(pimd_ctx *c, uint32_t t)
+int launch_nm(pimd_ctx *c, const uint32_t *t_dev, uint32_t t_off)
 {
     NmArgs a = make_args(c);
     if (MODE != 2 && c->thermostat == 1 && c->gamma_fs >= 0.0) {   // PILE-G: the replica's scale factor for this half-step
         const uint32_t tag = MODE == 0 ? 0u : 1u;
-        pileg_partial_kernel<<<dim3(PG_BLOCKS, c->R), PG_THREADS, 0, c->stream>>>(a, t, tag, MODE == 1 ? 1 : 0, c->pileg_partial);
-        pileg_final_kernel<<<(c->R + 127) / 128, 128, 0, c->stream>>>(a, t, tag, c->pileg_partial, c->pileg_alpha);
+        pileg_partial_kernel<<<dim3(PG_BLOCKS, c->R), PG_THREADS, 0, c->stream>>>(a, t_dev, t_off, tag, MODE == 1 ? 1 : 0, c->pileg_partial);
+        pileg_final_kernel<<<(c->R + 127) / 128, 128, 0, c->stream>>>(a, t_dev, t_off, tag, c->pileg_partial, c->pileg_alpha);
         c->launches += 2;
     }
     size_t smem = (size_t)4 * c->P * a.TC * sizeof(double);
-    if (!(c->attr_done & (ATTR_NM << MODE))) {
-        PIMD_CUDA_CHECK(cudaFuncSetAttribute(nm_kernel<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-        c->attr_done |= (ATTR_NM << MODE);
+    if (!(c->attr_done & ATTR_NM)) {   // all three variants at once (no attribute call inside a stream capture)
+        PIMD_CUDA_CHECK(cudaFuncSetAttribute(nm_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+        PIMD_CUDA_CHECK(cudaFuncSetAttribute(nm_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+        PIMD_CUDA_CHECK(cudaFuncSetAttribute(nm_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+        c->attr_done |= ATTR_NM;
     }
     dim3 grid((3 * c->N + a.TC - 1) / a.TC, c->R), block(a.TC, NM_TY);
-    nm_kernel<MODE><<<grid, block, smem, c->stream>>>(a, t);
+    nm_kernel<MODE><<<grid, block, smem, c->stream>>>(a, t_dev, t_off);
     c->launches++;
     PIMD_CUDA_CHECK(cudaGetLastError());
     return 0;
@@ -376,9 +387,17 @@ __global__ void estimators_final_kernel(int R, int N, int P, int kind, double kT
 
 }  // namespace
 
-int pimd_launch_init_momenta(pimd_ctx *c) { return launch_nm<2>(c, 0u); }
-int pimd_launch_nm_pre(pimd_ctx *c, uint32_t t) { return launch_nm<0>(c, t); }
-int pimd_launch_nm_post(pimd_ctx *c, uint32_t t) { return launch_nm<1>(c, t); }
+int pimd_launch_init_momenta(pimd_ctx *c) { return launch_nm<2>(c, nullptr, 0u); }
+// the device step counter holds t before pimd_launch_step_inc and t + 1 after it
+int pimd_launch_nm_pre(pimd_ctx *c) { return launch_nm<0>(c, c->step_dev, 0u); }
+int pimd_launch_nm_post(pimd_ctx *c) { return launch_nm<1>(c, c->step_dev, 1u); }
+int pimd_launch_step_inc(pimd_ctx *c)
+{
+    step_inc_kernel<<<1, 1, 0, c->stream>>>(c->step_dev);
+    c->launches++;
+    PIMD_CUDA_CHECK(cudaGetLastError());
+    return 0;
+}
 
 int pimd_launch_simple_forces(pimd_ctx *c)
 {

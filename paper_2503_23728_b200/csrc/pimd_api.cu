@@ -345,10 +345,18 @@ int enter(pimd_ctx *c)
 // the Philox counter holds the step as one 32-bit word (S:N4)
 constexpr int64_t PIMD_MAX_STEP = 4294967295LL;
 
+// a captured step bakes in the kernel arguments: anything that changes them drops the graph (it is captured again on demand)
+void drop_step_graph(pimd_ctx *c)
+{
+    if (c->step_graph) { cudaStreamSynchronize(c->stream); cudaGraphExecDestroy(c->step_graph); c->step_graph = nullptr; }
+    c->graph_state = 0;
+}
+
 // candidate radius r_cut + skin of the reusable neighbour lists: the cell grid must have cells at least that wide
 int apply_skin(pimd_ctx *c, double skin)
 {
     if (c->kind != 0) return 0;
+    drop_step_graph(c);
     if (!(skin >= 0.0)) { pimd_set_error("skin must be >= 0"); return PIMD_ERR_ARG; }
     const double rl = (double)c->net.r_cut + skin;
     int nc[3] = {1, 1, 1};
@@ -453,6 +461,7 @@ extern "C" int pimd_create(pimd_ctx **out, int n_atoms, int n_replicas, const in
     c->transform = 0; c->thermostat = 0;
     c->Tq_fwd = c->CmatT; c->Tp_fwd = c->CmatT; c->Tq_inv = c->Cmat; c->Tp_inv = c->Cmat;   // normal modes: orthogonal
     c->err = (int *)(ws + L.err);
+    c->step_dev = (uint32_t *)(c->err + 2);          // (words 2, 3 of the error block)
     c->est_partial = (double *)(ws + L.est_partial); c->est_out = (double *)(ws + L.est_out);
 
     // host staging
@@ -484,7 +493,7 @@ extern "C" int pimd_create(pimd_ctx **out, int n_atoms, int n_replicas, const in
         }                                                                                   \
     } while (0)
     cudaStream_t st = c->stream;
-    CREATE_CHECK(cudaMemsetAsync(c->err, 0, sizeof(int) * 4, st));
+    CREATE_CHECK(cudaMemsetAsync(c->err, 0, sizeof(int) * 4, st));   // error word, step counter
     CREATE_CHECK(cudaMemsetAsync(c->F, 0, sizeof(double) * c->rows * 3, st));
     CREATE_CHECK(cudaMemcpyAsync(c->q, q0.data(), sizeof(double) * q0.size(), cudaMemcpyHostToDevice, st));
     CREATE_CHECK(cudaMemcpyAsync(c->species, species, sizeof(int) * N, cudaMemcpyHostToDevice, st));
@@ -628,6 +637,7 @@ extern "C" void pimd_destroy(pimd_ctx *c)
     if (!c) return;
     (void)enter(c);
     cudaStreamSynchronize(c->stream);
+    if (c->step_graph) cudaGraphExecDestroy(c->step_graph);
     if (c->prof) {
         c->prof->clear();
         for (auto e : c->prof->pool) cudaEventDestroy(e);
@@ -712,8 +722,35 @@ extern "C" int pimd_set_integrator(pimd_ctx *c, int transform, int thermostat)
     PIMD_CUDA_CHECK(cudaMemcpyAsync(c->gam_k, gam.data(), sizeof(double) * P, cudaMemcpyHostToDevice, c->stream));
     PIMD_CUDA_CHECK(cudaStreamSynchronize(c->stream));
     c->transform = transform; c->thermostat = thermostat;
+    drop_step_graph(c);
     return pimd_launch_init_momenta(c);   // S:N5 in the chosen representation
 }
+
+namespace {
+
+// one step: O B A | step counter | neighbour list + forces | B O   (S:N3); nothing in the launch sequence depends on the step
+int step_body(pimd_ctx *c)
+{
+    int rc;
+    {
+        ProfScope ps(c, PROF_NM);
+        if ((rc = pimd_launch_nm_pre(c))) return rc;
+        if ((rc = pimd_launch_step_inc(c))) return rc;
+    }
+    if ((rc = compute_forces(c))) return rc;
+    ProfScope ps(c, PROF_NM);
+    return pimd_launch_nm_post(c);
+}
+
+int sync_step_counter(pimd_ctx *c)
+{
+    const uint32_t t = (uint32_t)c->step;
+    PIMD_CUDA_CHECK(cudaMemcpyAsync(c->step_dev, &t, sizeof(t), cudaMemcpyHostToDevice, c->stream));
+    PIMD_CUDA_CHECK(cudaStreamSynchronize(c->stream));   // (t is a stack variable)
+    return 0;
+}
+
+}  // namespace
 
 extern "C" int pimd_step(pimd_ctx *c, int n)
 {
@@ -721,17 +758,32 @@ extern "C" int pimd_step(pimd_ctx *c, int n)
     if (c->step + n > PIMD_MAX_STEP) { pimd_set_error("step counter would exceed 2^32 - 1 (the noise counter holds 32 bits)"); return PIMD_ERR_ARG; }
     int rc;
     if ((rc = enter(c))) return rc;
-    if (!c->forces_valid && (rc = compute_forces(c))) return rc;
+    if (!c->forces_valid && (rc = compute_forces(c))) return rc;   // (also sets every opt-in kernel attribute before a capture)
+    const bool profiling = c->prof && c->prof->on;
+    // The launch sequence of a step is captured once as a CUDA graph and replayed: the small configurations are bound by
+    // launch overhead (17-35 launches per step).  Per-class event timing (pimd_profile) needs the plain launches.
     for (int s = 0; s < n; ++s) {
-        const uint32_t t = (uint32_t)c->step;
-        {
-            ProfScope ps(c, PROF_NM);
-            if ((rc = pimd_launch_nm_pre(c, t))) return rc;     // O(dt/2) B(dt/2) A(dt)
+        if (!profiling && c->graph_state == 0 && c->warm) {   // (the first step of a context runs uncaptured: lazy kernel attributes)
+            c->graph_state = -1;
+            cudaGraph_t g = nullptr;
+            const int64_t launches0 = c->launches;
+            if (cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+                rc = step_body(c);
+                const cudaError_t e = cudaStreamEndCapture(c->stream, &g);
+                c->launches_per_step = c->launches - launches0;
+                c->launches = launches0;
+                if (rc == 0 && e == cudaSuccess && g && cudaGraphInstantiate(&c->step_graph, g, 0) == cudaSuccess) c->graph_state = 1;
+                if (g) cudaGraphDestroy(g);
+            }
+            (void)cudaGetLastError();
         }
-        if ((rc = compute_forces(c))) return rc;            // neighbour list + forces at the new positions
-        {
-            ProfScope ps(c, PROF_NM);
-            if ((rc = pimd_launch_nm_post(c, t))) return rc;    // B(dt/2) O(dt/2)
+        if (!profiling && c->graph_state == 1) {
+            PIMD_CUDA_CHECK(cudaGraphLaunch(c->step_graph, c->stream));
+            c->launches += c->launches_per_step;
+            c->forces_valid = 1;
+        } else {
+            if ((rc = step_body(c))) return rc;
+            c->warm = 1;
         }
         c->step += 1;
     }
@@ -785,6 +837,7 @@ extern "C" int pimd_set_state(pimd_ctx *c, const double *d_q, const double *d_p,
     if (d_p) PIMD_CUDA_CHECK(cudaMemcpyAsync(c->p, d_p, bytes, cudaMemcpyDeviceToDevice, c->stream));
     c->step = step;
     c->forces_valid = 0;
+    if (int rc = sync_step_counter(c)) return rc;
     if (d_q) return pimd_launch_nlist_invalidate(c);   // positions jumped: the candidate lists are rebuilt at the next force evaluation
     return 0;
 }

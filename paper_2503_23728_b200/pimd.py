@@ -66,6 +66,7 @@ def load_library():
     L.pimd_sync.argtypes = [vp]
     L.pimd_profile.argtypes = [vp, C.c_int]
     L.pimd_profile_read.argtypes = [vp, dp, C.POINTER(C.c_int64)]
+    L.pimd_measure_fp32_fma_tflops.argtypes = [vp, dp]
     L.pimd_launch_count.argtypes = [vp]
     L.pimd_launch_count.restype = C.c_int64
     L.pimd_last_error.restype = C.c_char_p
@@ -73,6 +74,15 @@ def load_library():
     L.pimd_destroy.restype = None
     _lib = L
     return L
+
+
+def measure_fp32_fma_tflops(stream=None) -> float:
+    """Measured FP32 FMA rate of the current CUDA device (TFLOP/s); see include/pimd.h."""
+    import torch
+    st = stream if stream is not None else torch.cuda.current_stream()
+    v = C.c_double()
+    _check(load_library().pimd_measure_fp32_fma_tflops(C.c_void_p(st.cuda_stream), C.byref(v)))
+    return float(v.value)
 
 
 def _check(rc):
