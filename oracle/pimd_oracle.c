@@ -74,6 +74,14 @@ typedef struct {
     double *C;         /* [P][P], C[j*P+k], bead j, mode k */
     double *omega_k;   /* [P] */
     int forces_valid;
+    /* well-tempered metadynamics: one bias V_G(s) per replica, felt by every bead */
+    int md_cv;                   /* 0 off, 1 s_dimer, 2 Debye XRD intensity */
+    int md_atoms[6];             /* s_dimer: O1, H1, O2, O4, H2, O3 */
+    double md_f[16], md_Q;       /* Debye: scattering factor per species, Q = 4 pi sin(theta) / lambda */
+    double md_sigma, md_w0, md_biasf;
+    int md_every, md_max, *md_n; /* deposition stride (steps), capacity, Gaussians deposited per replica [R] */
+    double *md_c, *md_h;         /* [R][md_max] centres and heights */
+    double *md_s, *md_ds;        /* [R][P] CV of every bead; [R][P][N][3] its gradient */
     int transform;  /* 0 normal modes (N2), 1 staging, 2 primitive (no transformation, explicit spring forces) */
     int thermostat; /* 0 PILE-L / white-noise Langevin, 1 PILE-G (global velocity rescaling of the free mode) */
 } ref_ctx;
@@ -370,6 +378,109 @@ static void gfn_forces_system(const ref_ctx *c, const double *q, const int32_t *
 /* pair capacity used internally for one bead-system */
 static int64_t sys_pair_cap(const ref_ctx *c) { return (int64_t)c->N * (c->N - 1) + 1; }
 
+/* ------------------------------------------------------------------ */
+/* well-tempered metadynamics with the paper's two collective variables                            */
+/* ------------------------------------------------------------------ */
+/* P:L164  s_dimer = d(O1,H1) - d(O2,H1) + d(O4,H2) - d(O3,H2): distances of one bead-system (no periodic image: the dimer is an
+ * open cluster; with a box the minimum image is used).  grad adds +-(r_X - r_Y)/d to the six atoms. */
+static double md_dist(const ref_ctx *c, const double *qs, int x, int y, double u[3])
+{
+    double d2 = 0.0;
+    for (int a = 0; a < 3; ++a) {
+        double dx = qs[(size_t)x * 3 + a] - qs[(size_t)y * 3 + a];
+        if (c->periodic) dx = dx - c->box[a] * round(dx / c->box[a]);
+        u[a] = dx; d2 += dx * dx;
+    }
+    double d = sqrt(d2);
+    for (int a = 0; a < 3; ++a) u[a] /= d;
+    return d;
+}
+static double cv_dimer(const ref_ctx *c, const double *qs, double *grad)
+{
+    const int *t = c->md_atoms; /* O1, H1, O2, O4, H2, O3 */
+    const int pr[4][2] = {{t[0], t[1]}, {t[2], t[1]}, {t[3], t[4]}, {t[5], t[4]}};
+    const double sg[4] = {1.0, -1.0, 1.0, -1.0};
+    double s = 0.0;
+    memset(grad, 0, sizeof(double) * (size_t)c->N * 3);
+    for (int k = 0; k < 4; ++k) {
+        double u[3];
+        s += sg[k] * md_dist(c, qs, pr[k][0], pr[k][1], u);
+        for (int a = 0; a < 3; ++a) {
+            grad[(size_t)pr[k][0] * 3 + a] += sg[k] * u[a];
+            grad[(size_t)pr[k][1] * 3 + a] -= sg[k] * u[a];
+        }
+    }
+    return s;
+}
+/* P:L215, P:L450  s_water = (1/N) sum_i sum_j f_i f_j sin(Q R_ij) / (Q R_ij), the double sum over ALL ordered pairs including
+ * i = j (sinc(0) = 1), R_ij the minimum-image distance.  d/dr_i: the ordered pairs (i,j) and (j,i) both contain r_i. */
+static double cv_debye(const ref_ctx *c, const double *qs, double *grad)
+{
+    const int N = c->N;
+    double s = 0.0;
+    memset(grad, 0, sizeof(double) * (size_t)N * 3);
+    for (int i = 0; i < N; ++i) {
+        const double fi = c->md_f[c->species[i]];
+        for (int j = 0; j < N; ++j) {
+            const double fj = c->md_f[c->species[j]];
+            if (j == i) { s += fi * fj; continue; }
+            double u[3];
+            const double R = md_dist(c, qs, i, j, u), x = c->md_Q * R;
+            const double g = sin(x) / x;
+            s += fi * fj * g;
+            const double dg = (cos(x) - g) / R; /* d sinc(Q R) / dR */
+            for (int a = 0; a < 3; ++a) grad[(size_t)i * 3 + a] += 2.0 * fi * fj * dg * u[a] / (double)N;
+        }
+    }
+    return s / (double)N;
+}
+/* V_G(s) = sum_g h_g exp(-(s - c_g)^2 / (2 sigma^2))  (P:L140 with 2 sigma read as 2 sigma^2) and dV/ds */
+static double md_bias(const ref_ctx *c, int r, double s, double *dVds)
+{
+    double V = 0.0, dV = 0.0;
+    const double is2 = 1.0 / (c->md_sigma * c->md_sigma);
+    for (int g = 0; g < c->md_n[r]; ++g) {
+        const double d = s - c->md_c[(size_t)r * c->md_max + g];
+        const double e = c->md_h[(size_t)r * c->md_max + g] * exp(-0.5 * d * d * is2);
+        V += e; dV -= e * d * is2;
+    }
+    if (dVds) *dVds = dV;
+    return V;
+}
+/* the bias is a potential term like any other: every bead k feels F = -dV_G/ds(s_k) grad s(q_k) */
+static void metad_add_bias_forces(ref_ctx *c)
+{
+    const int N = c->N;
+    for (int r = 0; r < c->R; ++r)
+        for (int k = 0; k < c->P; ++k) {
+            const size_t sys = (size_t)r * c->P + k;
+            const double *qs = c->q + sys * N * 3;
+            double *gr = c->md_ds + sys * N * 3;
+            const double s = (c->md_cv == 1) ? cv_dimer(c, qs, gr) : cv_debye(c, qs, gr);
+            c->md_s[sys] = s;
+            double dV;
+            md_bias(c, r, s, &dV);
+            for (size_t t = 0; t < (size_t)N * 3; ++t) c->F[sys * N * 3 + t] -= dV * gr[t];
+        }
+}
+/* deposition: every md_every steps one Gaussian per bead at the bead's CV value, height
+ * (w0 / P) exp(-beta V_G(s_k) / (gamma - 1)) with V_G the bias BEFORE this deposition event and beta = 1 / k_B T */
+static void metad_deposit(ref_ctx *c)
+{
+    const double kT = KB_EV * c->T;
+    for (int r = 0; r < c->R; ++r) {
+        const int n0 = c->md_n[r];
+        double hs[1024];
+        for (int k = 0; k < c->P; ++k)
+            hs[k] = (c->md_w0 / c->P) * exp(-md_bias(c, r, c->md_s[(size_t)r * c->P + k], NULL) / (kT * (c->md_biasf - 1.0)));
+        for (int k = 0; k < c->P && n0 + k < c->md_max; ++k) {
+            c->md_c[(size_t)r * c->md_max + n0 + k] = c->md_s[(size_t)r * c->P + k];
+            c->md_h[(size_t)r * c->md_max + n0 + k] = hs[k];
+        }
+        c->md_n[r] = (n0 + c->P <= c->md_max) ? n0 + c->P : c->md_max;
+    }
+}
+
 static int compute_forces(ref_ctx *c)
 {
     const int N = c->N, nsys = c->R * c->P;
@@ -413,6 +524,7 @@ static int compute_forces(ref_ctx *c)
             free(rp); free(cl);
         }
     }
+    if (c->md_cv) metad_add_bias_forces(c);
     c->forces_valid = 1;
     return overflow ? -3 : 0;
 }
@@ -750,6 +862,12 @@ int ref_step(ref_ctx *c, int n)
             if (c->gamma_fs >= 0.0) step_O_general(c, t, 1u);
         }
         c->step += 1;
+        if (c->md_cv && c->md_every > 0 && c->step % c->md_every == 0) {
+            /* the Gaussians go in at the positions reached by this step; the forces F(q) of the state include them from here on */
+            metad_deposit(c);
+            rc = compute_forces(c);
+            if (rc) return rc;
+        }
     }
     return 0;
 }
@@ -863,6 +981,7 @@ void ref_destroy(ref_ctx *c)
 {
     if (!c) return;
     free(c->species); free(c->mass); free(c->q); free(c->p); free(c->F); free(c->Fgross); free(c->C); free(c->omega_k);
+    free(c->md_n); free(c->md_c); free(c->md_h); free(c->md_s); free(c->md_ds);
     if (c->net.kind == 0) {
         free(c->Emb); free(c->We1); free(c->be1); free(c->We2); free(c->be2);
         for (int l = 0; l < c->net.n_layers; ++l) {
@@ -972,6 +1091,54 @@ int ref_estimators(ref_ctx *c, ref_estimators_t *out)
         out[r].v_pot = (c->net.kind == 0) ? NAN : vpot / P;
         out[r].t_centroid = tc / (3.0 * N * KB_EV * P);
     }
+    return 0;
+}
+
+/* metadynamics API.  cv: 1 s_dimer (atoms6 = O1, H1, O2, O4, H2, O3), 2 Debye (f_species[S], Q).  Energies in eV. */
+int ref_metad_enable(ref_ctx *c, int cv, const int32_t *atoms6, const double *f_species, double Q, double sigma, double height_eV,
+                     double bias_factor, int deposit_every, int max_gaussians)
+{
+    if (!c || (cv != 1 && cv != 2) || !(sigma > 0.0) || !(bias_factor > 1.0) || deposit_every < 1 || max_gaussians < 1) return -1;
+    if (cv == 1) { if (!atoms6) return -1; for (int k = 0; k < 6; ++k) { if (atoms6[k] < 0 || atoms6[k] >= c->N) return -1; c->md_atoms[k] = atoms6[k]; } }
+    if (cv == 2) { if (!f_species || c->net.n_species > 16 || !(Q > 0.0)) return -1; for (int k = 0; k < c->net.n_species; ++k) c->md_f[k] = f_species[k]; c->md_Q = Q; }
+    c->md_cv = cv; c->md_sigma = sigma; c->md_w0 = height_eV; c->md_biasf = bias_factor; c->md_every = deposit_every; c->md_max = max_gaussians;
+    free(c->md_n); free(c->md_c); free(c->md_h); free(c->md_s); free(c->md_ds);
+    c->md_n = (int *)calloc((size_t)c->R, sizeof(int));
+    c->md_c = (double *)calloc((size_t)c->R * max_gaussians, sizeof(double));
+    c->md_h = (double *)calloc((size_t)c->R * max_gaussians, sizeof(double));
+    c->md_s = (double *)calloc((size_t)c->R * c->P, sizeof(double));
+    c->md_ds = (double *)calloc((size_t)c->R * c->P * c->N * 3, sizeof(double));
+    c->forces_valid = 0;
+    return 0;
+}
+/* CV of every bead [R][P] and its gradient [R][P][N][3] at the current positions; either may be NULL */
+int ref_metad_cv(ref_ctx *c, double *s_out, double *grad_out)
+{
+    if (!c || !c->md_cv) return -1;
+    int rc = compute_forces(c);
+    if (rc) return rc;
+    if (s_out) memcpy(s_out, c->md_s, sizeof(double) * (size_t)c->R * c->P);
+    if (grad_out) memcpy(grad_out, c->md_ds, sizeof(double) * (size_t)c->R * c->P * c->N * 3);
+    return 0;
+}
+/* deposited Gaussians of replica r: count; centres and heights into caller arrays of capacity cap */
+int ref_metad_gaussians(ref_ctx *c, int r, double *centres, double *heights, int cap)
+{
+    if (!c || !c->md_cv || r < 0 || r >= c->R) return -1;
+    const int n = c->md_n[r];
+    for (int g = 0; g < n && g < cap; ++g) { if (centres) centres[g] = c->md_c[(size_t)r * c->md_max + g]; if (heights) heights[g] = c->md_h[(size_t)r * c->md_max + g]; }
+    return n;
+}
+/* bias energy V_G(s) of replica r at a given CV value */
+double ref_metad_bias(ref_ctx *c, int r, double s) { return (c && c->md_cv && r >= 0 && r < c->R) ? md_bias(c, r, s, NULL) : 0.0; }
+/* one deposition event now (tests) */
+int ref_metad_deposit_now(ref_ctx *c)
+{
+    if (!c || !c->md_cv) return -1;
+    int rc = c->forces_valid ? 0 : compute_forces(c);
+    if (rc) return rc;
+    metad_deposit(c);
+    c->forces_valid = 0;
     return 0;
 }
 

@@ -53,6 +53,12 @@ def lib():
         L.ref_destroy.restype = None
         L.ref_step.argtypes = [C.c_void_p, C.c_int]
         L.ref_set_integrator.argtypes = [C.c_void_p, C.c_int, C.c_int]
+        L.ref_metad_enable.argtypes = [C.c_void_p, C.c_int, ip, dp, C.c_double, C.c_double, C.c_double, C.c_double, C.c_int, C.c_int]
+        L.ref_metad_cv.argtypes = [C.c_void_p, dp, dp]
+        L.ref_metad_gaussians.argtypes = [C.c_void_p, C.c_int, dp, dp, C.c_int]
+        L.ref_metad_bias.argtypes = [C.c_void_p, C.c_int, C.c_double]
+        L.ref_metad_bias.restype = C.c_double
+        L.ref_metad_deposit_now.argtypes = [C.c_void_p]
         for f in (L.ref_stage_fwd, L.ref_stage_inv, L.ref_stage_force, L.ref_stage_mom_to_bead):
             f.argtypes = [dp, dp, C.c_int]
             f.restype = None
@@ -210,6 +216,36 @@ class RefPIMD:
         rc = lib().ref_set_integrator(self._h, self.TRANSFORMS[transform], self.THERMOSTATS[thermostat])
         if rc != 0:
             raise RuntimeError(f"ref_set_integrator failed: {rc}")
+
+    # ---- well-tempered metadynamics ----
+    def metad_enable(self, cv, sigma, height, bias_factor, deposit_every, max_gaussians=4096, atoms=None, f_species=None, Q=0.0):
+        """cv 'dimer' (atoms = O1, H1, O2, O4, H2, O3) or 'debye' (f_species, Q); height in eV."""
+        a = np.ascontiguousarray(atoms if atoms is not None else np.zeros(6), dtype=np.int32)
+        f = np.ascontiguousarray(f_species if f_species is not None else np.zeros(16), dtype=np.float64)
+        rc = lib().ref_metad_enable(self._h, {"dimer": 1, "debye": 2}[cv], _ip(a), _dp(f), float(Q), float(sigma), float(height),
+                                    float(bias_factor), int(deposit_every), int(max_gaussians))
+        if rc != 0:
+            raise RuntimeError(f"ref_metad_enable failed: {rc}")
+
+    def metad_cv(self):
+        s = np.zeros(self.shape[:2]); g = np.zeros(self.shape)
+        rc = lib().ref_metad_cv(self._h, _dp(s), _dp(g))
+        if rc != 0:
+            raise RuntimeError(f"ref_metad_cv failed: {rc}")
+        return s, g
+
+    def metad_gaussians(self, r=0, cap=65536):
+        c = np.zeros(cap); h = np.zeros(cap)
+        n = lib().ref_metad_gaussians(self._h, int(r), _dp(c), _dp(h), cap)
+        return c[:n].copy(), h[:n].copy()
+
+    def metad_bias(self, s, r=0):
+        return lib().ref_metad_bias(self._h, int(r), float(s))
+
+    def metad_deposit_now(self):
+        rc = lib().ref_metad_deposit_now(self._h)
+        if rc != 0:
+            raise RuntimeError(f"ref_metad_deposit_now failed: {rc}")
 
     def step(self, n=1):
         rc = lib().ref_step(self._h, int(n))
