@@ -157,6 +157,24 @@ int pimd_set_nlist_skin(pimd_ctx *ctx, double skin);
 /* Number of cell-list passes (candidate-list rebuilds) so far.  h_count HOST.  Synchronises. */
 int pimd_nlist_rebuilds(pimd_ctx *ctx, int64_t *h_count);
 
+/* Well-tempered metadynamics with the paper's collective variables.  One bias V_G(s) per replica; the CV is evaluated
+ * on every bead and every bead feels F = -dV_G/ds(s_k) grad s(q_k), added to the forces of the potential.  Every
+ * `deposit_every` steps (100; 0.05 ps) one Gaussian per bead is deposited at the bead's CV value, width sigma
+ * (P:L140, 2 sigma read as 2 sigma^2), height (height_eV / P) exp(-V_G(s_k) / (k_B T (bias_factor - 1))) with the bias before the event.
+ *   cv 1  s_dimer = d(O1,H1) - d(O2,H1) + d(O4,H2) - d(O3,H2); atoms6 HOST = indices of O1, H1, O2, O4, H2, O3
+ *   cv 2  s_water = (1/N) sum_i sum_j f_i f_j sin(Q R_ij)/(Q R_ij) (all ordered pairs, i = j included, minimum image);
+ *         f_species HOST [S] scattering factor per type, Q in 1/A (4 pi sin(11.95 deg) / 1.54 A)
+ * The workspace holds up to 16384 Gaussians per replica (further depositions are dropped).  Steps run with plain launches.
+ *   pimd_metad_cv          d_s DEVICE double [R][P], d_grad DEVICE double [R][P][N][3] (either may be NULL): CV and its gradient at the
+ *                          current positions.  Asynchronous.
+ *   pimd_metad_gaussians   HOST copies of the centres and heights of one replica (first `cap`), *h_n = number deposited.  Synchronises.
+ *   pimd_metad_deposit_now one deposition event at the current positions (tests, restart). */
+int pimd_metad_enable(pimd_ctx *ctx, int cv, const int32_t *atoms6, const double *f_species, double Q, double sigma,
+                      double height_eV, double bias_factor, int deposit_every);
+int pimd_metad_cv(pimd_ctx *ctx, double *d_s, double *d_grad);
+int pimd_metad_gaussians(pimd_ctx *ctx, int replica, double *h_centres, double *h_heights, int cap, int *h_n);
+int pimd_metad_deposit_now(pimd_ctx *ctx);
+
 /* Waits for the stream and returns any latched device error. */
 int pimd_sync(pimd_ctx *ctx);
 

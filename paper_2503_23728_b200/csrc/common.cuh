@@ -63,6 +63,22 @@ struct NlistDev {
     int64_t pair_cap;
 };
 
+#define PIMD_METAD_MAX 16384           // Gaussians per replica the workspace holds
+#define PIMD_METAD_BLOCKS 256          // partial sums per bead-system of the Debye CV (N <= 32768)
+
+// well-tempered metadynamics: one bias per replica, felt by every bead
+struct pimd_metad {
+    int cv;                            // 0 off, 1 s_dimer, 2 Debye
+    int atoms[6];
+    double f[16], Q, sigma, w0, biasf;
+    int every;
+    int *n_g;                          // [R]
+    double *gc, *gh;                   // [R][PIMD_METAD_MAX]
+    double *s, *dV;                    // [R*P]
+    double *grad;                      // [rows][3]
+    double *partial;                   // [R*P][PIMD_METAD_BLOCKS]
+};
+
 struct pimd_ctx {
     int N, R, P, periodic;
     int64_t rows;                      // R*P*N
@@ -70,7 +86,7 @@ struct pimd_ctx {
     double T, dt, gamma_fs;            // gamma_fs < 0: NVE
     uint64_t seed;
     int64_t step;
-    int kind, gemm_dtype;
+    int kind, gemm_dtype, n_species_host;
     double harmonic_omega;
     cudaStream_t stream;
     int forces_valid;
@@ -114,6 +130,7 @@ struct pimd_ctx {
     float *Fraw;                       // [rows][4] complete-row partial force sums
     int gran_m, gran_f;                // pairs per reduction granule
     int64_t n_gran_m, n_gran_f;
+    pimd_metad md;
     struct PimdProf *prof;             // host-side event recorder (pimd_profile)
 };
 
@@ -149,6 +166,8 @@ int pimd_launch_estimators(pimd_ctx *c);
 int pimd_launch_nlist(pimd_ctx *c);
 int pimd_launch_nlist_invalidate(pimd_ctx *c);       // positions were replaced from outside: rebuild the candidate lists
 int pimd_launch_gfn_forces(pimd_ctx *c);
+int pimd_launch_metad_bias(pimd_ctx *c, int add_force);   // CV and dV_G/ds of every bead; add_force: F -= dV_G/ds grad s
+int pimd_launch_metad_deposit(pimd_ctx *c);               // one Gaussian per bead at the CV values of the last evaluation
 int pimd_launch_copy_forces_f32(pimd_ctx *c, float *d_out);
 size_t pimd_gfn_smem_bytes(int K, int H);
 bool pimd_gfn_supported(int K, int H);

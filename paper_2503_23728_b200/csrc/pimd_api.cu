@@ -60,7 +60,7 @@ void pimd_prof_end(pimd_ctx *c)
 namespace {
 
 struct Layout {
-    size_t q, p, F, species, mass, C, CT, omega, lam, gam, Tstage, pileg_partial, pileg_alpha, err, est_partial, est_out;
+    size_t q, p, F, species, mass, C, CT, omega, lam, gam, Tstage, pileg_partial, pileg_alpha, md_n, md_gc, md_gh, md_s, md_dV, md_grad, md_partial, err, est_partial, est_out;
     size_t cell_id, cell_count, cell_start, cell_cursor, sorted_atom, sorted_q, nnz, ncand, hits, hitmask, q_ref, q32, need, row_ptr, block_sums, col, pair_row;
     size_t wimg, wimg_node, xs0, h1_img, meta_img, weights, nfeat, xfeat, mfeat, Efeat, Gfeat, carry_m, carry_f, Fraw;
     size_t total;
@@ -158,6 +158,13 @@ int compute_layout(int N, int R, int P, const double box[3], const pimd_net_para
     L->Tstage = take(cur, sizeof(double) * 4 * P * P);
     L->pileg_partial = take(cur, sizeof(double) * (size_t)R * 64 * 2);
     L->pileg_alpha = take(cur, sizeof(double) * (size_t)R);
+    L->md_n = take(cur, sizeof(int) * (size_t)R);
+    L->md_gc = take(cur, sizeof(double) * (size_t)R * PIMD_METAD_MAX);
+    L->md_gh = take(cur, sizeof(double) * (size_t)R * PIMD_METAD_MAX);
+    L->md_s = take(cur, sizeof(double) * (size_t)R * P);
+    L->md_dV = take(cur, sizeof(double) * (size_t)R * P);
+    L->md_grad = take(cur, sizeof(double) * (size_t)rows * 3);
+    L->md_partial = take(cur, sizeof(double) * (size_t)R * P * PIMD_METAD_BLOCKS);
     L->err = take(cur, sizeof(int) * 4);
     L->est_partial = take(cur, sizeof(double) * (size_t)R * 64 * 8);
     L->est_out = take(cur, sizeof(double) * (size_t)R * 8);
@@ -385,6 +392,10 @@ int compute_forces(pimd_ctx *c)
         ProfScope ps(c, PROF_OTHER);
         if ((rc = pimd_launch_simple_forces(c))) return rc;
     }
+    if (c->md.cv) {
+        ProfScope ps(c, PROF_OTHER);
+        if ((rc = pimd_launch_metad_bias(c, 1))) return rc;
+    }
     c->forces_valid = 1;
     return 0;
 }
@@ -441,6 +452,7 @@ extern "C" int pimd_create(pimd_ctx **out, int n_atoms, int n_replicas, const in
     for (int a = 0; a < 3; ++a) c->box[a] = box[a];
     c->T = T_kelvin; c->dt = dt_fs; c->gamma_fs = gamma_centroid_per_ps < 0.0 ? -1.0 : gamma_centroid_per_ps * 1e-3;
     c->seed = seed; c->step = 0; c->kind = net->kind; c->gemm_dtype = net->gemm_dtype;
+    c->n_species_host = net->n_species;
     c->harmonic_omega = net->harmonic_omega;
     c->stream = (cudaStream_t)cuda_stream;
     int dev = 0;
@@ -459,6 +471,10 @@ extern "C" int pimd_create(pimd_ctx **out, int n_atoms, int n_replicas, const in
     c->lam_k = (double *)(ws + L.lam); c->gam_k = (double *)(ws + L.gam); c->Tstage = (double *)(ws + L.Tstage);
     c->pileg_partial = (double *)(ws + L.pileg_partial); c->pileg_alpha = (double *)(ws + L.pileg_alpha);
     c->transform = 0; c->thermostat = 0;
+    c->md.cv = 0;
+    c->md.n_g = (int *)(ws + L.md_n); c->md.gc = (double *)(ws + L.md_gc); c->md.gh = (double *)(ws + L.md_gh);
+    c->md.s = (double *)(ws + L.md_s); c->md.dV = (double *)(ws + L.md_dV); c->md.grad = (double *)(ws + L.md_grad);
+    c->md.partial = (double *)(ws + L.md_partial);
     c->Tq_fwd = c->CmatT; c->Tp_fwd = c->CmatT; c->Tq_inv = c->Cmat; c->Tp_inv = c->Cmat;   // normal modes: orthogonal
     c->err = (int *)(ws + L.err);
     c->step_dev = (uint32_t *)(c->err + 2);          // (words 2, 3 of the error block)
@@ -759,7 +775,7 @@ extern "C" int pimd_step(pimd_ctx *c, int n)
     int rc;
     if ((rc = enter(c))) return rc;
     if (!c->forces_valid && (rc = compute_forces(c))) return rc;   // (also sets every opt-in kernel attribute before a capture)
-    const bool profiling = c->prof && c->prof->on;
+    const bool profiling = (c->prof && c->prof->on) || c->md.cv != 0;   // (metadynamics: plain launches, the deposition is decided by the host)
     // The launch sequence of a step is captured once as a CUDA graph and replayed: the small configurations are bound by
     // launch overhead (17-35 launches per step).  Per-class event timing (pimd_profile) needs the plain launches.
     for (int s = 0; s < n; ++s) {
@@ -786,7 +802,81 @@ extern "C" int pimd_step(pimd_ctx *c, int n)
             c->warm = 1;
         }
         c->step += 1;
+        if (c->md.cv && c->step % c->md.every == 0) {   // a Gaussian per bead at the positions just reached; F(q) includes them from here on
+            if ((rc = pimd_launch_metad_deposit(c))) return rc;
+            if ((rc = compute_forces(c))) return rc;
+        }
     }
+    return 0;
+}
+
+// ---- well-tempered metadynamics ---------------------------------------------------------------------
+extern "C" int pimd_metad_enable(pimd_ctx *c, int cv, const int32_t *atoms6, const double *f_species, double Q, double sigma,
+                                 double height_eV, double bias_factor, int deposit_every)
+{
+    if (!c) { pimd_set_error("null context"); return PIMD_ERR_ARG; }
+    if ((cv != 1 && cv != 2) || !(sigma > 0.0) || !(bias_factor > 1.0) || deposit_every < 1 || !(height_eV >= 0.0)) {
+        pimd_set_error("metadynamics: cv in {1, 2}, sigma > 0, bias factor > 1, deposit_every >= 1");
+        return PIMD_ERR_ARG;
+    }
+    int rc;
+    if ((rc = enter(c))) return rc;
+    if (cv == 1) {
+        if (!atoms6) { pimd_set_error("s_dimer needs six atom indices"); return PIMD_ERR_ARG; }
+        for (int k = 0; k < 6; ++k) {
+            if (atoms6[k] < 0 || atoms6[k] >= c->N) { pimd_set_error("s_dimer atom index %d out of range", atoms6[k]); return PIMD_ERR_ARG; }
+            c->md.atoms[k] = atoms6[k];
+        }
+    } else {
+        const int S = c->kind == 0 ? c->net.S : 16;
+        if (!f_species || !(Q > 0.0) || c->N > PIMD_METAD_BLOCKS * 128) { pimd_set_error("Debye CV needs scattering factors, Q > 0 and N <= %d", PIMD_METAD_BLOCKS * 128); return PIMD_ERR_ARG; }
+        for (int k = 0; k < 16; ++k) c->md.f[k] = (k < S && k < c->n_species_host) ? f_species[k] : 0.0;
+        c->md.Q = Q;
+    }
+    c->md.sigma = sigma; c->md.w0 = height_eV; c->md.biasf = bias_factor; c->md.every = deposit_every;
+    PIMD_CUDA_CHECK(cudaMemsetAsync(c->md.n_g, 0, sizeof(int) * (size_t)c->R, c->stream));
+    PIMD_CUDA_CHECK(cudaMemsetAsync(c->md.grad, 0, sizeof(double) * (size_t)c->rows * 3, c->stream));
+    c->md.cv = cv;
+    c->forces_valid = 0;
+    drop_step_graph(c);
+    return 0;
+}
+
+extern "C" int pimd_metad_cv(pimd_ctx *c, double *d_s, double *d_grad)
+{
+    if (!c || !c->md.cv) { pimd_set_error("metadynamics is not enabled"); return PIMD_ERR_ARG; }
+    int rc;
+    if ((rc = enter(c))) return rc;
+    if ((rc = pimd_launch_metad_bias(c, 0))) return rc;
+    if (d_s) PIMD_CUDA_CHECK(cudaMemcpyAsync(d_s, c->md.s, sizeof(double) * (size_t)c->R * c->P, cudaMemcpyDeviceToDevice, c->stream));
+    if (d_grad) PIMD_CUDA_CHECK(cudaMemcpyAsync(d_grad, c->md.grad, sizeof(double) * (size_t)c->rows * 3, cudaMemcpyDeviceToDevice, c->stream));
+    return 0;
+}
+
+extern "C" int pimd_metad_gaussians(pimd_ctx *c, int replica, double *h_centres, double *h_heights, int cap, int *h_n)
+{
+    if (!c || !c->md.cv || !h_n || replica < 0 || replica >= c->R) { pimd_set_error("invalid argument"); return PIMD_ERR_ARG; }
+    int rc;
+    if ((rc = enter(c))) return rc;
+    int n = 0;
+    PIMD_CUDA_CHECK(cudaMemcpyAsync(&n, c->md.n_g + replica, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    PIMD_CUDA_CHECK(cudaStreamSynchronize(c->stream));
+    *h_n = n;
+    const int m = n < cap ? n : cap;
+    if (m > 0 && h_centres) PIMD_CUDA_CHECK(cudaMemcpyAsync(h_centres, c->md.gc + (size_t)replica * PIMD_METAD_MAX, sizeof(double) * m, cudaMemcpyDeviceToHost, c->stream));
+    if (m > 0 && h_heights) PIMD_CUDA_CHECK(cudaMemcpyAsync(h_heights, c->md.gh + (size_t)replica * PIMD_METAD_MAX, sizeof(double) * m, cudaMemcpyDeviceToHost, c->stream));
+    PIMD_CUDA_CHECK(cudaStreamSynchronize(c->stream));
+    return 0;
+}
+
+extern "C" int pimd_metad_deposit_now(pimd_ctx *c)
+{
+    if (!c || !c->md.cv) { pimd_set_error("metadynamics is not enabled"); return PIMD_ERR_ARG; }
+    int rc;
+    if ((rc = enter(c))) return rc;
+    if (!c->forces_valid && (rc = compute_forces(c))) return rc;   // the CV values of the current positions
+    if ((rc = pimd_launch_metad_deposit(c))) return rc;
+    c->forces_valid = 0;
     return 0;
 }
 

@@ -54,6 +54,10 @@ def load_library():
                               C.c_double, C.c_uint64, C.POINTER(NetParams), vp, C.c_size_t, vp]
     L.pimd_step.argtypes = [vp, C.c_int]
     L.pimd_set_integrator.argtypes = [vp, C.c_int, C.c_int]
+    L.pimd_metad_enable.argtypes = [vp, C.c_int, ip, dp, C.c_double, C.c_double, C.c_double, C.c_double, C.c_int]
+    L.pimd_metad_cv.argtypes = [vp, vp, vp]
+    L.pimd_metad_gaussians.argtypes = [vp, C.c_int, dp, dp, C.c_int, C.POINTER(C.c_int)]
+    L.pimd_metad_deposit_now.argtypes = [vp]
     L.pimd_set_nlist_skin.argtypes = [vp, C.c_double]
     L.pimd_nlist_rebuilds.argtypes = [vp, C.POINTER(C.c_int64)]
     L.pimd_forces.argtypes = [vp, vp]
@@ -166,6 +170,31 @@ class PIMD:
     def set_nlist_skin(self, skin):
         """Verlet skin (A) of the reusable candidate lists; 0 = cell-list pass every step.  Results do not depend on it."""
         _check(load_library().pimd_set_nlist_skin(self._h, float(skin)))
+
+    def metad_enable(self, cv, sigma, height, bias_factor, deposit_every, atoms=None, f_species=None, Q=0.0):
+        """Well-tempered metadynamics: cv 'dimer' (atoms = O1, H1, O2, O4, H2, O3) or 'debye' (f_species, Q); height in eV."""
+        a = np.ascontiguousarray(atoms if atoms is not None else np.zeros(6), dtype=np.int32)
+        f = np.ascontiguousarray(f_species if f_species is not None else np.zeros(16), dtype=np.float64)
+        self._keep += [a, f]
+        _check(load_library().pimd_metad_enable(self._h, {"dimer": 1, "debye": 2}[cv], a.ctypes.data_as(C.POINTER(C.c_int32)),
+                                                f.ctypes.data_as(C.POINTER(C.c_double)), float(Q), float(sigma), float(height),
+                                                float(bias_factor), int(deposit_every)))
+
+    def metad_cv(self):
+        t = self._torch
+        s = t.empty(self.shape[:2], dtype=t.float64, device=self.device)
+        g = t.empty(self.shape, dtype=t.float64, device=self.device)
+        _check(load_library().pimd_metad_cv(self._h, C.c_void_p(s.data_ptr()), C.c_void_p(g.data_ptr())))
+        return s, g
+
+    def metad_gaussians(self, r=0, cap=16384):
+        c = np.zeros(cap); h = np.zeros(cap); n = C.c_int()
+        _check(load_library().pimd_metad_gaussians(self._h, int(r), c.ctypes.data_as(C.POINTER(C.c_double)),
+                                                   h.ctypes.data_as(C.POINTER(C.c_double)), cap, C.byref(n)))
+        return c[: n.value].copy(), h[: n.value].copy()
+
+    def metad_deposit_now(self):
+        _check(load_library().pimd_metad_deposit_now(self._h))
 
     def nlist_rebuilds(self):
         n = C.c_int64()
