@@ -189,8 +189,6 @@ __device__ __forceinline__ void role_P(const PairArgs &a, unsigned char *S, uint
         }
         int jrow = 0, kind = 0;
         float w = 0.f, ux = 0.f, uy = 0.f, uz = 0.f, dist = 0.f;
-        int prev_row = -1;
-        if (lane == 0 && (p & (GP - 1)) != 0 && pg - 1 < n_pairs) prev_row = __ldg(a.pair_row + pg - 1);
         if (row >= 0) {
             const int sys = row / a.N;
             jrow = sys * a.N + cj;
@@ -210,7 +208,7 @@ __device__ __forceinline__ void role_P(const PairArgs &a, unsigned char *S, uint
             kind = seg_kind(rs, re, pg & ~(int64_t)(GP - 1), GP);
         }
         int prev = __shfl_up_sync(FULL, row, 1);
-        if (lane == 0) prev = ((p & (GP - 1)) == 0) ? -2 : prev_row;
+        if (lane == 0) prev = -2;                 // a granule is a warp's 32 pairs: its first pair always starts a segment
         const unsigned fm = __ballot_sync(FULL, row != prev);
         // ---- meta slot
         if ((p >> 5) == 1) {                      // poller of role P (warp 1)

@@ -130,7 +130,9 @@ int compute_layout(int N, int R, int P, const double box[3], const pimd_net_para
         } else {
             expect = 256.0;
         }
-        int64_t cap_row = (int64_t)ceil(2.0 * expect) + 32;
+        // pair capacity per row: 1.5 x the uniform-density expectation + 32 (the -3 latch of the scan kernel guards it; the tile
+        // images of the tcgen05 pipeline are sized by it: 35.9 KB per 128 pairs)
+        int64_t cap_row = (int64_t)ceil(1.5 * expect) + 32;
         if (cap_row > N - 1) cap_row = N - 1;
         if (cap_row > PIMD_MAX_NBR) cap_row = PIMD_MAX_NBR;
         if (cap_row < 1) cap_row = 1;

@@ -153,3 +153,19 @@ def test_integrator_variant_is_chosen_before_the_first_step(cuda_device):
     gpu.step(1)
     with pytest.raises(pb.PimdError):
         gpu.set_integrator("staging", "pile_l")
+
+
+def test_non_finite_positions_latch_the_nan_error(cuda_device):
+    """PIMD_ERR_NAN (-4): a non-finite position or force met by a kernel is latched in the device error word and returned by the
+    next synchronising call."""
+    import torch
+    import paper_2503_23728_b200 as pb
+    sp, pos = _system()
+    gpu, ref = make_pair(sp, pos, np.zeros(3), 4, 300.0, 0.25, 1.0, 1, _spec(1, 0.2))
+    q, p, st = gpu.get_state()
+    p[0, 1, 2, 0] = float("nan")                    # one poisoned momentum: the A step turns it into a non-finite position
+    gpu.set_state(q, p, st)
+    gpu.step(2)
+    with pytest.raises(pb.PimdError) as e:
+        gpu.sync()
+    assert e.value.code == -4
