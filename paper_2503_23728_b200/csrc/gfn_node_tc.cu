@@ -15,8 +15,9 @@
 // a single product, because x is gathered as bf16 by the message pass anyway.  The tensor pipe has the time (the kernel is
 // bound by its HBM reads and writes); shared memory does not hold ten 32 KB weight images, so the weight images stream
 // from L2 through a ring of 16 KB slots (TMA bulk copies, one producer warp), 18 (20 in the last layer) slots per tile.
-// The pair kernels gather x_j, E_j per directed pair in the message passes: that copy is written as packed bf16
-// (XE[row][c] = x | E << 16) so that one 32-bit load serves both and the L2 gather traffic halves.  G stays fp32:
+// The pair kernels gather x_j and y_j = E_j x_j per directed pair in the message passes: that copy is one 32-bit word per
+// channel (XE[row][c]: x as bf16 in the low half; the whole word read as fp32 is y to half a bf16 ulp, tc::pack_x_y), so one
+// load serves both and the L2 gather traffic halves.  G stays fp32:
 // G_i + G_j enters the force readout directly, with no averaging over neighbours behind it.
 // SiLU(x) = h tanh(h) + h with h = x/2: the 1/2 is folded (exactly) into the W_vn, W_vm images and b_v1.
 #include "common.cuh"
@@ -318,7 +319,7 @@ __global__ void __launch_bounds__(NTH, 1) node_tc_kernel(const __grid_constant__
         tc::mbar_wait(mbar_mma, par);
         par ^= 1;
         tc::tc_fence_after_sync();
-        // ---- E <- E + D0 + b_a ; XE = (x, E) packed bf16, or E -> A1 for G = W_f1 E
+        // ---- E <- E + D0 + b_a ; XE = x (bf16, low half) with y = E x in the whole word (tc::pack_x_y), or E -> A1 for G = W_f1 E
 #pragma unroll
         for (int j = 0; j < 2; ++j) {
             const int c0 = g * 32 + j * 16;
@@ -345,8 +346,8 @@ __global__ void __launch_bounds__(NTH, 1) node_tc_kernel(const __grid_constant__
 #pragma unroll
                 for (int e4 = 0; e4 < 4; ++e4)
                     *(uint4 *)(xs + (((j * 4 + e4) ^ (lane & 7)) << 4)) =
-                        make_uint4(tc::pack_bf16(v[e4 * 4], ee[e4 * 4]), tc::pack_bf16(v[e4 * 4 + 1], ee[e4 * 4 + 1]),
-                                   tc::pack_bf16(v[e4 * 4 + 2], ee[e4 * 4 + 2]), tc::pack_bf16(v[e4 * 4 + 3], ee[e4 * 4 + 3]));
+                        make_uint4(tc::pack_x_y(v[e4 * 4], ee[e4 * 4]), tc::pack_x_y(v[e4 * 4 + 1], ee[e4 * 4 + 1]),
+                                   tc::pack_x_y(v[e4 * 4 + 2], ee[e4 * 4 + 2]), tc::pack_x_y(v[e4 * 4 + 3], ee[e4 * 4 + 3]));
             } else {
                 store_operand16(A1h, A1l, r, c0, ee);
             }

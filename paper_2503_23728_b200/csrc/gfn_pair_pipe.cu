@@ -10,7 +10,7 @@
 //   MMA 1 thread               : D1 = A1 (W_e1/2)^T  (4 x UMMA 128x128x16);  D2^T = W2 A2^T  (8 x UMMA), W2 = W_e2 or W_f1 W_e2/2
 //   H   4 warps, thread = pair : D1 (TMEM) + b -> SiLU -> A2 (bf16 operand of the second product)
 //   S   1 warp                 : TMA bulk stores of the tile's A2 image (32 KB) and meta record to HBM
-//   G   4 warps                : TMA tile::gather4 copies of the gathered rows (x_j|E_j packed bf16, or G_j fp32; 4 x 512 B per copy)
+//   G   4 warps                : TMA tile::gather4 copies of the gathered rows (x_j, y_j = E_j x_j in one word, or G_j fp32; 4 x 512 B per copy)
 //                                into an 8-slot shared-memory ring, 16 pairs per slot
 //   E   16 warps, thread = (channel, quarter tile): D2^T (TMEM lane = channel) -> e_ij = e0_ij + E_i + E_j (S:G5) ->
 //                                private running sums over CSR row segments, cut at row boundaries.
@@ -102,7 +102,8 @@ struct PairArgs {
     const uint16_t *W1img, *W2img;        // bf16 UMMA images: 0.5 W_e1 [128][64]; W_e2 (message) or 0.5 W_f1 W_e2 (head), 2 x [128][64]
     float b1h[H];                         // b_e1 / 2 (kernel-parameter constant bank: immediate operands in role H)
     const float *b2;
-    const void *gsrc;                     // message: XE packed bf16 (x | E << 16) [rows][128] u32; head: G fp32 [rows][128]
+    const void *gsrc;                     // message: XE [rows][128] u32, x bf16 in the low half, the word as fp32 = y = E x (tc::pack_x_y); head: G fp32 [rows][128]
+    const float *Emaster;                 // message: fp32 master of E, tile-blocked (gfn_node_tc.cu), for E_i
     const float *wf2; float bf2;
     float *m_out, *carry_m, *Fraw, *carry_f;
     unsigned char *h1_img, *meta_img;     // per tile: A2 operand image (32 KB) and Meta, written by the first pass of a force
@@ -299,32 +300,32 @@ __device__ __forceinline__ uint64_t make_desc_mn_sw128(uint32_t addr, uint32_t l
 
 // ---- role E, message pass: m_i = agg_norm sum_j c_ij (e0_ij + E_i + E_j) (.) x_j  (S:G3, G5).
 // D2 is TRANSPOSED (TMEM lane = channel c, column = pair): the thread walks the 32 pairs of its quarter tile in CSR
-// order.  With wx = c_ij x_j:  m_i = sum_j (e0 + E_j) wx + (b + E_i) sum_j wx, so the two private running sums do not
-// depend on the row and a row boundary only cuts them.  x_j, E_j come from the gather ring (lanes = consecutive
-// channels: conflict-free).  Code is kept small on purpose (five roles share the instruction cache).
+// order.  m_i = sum_j c_ij (e0 x_j + y_j) + (b + E_i) sum_j c_ij x_j with y_j = E_j x_j formed once per atom by the node kernel,
+// so the two private running sums do not depend on the row and a row boundary only cuts them.  The gathered word carries
+// x_j in its low half and IS y_j when read as an fp32 (tc::pack_x_y): per (pair, channel) one shared-memory load, one shift
+// and three FMAs.  Lanes = consecutive channels: conflict-free.  E_i comes from the fp32 master (tile-blocked, gfn_node_tc.cu).
+// Code is kept small on purpose (five roles share the instruction cache).
 struct MsgState {
-    int cur, kind, nx_row;       // current row (-1 none), its segment kind, row whose E_i is prefetched
-    uint32_t nx_val;
-    float s1, s2, be;
+    int cur, kind;               // current row (-1 none), its segment kind
+    float s1, s2, ei;            // running sums; E_i of the row (in flight until the flush)
 };
 
-__device__ __forceinline__ void msg_flush(const PairArgs &a, const MsgState &st, int64_t gidx, int c)
+__device__ __forceinline__ void msg_flush(const PairArgs &a, const MsgState &st, int64_t gidx, int c, float b2c)
 {
     if (st.cur >= 0) {
         float *dst = (st.kind == 0) ? a.m_out + (size_t)st.cur * H + c : a.carry_m + (size_t)(gidx * 2 + (st.kind - 1)) * H + c;
-        *dst = a.wscale * fmaf(st.be, st.s2, st.s1);     // wscale = agg_norm
+        *dst = a.wscale * fmaf(b2c + st.ei, st.s2, st.s1);     // wscale = agg_norm
     }
 }
 
 // b + E_i of the row that starts: prefetched at the previous boundary (CSR rows are consecutive), else loaded now
+__device__ __forceinline__ size_t e_master_off(int row, int c) { return ((size_t)(row >> 7) * (H / 4) + (c >> 2)) * (128 * 4) + (size_t)(row & 127) * 4 + (c & 3); }
+// E_i of the row that starts.  The load is only issued here; its value is first used when the segment is flushed, so its
+// latency (the fp32 master is not kept in L2 by the gathers the way XE is) hides behind the segment's pairs.
 template <bool FIRST>
-__device__ __forceinline__ void msg_row_bias(const uint32_t *__restrict__ XE, MsgState &st, int64_t rows, float b2c, int c)
+__device__ __forceinline__ void msg_row_bias(const float *__restrict__ Em, MsgState &st, int c)
 {
-    if (FIRST) { st.be = b2c; return; }
-    const uint32_t raw = (st.cur == st.nx_row) ? st.nx_val : __ldg(XE + (size_t)st.cur * H + c);
-    st.be = b2c + tc::bf16hi_to_f32(raw);
-    st.nx_row = (st.cur + 1 < rows) ? st.cur + 1 : st.cur;
-    st.nx_val = __ldg(XE + (size_t)st.nx_row * H + c);
+    st.ei = FIRST ? 0.f : __ldg(Em + e_master_off(st.cur, c));
 }
 
 // FIRST: the first message pass of an evaluation is layer 0, where E = 0 for every atom (a4): e_ij = e0_ij + b, so the E_j unpack
@@ -335,12 +336,11 @@ __device__ __forceinline__ void role_E_msg(const PairArgs &a, unsigned char *S, 
 {
     STATS_BEGIN
     const float b2c = ((const float *)(S + OFF_BIAS))[H + c];
-    const uint32_t *__restrict__ XE = (const uint32_t *)a.gsrc;
     const uint32_t lane_field = (uint32_t)(c & ~31) << 16;
     const int64_t stride = (int64_t)gridDim.x * TP;
     int64_t tile0 = (int64_t)blockIdx.x * TP;
     MsgState st;
-    st.cur = -1; st.kind = 0; st.nx_row = -1; st.nx_val = 0; st.s1 = st.s2 = st.be = 0.f;
+    st.cur = -1; st.kind = 0; st.s1 = st.s2 = st.ei = 0.f;
     for (int it = 0; it < n_my; ++it, tile0 += stride) {
         const Meta &M = meta_of(S, it);
         const int64_t gidx = (tile0 >> 5) + qt;
@@ -363,7 +363,7 @@ __device__ __forceinline__ void role_E_msg(const PairArgs &a, unsigned char *S, 
                 const int rk = M.rowk[qt * 32];
                 st.cur = (rk < 0) ? -1 : (rk & 0x1FFFFFFF);
                 st.kind = (rk < 0) ? 0 : (rk >> 29);
-                if (st.cur >= 0) msg_row_bias<FIRST>(XE, st, a.rows, b2c, c);
+                if (st.cur >= 0) msg_row_bias<FIRST>(a.Emaster, st, c);
             }
             float v[16];
             tc::tmem_ld16(td2 + q0, v);
@@ -373,23 +373,20 @@ __device__ __forceinline__ void role_E_msg(const PairArgs &a, unsigned char *S, 
                 if (lane == 0) tc::mbar_arrive(&bar[D2_EMPTY + (it & 1)]);
             }
             const uint32_t *xr = (const uint32_t *)(S + OFF_RING + slot * 8192) + c;
-            float wx[16];
+            // v <- e0 x_j + y_j, xv <- x_j; the cutoff weights c_ij stay in shared memory and enter in the sums (two FMAs per term)
+            float xv[16];
 #pragma unroll
-            for (int e4 = 0; e4 < 4; ++e4) {
-                const float4 w4 = *(const float4 *)&M.w[q0 + e4 * 4];
-                const float wv[4] = {w4.x, w4.y, w4.z, w4.w};
-#pragma unroll
-                for (int k = 0; k < 4; ++k) {
-                    const uint32_t xe = xr[(e4 * 4 + k) * H];
-                    wx[e4 * 4 + k] = wv[k] * tc::bf16lo_to_f32(xe);       // c_ij x_j
-                    if (!FIRST) v[e4 * 4 + k] += tc::bf16hi_to_f32(xe);   // e0 + E_j
-                }
+            for (int e = 0; e < 16; ++e) {
+                const uint32_t xe = xr[e * H];
+                xv[e] = tc::bf16lo_to_f32(xe);
+                v[e] = FIRST ? v[e] * xv[e] : fmaf(v[e], xv[e], __uint_as_float(xe));
             }
+            const float *wq = &M.w[q0];
             unsigned mask = M.fmask[qt * 2 + cc];
             if (cc == 0) mask &= ~1u;            // handled above
             if (mask == 0u) {
 #pragma unroll
-                for (int e = 0; e < 16; ++e) { st.s1 = fmaf(v[e], wx[e], st.s1); st.s2 += wx[e]; }
+                for (int e = 0; e < 16; ++e) { const float w = wq[e]; st.s1 = fmaf(w, v[e], st.s1); st.s2 = fmaf(w, xv[e], st.s2); }
             } else if ((mask & (mask - 1)) == 0u) {
                 // exactly one row boundary in the chunk (the usual case: rows are longer than 16 pairs): the pairs
                 // before it close the running sums, the pairs from it on open the next row's (warp-uniform predicates)
@@ -397,15 +394,16 @@ __device__ __forceinline__ void role_E_msg(const PairArgs &a, unsigned char *S, 
                 float t1 = 0.f, t2 = 0.f;
 #pragma unroll
                 for (int e = 0; e < 16; ++e) {
-                    if (e < hi) { st.s1 = fmaf(v[e], wx[e], st.s1); st.s2 += wx[e]; }
-                    else        { t1 = fmaf(v[e], wx[e], t1); t2 += wx[e]; }
+                    const float w = wq[e];
+                    if (e < hi) { st.s1 = fmaf(w, v[e], st.s1); st.s2 = fmaf(w, xv[e], st.s2); }
+                    else        { t1 = fmaf(w, v[e], t1); t2 = fmaf(w, xv[e], t2); }
                 }
-                msg_flush(a, st, gidx, c);
+                msg_flush(a, st, gidx, c, b2c);
                 const int rk = M.rowk[q0 + hi];
                 st.cur = (rk < 0) ? -1 : (rk & 0x1FFFFFFF);
                 st.kind = (rk < 0) ? 0 : (rk >> 29);
                 st.s1 = t1; st.s2 = t2;
-                if (st.cur >= 0) msg_row_bias<FIRST>(XE, st, a.rows, b2c, c);
+                if (st.cur >= 0) msg_row_bias<FIRST>(a.Emaster, st, c);
             } else {
                 int lo = 0;
 #pragma unroll 1
@@ -413,21 +411,21 @@ __device__ __forceinline__ void role_E_msg(const PairArgs &a, unsigned char *S, 
                     const int hi = mask ? (__ffs(mask) - 1) : 16;
 #pragma unroll
                     for (int e = 0; e < 16; ++e)
-                        if (e >= lo && e < hi) { st.s1 = fmaf(v[e], wx[e], st.s1); st.s2 += wx[e]; }
+                        if (e >= lo && e < hi) { const float w = wq[e]; st.s1 = fmaf(w, v[e], st.s1); st.s2 = fmaf(w, xv[e], st.s2); }
                     if (!mask) break;
                     mask &= mask - 1;
                     lo = hi;
-                    msg_flush(a, st, gidx, c);   // a new row segment starts at pair q0 + hi
+                    msg_flush(a, st, gidx, c, b2c);   // a new row segment starts at pair q0 + hi
                     const int rk = M.rowk[q0 + hi];
                     st.cur = (rk < 0) ? -1 : (rk & 0x1FFFFFFF);
                     st.kind = (rk < 0) ? 0 : (rk >> 29);
                     st.s1 = 0.f; st.s2 = 0.f;
-                    if (st.cur >= 0) msg_row_bias<FIRST>(XE, st, a.rows, b2c, c);
+                    if (st.cur >= 0) msg_row_bias<FIRST>(a.Emaster, st, c);
                 }
             }
             if (it + 1 < n_my) tc::named_bar_arrive(NB_SLOT + slot, 160);   // slot consumed: its refill overlaps the other chunk
         }
-        msg_flush(a, st, gidx, c);
+        msg_flush(a, st, gidx, c, b2c);
         __syncwarp();
         if (lane == 0) tc::mbar_arrive(&bar[META_EMPTY + (it & (NM - 1))]);
     }
@@ -829,10 +827,11 @@ __device__ __forceinline__ void role_G(const PairArgs &a, unsigned char *S, uint
             if (it > 0) {                                    // the consumers have read the slot
                 WAITED(tc::named_bar_sync(NB_SLOT + qt * 2 + h, 160));   // the 128 consumers + this warp
             }
-            if (lane == 16 * h) tc::mbar_arrive_expect_tx(&bar[XE_FULL + qt * 2 + h], 8192);
-            __syncwarp();
-            // four gathered rows (4 x 512 B, consecutive in the slot) per copy: lanes 0, 4, 8, 12 of the half warp issue
+            // four gathered rows (4 x 512 B, consecutive in the slot) per copy: lanes 0, 4, 8, 12 of the half warp issue.  The
+            // copies are on the consumers' critical path (slot read -> slot refilled); the barrier's arrival with the byte count is
+            // not and follows them (the phase cannot complete before it, whatever has landed by then).
             if ((lane >> 4) == h && (lane & 3) == 0) tc::tma_gather4(dst, &a.gmap, jrow, j1, j2, j3, &bar[XE_FULL + slot]);
+            if (lane == 16 * h) tc::mbar_arrive_expect_tx(&bar[XE_FULL + qt * 2 + h], 8192);
         }
     }
     STATS_END("G")
@@ -877,6 +876,17 @@ __device__ __forceinline__ void role_L(const PairArgs &a, unsigned char *S, uint
             tc::bulk_g2s(&meta_of(S, it), a.meta_img + tile * (int64_t)sizeof(Meta), (uint32_t)sizeof(Meta), &bar[META_FULL + m]);
             tc::mbar_arrive_expect_tx(&bar[A2_FULL + s], 32768);
             tc::bulk_g2s(S + OFF_A2 + s * 32768, a.h1_img + tile * 32768, 32768, &bar[A2_FULL + s]);
+        }
+        if (a.Emaster != nullptr) {
+            // E_i of the tile's rows (role E loads it per row segment) is touched once per pass and does not stay in L2 behind the
+            // image stream: this warp, two tiles ahead of role E, pulls the rows' lines into L2 (4 rows x 32 sectors)
+            const int64_t p0 = tile * TP;
+            const int r0 = __ldg(a.pair_row + p0);
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const int r = r0 + k;
+                if (r < a.rows) asm volatile("prefetch.global.L2 [%0];" ::"l"(a.Emaster + e_master_off(r, lane * 4)));
+            }
         }
         __syncwarp();
     }
@@ -974,6 +984,7 @@ int launch_pair_pipe(pimd_ctx *c, bool head, bool first)
     for (int k = 0; k < H; ++k) a.b1h[k] = c->h_be1_half[k];
     a.b2 = head ? c->net.bfe : c->net.be2;
     a.gsrc = head ? (const void *)c->Gfeat : (const void *)c->XE;
+    a.Emaster = head ? nullptr : c->Efeat;
     a.wf2 = c->net.wf2; a.bf2 = c->net.bf2;
     a.m_out = c->mfeat; a.carry_m = c->carry_m; a.Fraw = c->Fraw; a.carry_f = c->carry_f;
     a.h1_img = c->h1_img; a.meta_img = c->meta_img;

@@ -256,6 +256,18 @@ __device__ __forceinline__ float silu_tanh(float x)
     return fmaf(h, tanh_approx(h), h);
 }
 
+// Gathered word of the message passes: low half = x as bf16 (round to nearest even); the WHOLE word, read as an fp32, is
+// y = E * x(bf16) to within half a bf16 ulp: the high half is chosen so that (high << 16 | low) is the 32-bit pattern nearest to
+// y's (same sign; integer distance between patterns of one sign is monotone in the value).  The consumer needs one shift for x
+// and none for y.
+__device__ __forceinline__ uint32_t pack_x_y(float x, float E)
+{
+    const uint32_t lo = (uint32_t)__bfloat16_as_ushort(__float2bfloat16_rn(x));
+    const uint32_t yb = __float_as_uint(E * __uint_as_float(lo << 16));
+    int32_t hi = ((int32_t)((yb & 0x7FFFFFFFu) - lo) + 0x8000) >> 16;
+    hi = hi < 0 ? 0 : hi;
+    return (yb & 0x80000000u) | ((uint32_t)hi << 16) | lo;
+}
 __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi)
 {
     __nv_bfloat162 t = __floats2bfloat162_rn(lo, hi);
