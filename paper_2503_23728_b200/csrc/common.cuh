@@ -156,6 +156,29 @@ void pimd_set_error(const char *fmt, ...);
         }                                                                                \
     } while (0)
 
+// Programmatic dependent launch: every kernel of the step is launched with programmatic stream serialisation, so that its
+// launch is processed while the kernel before it still runs and it starts the moment that one ends -- in a captured graph too
+// (ice512 -2 %, fad_p8 -17 % per step).  A kernel so launched must not touch memory written by its predecessors before
+// pdl_enter() (griddepcontrol.wait returns when the grids before it have completed and flushed): it is the first statement of
+// every such kernel.  No kernel triggers its dependents early (griddepcontrol.launch_dependents): measured, early-resident
+// blocks of the next kernel cost fad_x64_p32 +26 % per step and ice512 gained nothing over the implicit trigger at exit.
+#if defined(__CUDACC__)
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_enter() { pdl_wait(); }
+
+template <typename... KArgs, typename... Args>
+static inline cudaError_t pimd_launch(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream, Args &&...args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+#endif
+
 // kernel launchers (each returns 0 or PIMD_ERR_CUDA)
 int pimd_launch_init_momenta(pimd_ctx *c);
 int pimd_launch_nm_pre(pimd_ctx *c);                 // O B A with the noise of step *step_dev

@@ -52,7 +52,7 @@ __device__ __forceinline__ float4 assemble_m(const NodeArgs &a, int64_t row, int
 
 template <int H>
 __global__ void __launch_bounds__(NT, 1) node_kernel(NodeArgs a)
-{
+{ pdl_enter();
     extern __shared__ __align__(16) unsigned char smem_raw[];
     NodeSmem<H> &S = *reinterpret_cast<NodeSmem<H> *>(smem_raw);
     constexpr int CPT = Tile<H>::CPT;
@@ -171,7 +171,7 @@ __global__ void __launch_bounds__(NT, 1) node_kernel(NodeArgs a)
 __global__ void force_finalize_kernel(int64_t rows, const int *__restrict__ row_ptr, int gran, float force_scale,
                                       const float *__restrict__ Fraw, const float *__restrict__ carry,
                                       double *__restrict__ F)
-{
+{ pdl_enter();
     int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (row >= rows) return;
     const int rs = row_ptr[row], re = row_ptr[row + 1];
@@ -198,7 +198,7 @@ int launch_node_t(pimd_ctx *c, const NodeArgs &a)
         c->attr_done |= ATTR_NODE32;
     }
     unsigned grid = (unsigned)((c->rows + TP - 1) / TP);
-    node_kernel<H><<<grid, NT, smem, c->stream>>>(a);
+    pimd_launch(node_kernel<H>, grid, NT, smem, c->stream, a);
     c->launches++;
     PIMD_CUDA_CHECK(cudaGetLastError());
     return 0;
@@ -263,7 +263,7 @@ int pimd_launch_gfn_forces(pimd_ctx *c)
         if ((rc = gfn::launch_pair(c, L, true))) return rc;
     }
     ProfScope ps(c, PROF_OTHER);
-    gfn::force_finalize_kernel<<<(unsigned)((c->rows + 255) / 256), 256, 0, c->stream>>>(
+    pimd_launch(gfn::force_finalize_kernel, (unsigned)((c->rows + 255) / 256), 256, 0, c->stream, 
         c->rows, c->nl.row_ptr, c->gran_f, c->net.force_scale, c->Fraw, c->carry_f, c->F);
     c->launches++;
     PIMD_CUDA_CHECK(cudaGetLastError());

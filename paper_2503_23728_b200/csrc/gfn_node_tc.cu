@@ -131,7 +131,7 @@ struct Ring {
 };
 
 __global__ void __launch_bounds__(NTH, 1) node_tc_kernel(const __grid_constant__ Args a)
-{
+{ pdl_enter();
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     unsigned char *S = smem_raw + ((1024u - (tc::smem_u32(smem_raw) & 1023u)) & 1023u);
     unsigned char *A0h = S + OFF_A0H, *A0l = S + OFF_A0L, *A1h = S + OFF_A1H, *A1l = S + OFF_A1L;
@@ -405,7 +405,7 @@ __global__ void __launch_bounds__(NTH, 1) node_tc_kernel(const __grid_constant__
 __global__ void node_init_tc_kernel(int64_t rows, int N, const int *__restrict__ species, const float *__restrict__ Emb,
                                     const float *__restrict__ xs0, float *__restrict__ n, float *__restrict__ E,
                                     uint32_t *__restrict__ XE)
-{
+{ pdl_enter();
     const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;      // over the rows rounded up to whole tiles
     {   // tile-blocked masters: consecutive threads = consecutive rows of one 4-column group (16 contiguous bytes each)
         const int64_t tile = idx >> 12;
@@ -432,7 +432,7 @@ int launch_node_tc(pimd_ctx *c, int mode, int layer)
     const GfnDev &n = c->net;
     if (mode == 0) {
         const int64_t work = (c->rows + 127) / 128 * 128 * (H / 4);
-        node_init_tc_kernel<<<(unsigned)((work + 255) / 256), 256, 0, c->stream>>>(c->rows, c->N, c->species, n.Emb, c->xs0,
+        pimd_launch(node_init_tc_kernel, (unsigned)((work + 255) / 256), 256, 0, c->stream, c->rows, c->N, c->species, n.Emb, c->xs0,
                                                                                  c->nfeat, c->Efeat, c->XE);
         c->launches++;
         PIMD_CUDA_CHECK(cudaGetLastError());
@@ -453,7 +453,7 @@ int launch_node_tc(pimd_ctx *c, int mode, int layer)
         c->attr_done |= ATTR_NODETC;
     }
     const int grid = a.n_tiles < c->num_sms ? a.n_tiles : c->num_sms;
-    node_tc_kernel<<<grid, NTH, smem, c->stream>>>(a);
+    pimd_launch(node_tc_kernel, grid, NTH, smem, c->stream, a);
     c->launches++;
     PIMD_CUDA_CHECK(cudaGetLastError());
     return 0;

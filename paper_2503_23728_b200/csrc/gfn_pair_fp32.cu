@@ -43,7 +43,7 @@ struct PairSmem {
 
 template <int K, int H, bool HEAD>
 __global__ void __launch_bounds__(NT, 1) pair_kernel(PairArgs a)
-{
+{ pdl_enter();
     extern __shared__ __align__(16) unsigned char smem_raw[];
     PairSmem<K, H> &S = *reinterpret_cast<PairSmem<K, H> *>(smem_raw);
     constexpr int CPT = Tile<H>::CPT;
@@ -227,8 +227,8 @@ int launch_pair_t(pimd_ctx *c, const PairArgs &a, bool head)
         PIMD_CUDA_CHECK(cudaFuncSetAttribute(pair_kernel<K, H, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         c->attr_done |= ATTR_PAIR32;
     }
-    if (head) pair_kernel<K, H, true><<<c->num_sms, NT, smem, c->stream>>>(a);
-    else pair_kernel<K, H, false><<<c->num_sms, NT, smem, c->stream>>>(a);
+    if (head) pimd_launch(pair_kernel<K, H, true>, c->num_sms, NT, smem, c->stream, a);
+    else pimd_launch(pair_kernel<K, H, false>, c->num_sms, NT, smem, c->stream, a);
     c->launches++;
     PIMD_CUDA_CHECK(cudaGetLastError());
     return 0;

@@ -895,7 +895,7 @@ __device__ __forceinline__ void role_L(const PairArgs &a, unsigned char *S, uint
 
 template <bool HEAD, int MODE>
 __global__ void __launch_bounds__(Warps<HEAD, MODE>::THREADS, 1) pair_pipe_kernel(const __grid_constant__ PairArgs a)
-{
+{ pdl_enter();
     using WL = Warps<HEAD, MODE>;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     unsigned char *S = smem_raw + ((1024u - (tc::smem_u32(smem_raw) & 1023u)) & 1023u);
@@ -998,11 +998,11 @@ int launch_pair_pipe(pimd_ctx *c, bool head, bool first)
         c->attr_done |= ATTR_PIPE;
     }
     if (head) {
-        if (first) pair_pipe_kernel<true, 0><<<c->num_sms, Warps<true, 0>::THREADS, smem, c->stream>>>(a);
-        else pair_pipe_kernel<true, 1><<<c->num_sms, Warps<true, 1>::THREADS, smem, c->stream>>>(a);
+        if (first) pimd_launch(pair_pipe_kernel<true, 0>, c->num_sms, Warps<true, 0>::THREADS, smem, c->stream, a);
+        else pimd_launch(pair_pipe_kernel<true, 1>, c->num_sms, Warps<true, 1>::THREADS, smem, c->stream, a);
     } else {
-        if (first) pair_pipe_kernel<false, 0><<<c->num_sms, Warps<false, 0>::THREADS, smem, c->stream>>>(a);
-        else pair_pipe_kernel<false, 1><<<c->num_sms, Warps<false, 1>::THREADS, smem, c->stream>>>(a);
+        if (first) pimd_launch(pair_pipe_kernel<false, 0>, c->num_sms, Warps<false, 0>::THREADS, smem, c->stream, a);
+        else pimd_launch(pair_pipe_kernel<false, 1>, c->num_sms, Warps<false, 1>::THREADS, smem, c->stream, a);
     }
     c->launches++;
     PIMD_CUDA_CHECK(cudaGetLastError());

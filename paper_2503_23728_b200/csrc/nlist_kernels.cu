@@ -35,7 +35,7 @@ struct NlArgs {
 
 // displacement since the candidate lists were built: any atom at or beyond skin/2 raises the rebuild flag
 __global__ void verlet_check_kernel(NlArgs a)
-{
+{ pdl_enter();
     int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (row >= a.rows) return;
     double d2 = 0.0;
@@ -47,7 +47,7 @@ __global__ void verlet_check_kernel(NlArgs a)
 }
 
 __global__ void bin_kernel(NlArgs a)
-{
+{ pdl_enter();
     if (!*a.need) return;
     int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (row >= a.rows) return;
@@ -104,7 +104,7 @@ __device__ __forceinline__ int block_exclusive_scan(int v, int *total)
 
 // one block per bead-system: cell_start (relative) = exclusive scan of cell_count; zero the cursors
 __global__ void __launch_bounds__(256) scan_cells_kernel(NlArgs a)
-{
+{ pdl_enter();
     if (!*a.need) return;
     __shared__ int tot;
     const int sys = blockIdx.x;
@@ -124,7 +124,7 @@ __global__ void __launch_bounds__(256) scan_cells_kernel(NlArgs a)
 }
 
 __global__ void scatter_kernel(NlArgs a)
-{
+{ pdl_enter();
     if (!*a.need) return;
     int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (row >= a.rows) return;
@@ -165,7 +165,7 @@ constexpr int CAND_CHUNK = 1024, COUNT_THREADS = 128, HOME_MAX = 128;
 // per-pair image shift can be left out.
 template <bool WRAP>
 __global__ void __launch_bounds__(COUNT_THREADS) count_cell_kernel(NlArgs a)
-{
+{ pdl_enter();
     __shared__ int sp[CAND_CHUNK];             // candidate: position in the cell-ordered arrays
     __shared__ int cfirst[28], cpre[28];       // first sorted position (relative to the system) and prefix count per stencil cell
     __shared__ int n_st;
@@ -311,7 +311,7 @@ __global__ void __launch_bounds__(COUNT_THREADS) count_cell_kernel(NlArgs a)
 // candidates of a row -> ascending j, in place: the row's candidates set bits in a per-warp bitmask over the atoms of the
 // bead-system (shared memory, N/32 words) and the set bits are written back in order.  N <= 32768 (checked by pimd_create).
 __global__ void __launch_bounds__(256) sort_candidates_kernel(NlArgs a, int nw)
-{
+{ pdl_enter();
     extern __shared__ unsigned smask[];       // [8][nw]
     if (!*a.need) return;
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -366,7 +366,7 @@ __global__ void __launch_bounds__(256) sort_candidates_kernel(NlArgs a, int nw)
 // around r_c^2, the fp64 predicate of S:L3 decides inside it; the ballots are kept as the row's hit mask.
 constexpr int MASK_WORDS = PIMD_MAX_NBR / 32;
 __global__ void __launch_bounds__(256) filter_count_kernel(NlArgs a)
-{
+{ pdl_enter();
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int64_t row = (int64_t)blockIdx.x * 8 + w;
     if (row >= a.rows) return;
@@ -401,7 +401,7 @@ __global__ void __launch_bounds__(256) filter_count_kernel(NlArgs a)
 
 // row_ptr: three-kernel exclusive scan over rows (1024 rows per block)
 __global__ void __launch_bounds__(1024) scan_rows_local_kernel(NlArgs a)
-{
+{ pdl_enter();
     __shared__ int tot;
     int64_t row = (int64_t)blockIdx.x * 1024 + threadIdx.x;
     int v = (row < a.rows) ? a.d.nnz[row] : 0;
@@ -411,7 +411,7 @@ __global__ void __launch_bounds__(1024) scan_rows_local_kernel(NlArgs a)
 }
 
 __global__ void __launch_bounds__(1024) scan_block_sums_kernel(NlArgs a, int nblocks)
-{
+{ pdl_enter();
     __shared__ int tot;
     long long carry = 0;
     for (int base = 0; base < nblocks; base += 1024) {
@@ -432,7 +432,7 @@ __global__ void __launch_bounds__(1024) scan_block_sums_kernel(NlArgs a, int nbl
 }
 
 __global__ void scan_rows_add_kernel(NlArgs a)
-{
+{ pdl_enter();
     int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (row < a.rows) a.d.row_ptr[row] += a.d.block_sums[row >> 10];
 }
@@ -440,7 +440,7 @@ __global__ void scan_rows_add_kernel(NlArgs a)
 // CSR fill with ascending rows and no sort: the row's hits set bits in a per-warp bitmask over the atoms of the bead-system
 // (shared memory, N/32 words), and the set bits are emitted in ascending order.  N <= 32768 (checked by pimd_create).
 __global__ void __launch_bounds__(256) fill_bitmask_kernel(NlArgs a, int nw)
-{
+{ pdl_enter();
     extern __shared__ unsigned smask[];       // [8][nw]
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int64_t row = (int64_t)blockIdx.x * 8 + w;
@@ -479,7 +479,7 @@ __global__ void __launch_bounds__(256) fill_bitmask_kernel(NlArgs a, int nw)
 
 // CSR fill: the row's hit mask selects from its sorted candidates, so the rows come out in ascending j
 __global__ void __launch_bounds__(256) filter_fill_kernel(NlArgs a)
-{
+{ pdl_enter();
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int64_t row = (int64_t)blockIdx.x * 8 + w;
     if (blockIdx.x == 0 && threadIdx.x == 0) *a.need_w = 0;   // the candidate lists are current; the next check may raise the flag again
@@ -502,7 +502,7 @@ __global__ void __launch_bounds__(256) filter_fill_kernel(NlArgs a)
 
 }  // namespace
 
-__global__ void set_flag_kernel(int *f, int v) { *f = v; }
+__global__ void set_flag_kernel(int *f, int v) { pdl_enter(); *f = v; }
 
 int pimd_launch_nlist(pimd_ctx *c)
 {
@@ -526,36 +526,36 @@ int pimd_launch_nlist(pimd_ctx *c)
     if (c->nl.skin == 0.0) {
         // no reuse: the cell-list pass at r_cut IS the list of this step (count -> scan -> fill through the bitmask, ascending j)
         a.d.nnz = a.d.ncand;           // the count kernel's output is the row length
-        set_flag_kernel<<<1, 1, 0, c->stream>>>(c->nl.need, 1);
+        pimd_launch(set_flag_kernel, 1, 1, 0, c->stream, c->nl.need, 1);
         PIMD_CUDA_CHECK(cudaMemsetAsync(c->nl.cell_count, 0, sizeof(int) * (size_t)a.nsys * a.nct, c->stream));
-        bin_kernel<<<gthr, 256, 0, c->stream>>>(a);
-        scan_cells_kernel<<<a.nsys, 256, 0, c->stream>>>(a);
-        scatter_kernel<<<gthr, 256, 0, c->stream>>>(a);
-        if (wrap) count_cell_kernel<true><<<(unsigned)(a.nsys * a.nct), COUNT_THREADS, 0, c->stream>>>(a);
-        else count_cell_kernel<false><<<(unsigned)(a.nsys * a.nct), COUNT_THREADS, 0, c->stream>>>(a);
-        scan_rows_local_kernel<<<nblk, 1024, 0, c->stream>>>(a);
-        scan_block_sums_kernel<<<1, 1024, 0, c->stream>>>(a, nblk);
-        scan_rows_add_kernel<<<gthr, 256, 0, c->stream>>>(a);
-        fill_bitmask_kernel<<<gwarp, 256, (size_t)8 * nw * sizeof(unsigned), c->stream>>>(a, nw);
+        pimd_launch(bin_kernel, gthr, 256, 0, c->stream, a);
+        pimd_launch(scan_cells_kernel, a.nsys, 256, 0, c->stream, a);
+        pimd_launch(scatter_kernel, gthr, 256, 0, c->stream, a);
+        if (wrap) pimd_launch(count_cell_kernel<true>, (unsigned)(a.nsys * a.nct), COUNT_THREADS, 0, c->stream, a);
+        else pimd_launch(count_cell_kernel<false>, (unsigned)(a.nsys * a.nct), COUNT_THREADS, 0, c->stream, a);
+        pimd_launch(scan_rows_local_kernel, nblk, 1024, 0, c->stream, a);
+        pimd_launch(scan_block_sums_kernel, 1, 1024, 0, c->stream, a, nblk);
+        pimd_launch(scan_rows_add_kernel, gthr, 256, 0, c->stream, a);
+        pimd_launch(fill_bitmask_kernel, gwarp, 256, (size_t)8 * nw * sizeof(unsigned), c->stream, a, nw);
         c->launches += 9;
         PIMD_CUDA_CHECK(cudaGetLastError());
         return 0;
     }
     // candidate lists (r_cut + skin): rebuilt only when the flag is up; these kernels return at once otherwise
-    verlet_check_kernel<<<gthr, 256, 0, c->stream>>>(a);
+    pimd_launch(verlet_check_kernel, gthr, 256, 0, c->stream, a);
     PIMD_CUDA_CHECK(cudaMemsetAsync(c->nl.cell_count, 0, sizeof(int) * (size_t)a.nsys * a.nct, c->stream));
-    bin_kernel<<<gthr, 256, 0, c->stream>>>(a);
-    scan_cells_kernel<<<a.nsys, 256, 0, c->stream>>>(a);
-    scatter_kernel<<<gthr, 256, 0, c->stream>>>(a);
-    if (wrap) count_cell_kernel<true><<<(unsigned)(a.nsys * a.nct), COUNT_THREADS, 0, c->stream>>>(a);
-    else count_cell_kernel<false><<<(unsigned)(a.nsys * a.nct), COUNT_THREADS, 0, c->stream>>>(a);
-    sort_candidates_kernel<<<gwarp, 256, (size_t)8 * nw * sizeof(unsigned), c->stream>>>(a, nw);
+    pimd_launch(bin_kernel, gthr, 256, 0, c->stream, a);
+    pimd_launch(scan_cells_kernel, a.nsys, 256, 0, c->stream, a);
+    pimd_launch(scatter_kernel, gthr, 256, 0, c->stream, a);
+    if (wrap) pimd_launch(count_cell_kernel<true>, (unsigned)(a.nsys * a.nct), COUNT_THREADS, 0, c->stream, a);
+    else pimd_launch(count_cell_kernel<false>, (unsigned)(a.nsys * a.nct), COUNT_THREADS, 0, c->stream, a);
+    pimd_launch(sort_candidates_kernel, gwarp, 256, (size_t)8 * nw * sizeof(unsigned), c->stream, a, nw);
     // exact list of this step, filtered from the candidates
-    filter_count_kernel<<<gwarp, 256, 0, c->stream>>>(a);
-    scan_rows_local_kernel<<<nblk, 1024, 0, c->stream>>>(a);
-    scan_block_sums_kernel<<<1, 1024, 0, c->stream>>>(a, nblk);
-    scan_rows_add_kernel<<<gthr, 256, 0, c->stream>>>(a);
-    filter_fill_kernel<<<gwarp, 256, 0, c->stream>>>(a);
+    pimd_launch(filter_count_kernel, gwarp, 256, 0, c->stream, a);
+    pimd_launch(scan_rows_local_kernel, nblk, 1024, 0, c->stream, a);
+    pimd_launch(scan_block_sums_kernel, 1, 1024, 0, c->stream, a, nblk);
+    pimd_launch(scan_rows_add_kernel, gthr, 256, 0, c->stream, a);
+    pimd_launch(filter_fill_kernel, gwarp, 256, 0, c->stream, a);
     c->launches += 11;
     PIMD_CUDA_CHECK(cudaGetLastError());
     return 0;
@@ -565,7 +565,7 @@ int pimd_launch_nlist(pimd_ctx *c)
 int pimd_launch_nlist_invalidate(pimd_ctx *c)
 {
     if (c->kind != 0) return 0;
-    set_flag_kernel<<<1, 1, 0, c->stream>>>(c->nl.need, 1);
+    pimd_launch(set_flag_kernel, 1, 1, 0, c->stream, c->nl.need, 1);
     c->launches++;
     PIMD_CUDA_CHECK(cudaGetLastError());
     return 0;

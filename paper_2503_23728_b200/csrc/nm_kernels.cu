@@ -114,11 +114,11 @@ __device__ __forceinline__ double spring_force(const NmArgs &a, const double *bQ
 // of one step does not depend on the step and can be captured once as a CUDA graph and replayed.
 __device__ __forceinline__ uint32_t step_of(const uint32_t *t_dev, uint32_t t_off) { return t_dev ? *t_dev - t_off : 0u; }
 
-__global__ void step_inc_kernel(uint32_t *t_dev) { *t_dev += 1u; }
+__global__ void step_inc_kernel(uint32_t *t_dev) { pdl_enter(); *t_dev += 1u; }
 
 template <int MODE>
 __global__ void __launch_bounds__(32 * NM_TY) nm_kernel(NmArgs a, const uint32_t *t_dev, uint32_t t_off)
-{
+{ pdl_enter();
     const uint32_t t = step_of(t_dev, t_off);
     extern __shared__ double sm[];
     const int P = a.P, TC = a.TC;
@@ -224,7 +224,7 @@ __global__ void __launch_bounds__(32 * NM_TY) nm_kernel(NmArgs a, const uint32_t
 constexpr int PG_BLOCKS = 64, PG_THREADS = 128;
 
 __global__ void __launch_bounds__(PG_THREADS) pileg_partial_kernel(NmArgs a, const uint32_t *t_dev, uint32_t t_off, uint32_t tag, int after_B, double *__restrict__ partial)
-{
+{ pdl_enter();
     const uint32_t t = step_of(t_dev, t_off);
     __shared__ double red[2][PG_THREADS];
     const int r = blockIdx.y, P = a.P, ncol = 3 * a.N;
@@ -255,7 +255,7 @@ __global__ void __launch_bounds__(PG_THREADS) pileg_partial_kernel(NmArgs a, con
 }
 
 __global__ void pileg_final_kernel(NmArgs a, const uint32_t *t_dev, uint32_t t_off, uint32_t tag, const double *__restrict__ partial, double *__restrict__ alpha)
-{
+{ pdl_enter();
     const uint32_t t = step_of(t_dev, t_off);
     const int r = blockIdx.x * blockDim.x + threadIdx.x;
     if (r >= a.R) return;
@@ -292,8 +292,8 @@ int launch_nm(pimd_ctx *c, const uint32_t *t_dev, uint32_t t_off)
     NmArgs a = make_args(c);
     if (MODE != 2 && c->thermostat == 1 && c->gamma_fs >= 0.0) {   // PILE-G: the replica's scale factor for this half-step
         const uint32_t tag = MODE == 0 ? 0u : 1u;
-        pileg_partial_kernel<<<dim3(PG_BLOCKS, c->R), PG_THREADS, 0, c->stream>>>(a, t_dev, t_off, tag, MODE == 1 ? 1 : 0, c->pileg_partial);
-        pileg_final_kernel<<<(c->R + 127) / 128, 128, 0, c->stream>>>(a, t_dev, t_off, tag, c->pileg_partial, c->pileg_alpha);
+        pimd_launch(pileg_partial_kernel, dim3(PG_BLOCKS, c->R), PG_THREADS, 0, c->stream, a, t_dev, t_off, tag, MODE == 1 ? 1 : 0, c->pileg_partial);
+        pimd_launch(pileg_final_kernel, (c->R + 127) / 128, 128, 0, c->stream, a, t_dev, t_off, tag, c->pileg_partial, c->pileg_alpha);
         c->launches += 2;
     }
     size_t smem = (size_t)4 * c->P * a.TC * sizeof(double);
@@ -304,7 +304,7 @@ int launch_nm(pimd_ctx *c, const uint32_t *t_dev, uint32_t t_off)
         c->attr_done |= ATTR_NM;
     }
     dim3 grid((3 * c->N + a.TC - 1) / a.TC, c->R), block(a.TC, NM_TY);
-    nm_kernel<MODE><<<grid, block, smem, c->stream>>>(a, t_dev, t_off);
+    pimd_launch(nm_kernel<MODE>, grid, block, smem, c->stream, a, t_dev, t_off);
     c->launches++;
     PIMD_CUDA_CHECK(cudaGetLastError());
     return 0;
@@ -313,7 +313,7 @@ int launch_nm(pimd_ctx *c, const uint32_t *t_dev, uint32_t t_off)
 // ---------------------------------------------------------------------------------------------
 __global__ void simple_forces_kernel(int kind, int N, int64_t n3, double w2, const double *__restrict__ mass,
                                      const double *__restrict__ q, double *__restrict__ F)
-{
+{ pdl_enter();
     int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= n3) return;
     if (kind == 2) { F[t] = 0.0; return; }
@@ -393,7 +393,7 @@ int pimd_launch_nm_pre(pimd_ctx *c) { return launch_nm<0>(c, c->step_dev, 0u); }
 int pimd_launch_nm_post(pimd_ctx *c) { return launch_nm<1>(c, c->step_dev, 1u); }
 int pimd_launch_step_inc(pimd_ctx *c)
 {
-    step_inc_kernel<<<1, 1, 0, c->stream>>>(c->step_dev);
+    pimd_launch(step_inc_kernel, 1, 1, 0, c->stream, c->step_dev);
     c->launches++;
     PIMD_CUDA_CHECK(cudaGetLastError());
     return 0;
@@ -403,7 +403,7 @@ int pimd_launch_simple_forces(pimd_ctx *c)
 {
     int64_t n3 = c->rows * 3;
     double w2 = c->harmonic_omega * c->harmonic_omega;
-    simple_forces_kernel<<<(unsigned)((n3 + 255) / 256), 256, 0, c->stream>>>(c->kind, c->N, n3, w2, c->mass, c->q, c->F);
+    pimd_launch(simple_forces_kernel, (unsigned)((n3 + 255) / 256), 256, 0, c->stream, c->kind, c->N, n3, w2, c->mass, c->q, c->F);
     c->launches++;
     PIMD_CUDA_CHECK(cudaGetLastError());
     return 0;
