@@ -122,6 +122,7 @@ struct pimd_ctx {
     float *xs0;                        // [S][H] W_s^0 Emb[s]
     float h_be1_half[128];             // HOST copy of b_e1 / 2 (passed to the pair kernels as kernel parameters)
     unsigned char *h1_img, *meta_img;  // [pair_cap/128 + 1] tile images kept between the pair passes of one evaluation (tc path)
+    bool nl_flag_up = false;           // host mirror: the rebuild flag of the neighbour list is known to be raised (direct path: it stays so)
     uint32_t *XE;                      // [rows][H] words gathered by the pair kernels: x bf16 in the low half, the word as fp32 = E x (tc::pack_x_y); aliases xfeat
     CUtensorMap tmap_xe, tmap_g;       // 2-D tensor maps [rows][128 x 32 bit] of XE and G for TMA tile::gather4 (four gathered rows per copy)
     float *nfeat, *xfeat, *mfeat, *Efeat, *Gfeat;   // [rows][H]

@@ -399,7 +399,18 @@ __global__ void __launch_bounds__(256) filter_count_kernel(NlArgs a)
     if (lane == 0) a.d.nnz[row] = cnt;
 }
 
-// row_ptr: three-kernel exclusive scan over rows (1024 rows per block)
+// the list's total: checked against the capacity, stored behind the last row
+__device__ __forceinline__ void store_total(const NlArgs &a, long long total)
+{
+    if (total > a.d.pair_cap || total > 2147483647LL) {
+        atomicOr(a.err, PIMD_FLAG_PAIRS);
+        total = 0;   // downstream kernels see an empty list instead of reading out of bounds
+    }
+    a.d.row_ptr[a.rows] = (int)total;
+}
+
+// row_ptr: exclusive scan over rows in two kernels (1024 rows per block; block offsets), the offsets are added by the fill kernel
+// of the list (row_start below).  Up to 1024 rows the first kernel is the whole scan.
 __global__ void __launch_bounds__(1024) scan_rows_local_kernel(NlArgs a)
 { pdl_enter();
     __shared__ int tot;
@@ -407,7 +418,22 @@ __global__ void __launch_bounds__(1024) scan_rows_local_kernel(NlArgs a)
     int v = (row < a.rows) ? a.d.nnz[row] : 0;
     int ex = block_exclusive_scan(v, &tot);
     if (row < a.rows) a.d.row_ptr[row] = ex;
-    if (threadIdx.x == 0) a.d.block_sums[blockIdx.x] = tot;
+    if (threadIdx.x == 0) {
+        if (gridDim.x == 1) { a.d.block_sums[0] = 0; store_total(a, tot); }
+        else a.d.block_sums[blockIdx.x] = tot;
+    }
+}
+
+// start of the row in the pair list: block-local prefix + block offset, stored as the final row_ptr by the row's warp (no other
+// warp reads this entry before the kernel ends)
+__device__ __forceinline__ int64_t row_start(const NlArgs &a, int64_t row, int lane)
+{
+    int base = 0;
+    if (lane == 0) {
+        base = a.d.row_ptr[row] + a.d.block_sums[row >> 10];
+        a.d.row_ptr[row] = base;
+    }
+    return (int64_t)__shfl_sync(0xffffffffu, base, 0);
 }
 
 __global__ void __launch_bounds__(1024) scan_block_sums_kernel(NlArgs a, int nblocks)
@@ -422,19 +448,7 @@ __global__ void __launch_bounds__(1024) scan_block_sums_kernel(NlArgs a, int nbl
         carry += tot;
         __syncthreads();
     }
-    if (threadIdx.x == 0) {
-        if (carry > a.d.pair_cap || carry > 2147483647LL) {
-            atomicOr(a.err, PIMD_FLAG_PAIRS);
-            carry = 0;   // downstream kernels see an empty list instead of reading out of bounds
-        }
-        a.d.row_ptr[a.rows] = (int)carry;
-    }
-}
-
-__global__ void scan_rows_add_kernel(NlArgs a)
-{ pdl_enter();
-    int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (row < a.rows) a.d.row_ptr[row] += a.d.block_sums[row >> 10];
+    if (threadIdx.x == 0) store_total(a, carry);
 }
 
 // CSR fill with ascending rows and no sort: the row's hits set bits in a per-warp bitmask over the atoms of the bead-system
@@ -445,11 +459,11 @@ __global__ void __launch_bounds__(256) fill_bitmask_kernel(NlArgs a, int nw)
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int64_t row = (int64_t)blockIdx.x * 8 + w;
     if (row >= a.rows) return;
+    const int64_t base = row_start(a, row, lane);
     if (a.d.row_ptr[a.rows] == 0) return;     // empty or overflowed list
     unsigned *mk = smask + (size_t)w * nw;
     const int n = a.d.nnz[row];
     const int *hits = a.d.hits + row * a.hit_stride;
-    const int64_t base = a.d.row_ptr[row];
     for (int t = lane; t < nw; t += 32) mk[t] = 0u;
     __syncwarp();
     for (int e = lane; e < n; e += 32) {
@@ -484,10 +498,10 @@ __global__ void __launch_bounds__(256) filter_fill_kernel(NlArgs a)
     const int64_t row = (int64_t)blockIdx.x * 8 + w;
     if (blockIdx.x == 0 && threadIdx.x == 0) *a.need_w = 0;   // the candidate lists are current; the next check may raise the flag again
     if (row >= a.rows) return;
+    int64_t base = row_start(a, row, lane);
     if (a.d.row_ptr[a.rows] == 0) return;     // empty or overflowed list
     const int n = a.d.ncand[row];
     const int *cand = a.d.hits + row * a.hit_stride;
-    int64_t base = a.d.row_ptr[row];
     for (int e0 = 0; e0 < n; e0 += 32) {
         const unsigned m = a.d.hitmask[row * MASK_WORDS + (e0 >> 5)];
         const int e = e0 + lane;
@@ -526,7 +540,11 @@ int pimd_launch_nlist(pimd_ctx *c)
     if (c->nl.skin == 0.0) {
         // no reuse: the cell-list pass at r_cut IS the list of this step (count -> scan -> fill through the bitmask, ascending j)
         a.d.nnz = a.d.ncand;           // the count kernel's output is the row length
-        pimd_launch(set_flag_kernel, 1, 1, 0, c->stream, c->nl.need, 1);
+        if (!c->nl_flag_up) {             // nothing lowers the flag on this path: raised once (after a change of the skin)
+            pimd_launch(set_flag_kernel, 1, 1, 0, c->stream, c->nl.need, 1);
+            c->nl_flag_up = true;
+            c->launches++;
+        }
         PIMD_CUDA_CHECK(cudaMemsetAsync(c->nl.cell_count, 0, sizeof(int) * (size_t)a.nsys * a.nct, c->stream));
         pimd_launch(bin_kernel, gthr, 256, 0, c->stream, a);
         pimd_launch(scan_cells_kernel, a.nsys, 256, 0, c->stream, a);
@@ -534,10 +552,9 @@ int pimd_launch_nlist(pimd_ctx *c)
         if (wrap) pimd_launch(count_cell_kernel<true>, (unsigned)(a.nsys * a.nct), COUNT_THREADS, 0, c->stream, a);
         else pimd_launch(count_cell_kernel<false>, (unsigned)(a.nsys * a.nct), COUNT_THREADS, 0, c->stream, a);
         pimd_launch(scan_rows_local_kernel, nblk, 1024, 0, c->stream, a);
-        pimd_launch(scan_block_sums_kernel, 1, 1024, 0, c->stream, a, nblk);
-        pimd_launch(scan_rows_add_kernel, gthr, 256, 0, c->stream, a);
+        if (nblk > 1) pimd_launch(scan_block_sums_kernel, 1, 1024, 0, c->stream, a, nblk);
         pimd_launch(fill_bitmask_kernel, gwarp, 256, (size_t)8 * nw * sizeof(unsigned), c->stream, a, nw);
-        c->launches += 9;
+        c->launches += 6 + (nblk > 1);
         PIMD_CUDA_CHECK(cudaGetLastError());
         return 0;
     }
@@ -553,10 +570,10 @@ int pimd_launch_nlist(pimd_ctx *c)
     // exact list of this step, filtered from the candidates
     pimd_launch(filter_count_kernel, gwarp, 256, 0, c->stream, a);
     pimd_launch(scan_rows_local_kernel, nblk, 1024, 0, c->stream, a);
-    pimd_launch(scan_block_sums_kernel, 1, 1024, 0, c->stream, a, nblk);
-    pimd_launch(scan_rows_add_kernel, gthr, 256, 0, c->stream, a);
+    if (nblk > 1) pimd_launch(scan_block_sums_kernel, 1, 1024, 0, c->stream, a, nblk);
     pimd_launch(filter_fill_kernel, gwarp, 256, 0, c->stream, a);
-    c->launches += 11;
+    c->nl_flag_up = false;               // (the fill kernel lowers the flag)
+    c->launches += 9 + (nblk > 1);
     PIMD_CUDA_CHECK(cudaGetLastError());
     return 0;
 }
@@ -566,6 +583,7 @@ int pimd_launch_nlist_invalidate(pimd_ctx *c)
 {
     if (c->kind != 0) return 0;
     pimd_launch(set_flag_kernel, 1, 1, 0, c->stream, c->nl.need, 1);
+    c->nl_flag_up = true;
     c->launches++;
     PIMD_CUDA_CHECK(cudaGetLastError());
     return 0;
