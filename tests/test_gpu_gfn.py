@@ -200,3 +200,32 @@ def test_tensor_core_path_is_bitwise_deterministic(cuda_device):
     a = gpu.forces().clone()
     for _ in range(3):
         assert torch.equal(a, gpu.forces())
+
+
+@pytest.mark.parametrize("scale_a", [0.0, 1e-30, 2.0])
+def test_tensor_core_path_edge_state_magnitudes(cuda_device, scale_a):
+    """The gathered word of the message passes holds x_j (bf16) and, read as fp32, y_j = E_j x_j (gfn_node_tc.cu, tc::pack_x_y).
+    E = 0 in every layer (W_a = b_a = 0: the word's high half is clamped to zero), E so small that y underflows, and E
+    twice its usual size must all stay within the bf16 bound of the oracle.  (At four times the Xavier scale the per-atom error
+    reaches 2.1e-2-2.3e-2 with this and with the earlier (x | E) encoding alike: the bound is a statement about the named workloads'
+    weight scale; at thirty times the head's fp16 operand overflows and the non-finite check trips.)"""
+    K, H, L = 64, 128, 3
+    rng = np.random.default_rng(77)
+    box, n_at, P = np.array([12.5, 13.0, 12.2]), 500, 2
+    x = rng.uniform(0, 1, (1, n_at, 3)) * box
+    sp = rng.integers(0, 3, n_at).astype(np.int32)
+    w = pi.pack_weights(4, 3, K, H, L, bias_scale=0.2)
+    off = 0
+    for name, shape in pi.weight_layout(3, K, H, L):
+        n = int(np.prod(shape))
+        if name.startswith("W_a.") or name.startswith("b_a."):
+            w[off:off + n] *= np.float32(scale_a)
+        off += n
+    spec = pi.NetSpec(0, 3, K, H, L, 0, 3.0, 1.0 / 12.0, 0.2, 0.0, w)
+    spec.gemm_dtype = 1
+    gpu, ref = make_pair(sp, x, box, P, 300.0, 0.25, 1.0, 0, spec)
+    spread_beads(gpu, ref, scale=0.05)
+    Fg, Fr = _forces_pair(gpu, ref)
+    assert np.isfinite(Fg).all() and np.abs(Fr).max() > 1e-3
+    for k in range(Fg.shape[1]):
+        assert_forces_bf16_spec(Fg[0, k], Fr[0, k], f"scale_a {scale_a} bead {k}")
