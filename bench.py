@@ -254,30 +254,30 @@ def run_ours(args):
     pairs_last = int(rp1[-1].item())
 
     # ---- end to end: the full dynamical state (q, p and the forces at q) of EVERY step comes from pinned host memory and
-    # goes back to it: H2D -> pimd_set_state + pimd_set_forces_cached -> pimd_step(1) -> pimd_get_state +
-    # pimd_get_forces_cached -> D2H, then a stream synchronisation (the host owns the result before the next step starts)
+    # goes back to it through the C-ABI with HOST pointers: pimd_set_state + pimd_set_forces_cached (H2D on the library's
+    # stream) -> pimd_step(1) -> pimd_get_forces_cached + pimd_get_state (D2H; pimd_get_state synchronises: the host owns the
+    # result before the next step starts)
     q, p, st = sim.get_state()
     F = sim.get_forces_cached()
     hq, hp, hF = q.cpu().pin_memory(), p.cpu().pin_memory(), F.cpu().pin_memory()
-    dq, dp, dF = torch.empty_like(q), torch.empty_like(p), torch.empty_like(F)
-    q2, p2, F2 = torch.empty_like(q), torch.empty_like(p), torch.empty_like(F)
+    hq2, hp2, hF2 = torch.empty_like(hq).pin_memory(), torch.empty_like(hp).pin_memory(), torch.empty_like(hF).pin_memory()
     e2e_steps = max(3, min(args.steps, 10))
     lib = pb.load_library()
     import ctypes as C
+    h = sim._h
+    sim.sync()
     barrier()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record(stream)
     for i in range(e2e_steps):
-        dq.copy_(hq, non_blocking=True); dp.copy_(hp, non_blocking=True); dF.copy_(hF, non_blocking=True)
-        sim.set_state_async(dq, dp, st + i)
-        sim.set_forces_cached(dF)
-        sim.step(1)
+        rc = lib.pimd_set_state(h, C.c_void_p(hq.data_ptr()), C.c_void_p(hp.data_ptr()), C.c_int64(st + i))
+        rc = rc or lib.pimd_set_forces_cached(h, C.c_void_p(hF.data_ptr()))
+        rc = rc or lib.pimd_step(h, 1)
+        rc = rc or lib.pimd_get_forces_cached(h, C.c_void_p(hF2.data_ptr()))
         stc = C.c_int64()
-        rc = lib.pimd_get_state(sim._h, C.c_void_p(q2.data_ptr()), C.c_void_p(p2.data_ptr()), C.byref(stc))
+        rc = rc or lib.pimd_get_state(h, C.c_void_p(hq2.data_ptr()), C.c_void_p(hp2.data_ptr()), C.byref(stc))
         assert rc == 0, lib.pimd_last_error()
-        sim.get_forces_cached(F2)
-        hq.copy_(q2, non_blocking=True); hp.copy_(p2, non_blocking=True); hF.copy_(F2, non_blocking=True)
-        stream.synchronize()
+        hq, hq2 = hq2, hq; hp, hp2 = hp2, hp; hF, hF2 = hF2, hF   # the step's output is the next step's input
     e1.record(stream)
     barrier()
     t_e2e = e0.elapsed_time(e1) * 1e-3
@@ -342,7 +342,7 @@ def run_ours(args):
             "wall_ms_per_step_incl_flush": 1e3 * wall / args.steps,
             "e2e": {"value": whole_job_value(w.rows, e2e_steps, world, t_e2e), "unit": UNIT, "h2d_bytes_per_step": state_bytes,
                     "d2h_bytes_per_step": state_bytes, "steps": e2e_steps,
-                    "path": "pinned host q,p,F -> H2D -> pimd_set_state + pimd_set_forces_cached -> pimd_step(1) -> pimd_get_state + pimd_get_forces_cached -> D2H -> stream sync, every step"},
+                    "path": "pinned host q,p,F -> pimd_set_state + pimd_set_forces_cached (host pointers: the H2D copies are inside the C-ABI calls) -> pimd_step(1) -> pimd_get_forces_cached + pimd_get_state (host pointers: D2H inside the calls; pimd_get_state synchronises), every step"},
             "gpu_launches": int(launches),
             "clocks": clocks,
             "kernel_ms_per_step": {k: v[0] / args.steps for k, v in prof.items()},

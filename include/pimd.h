@@ -125,17 +125,22 @@ int pimd_forces(pimd_ctx *ctx, float *d_out);
 /* h_out HOST [R].  Synchronises the stream. */
 int pimd_estimators(pimd_ctx *ctx, pimd_estimators_t *h_out);
 
-/* State access for parity tests and checkpoint/resume.  d_q, d_p DEVICE double [R][P][N][3]
- * (A, amu*A/fs * 103.6426965268 i.e. eV fs/A); either may be NULL.  `step` HOST.
- * pimd_get_state synchronises; pimd_set_state is asynchronous and invalidates the cached forces. */
+/* State access for parity tests, checkpoint/resume and a host-driven loop.  d_q, d_p double [R][P][N][3]
+ * (A, amu*A/fs * 103.6426965268 i.e. eV fs/A), in DEVICE memory or in PAGE-LOCKED HOST memory (the copies are
+ * cudaMemcpyAsync with cudaMemcpyDefault on the context's stream; pageable host memory is not supported: the caller
+ * could not know when an asynchronous copy has read it); either may be NULL.  `step` HOST.
+ * pimd_get_state synchronises (the buffers are the caller's when it returns); pimd_set_state is asynchronous -- the
+ * source buffers must stay untouched until the stream has passed the call (pimd_sync, or any synchronising call) --
+ * and invalidates the cached forces. */
 int pimd_get_state(pimd_ctx *ctx, double *d_q, double *d_p, int64_t *step);
 int pimd_set_state(pimd_ctx *ctx, const double *d_q, const double *d_p, int64_t step);
 
 /* The cached forces F(q) belong to a checkpoint too: a resume that restores them skips the force evaluation
  * pimd_set_state would otherwise trigger (same trajectory bit for bit either way; S:N3 step 4 recomputes F from q).
- *   pimd_get_forces_cached  d_F DEVICE double [R][P][N][3] eV/A, the forces at the current q (evaluated if stale);
+ *   pimd_get_forces_cached  d_F double [R][P][N][3] eV/A (device or page-locked host, as above), the forces at the current q
+ *                           (evaluated if stale);
  *                           asynchronous.
- *   pimd_set_forces_cached  d_F DEVICE; the caller asserts that d_F = F(q) for the q given to the last pimd_set_state.
+ *   pimd_set_forces_cached  d_F device or page-locked host; the caller asserts that d_F = F(q) for the q given to the last pimd_set_state.
  *                           Asynchronous; marks the cached forces valid. */
 int pimd_get_forces_cached(pimd_ctx *ctx, double *d_F);
 int pimd_set_forces_cached(pimd_ctx *ctx, const double *d_F);

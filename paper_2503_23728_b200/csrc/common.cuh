@@ -184,6 +184,7 @@ static inline cudaError_t pimd_launch(void (*kernel)(KArgs...), dim3 grid, dim3 
 int pimd_launch_init_momenta(pimd_ctx *c);
 int pimd_launch_nm_pre(pimd_ctx *c);                 // O B A with the noise of step *step_dev
 int pimd_launch_step_inc(pimd_ctx *c);               // *step_dev += 1
+int pimd_launch_set_step(pimd_ctx *c, uint32_t t);   // *step_dev = t
 int pimd_launch_nm_post(pimd_ctx *c);                // B O with the noise of step *step_dev - 1
 int pimd_launch_simple_forces(pimd_ctx *c);          // kinds 1, 2
 int pimd_launch_estimators(pimd_ctx *c);

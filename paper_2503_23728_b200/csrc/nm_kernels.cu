@@ -115,6 +115,7 @@ __device__ __forceinline__ double spring_force(const NmArgs &a, const double *bQ
 __device__ __forceinline__ uint32_t step_of(const uint32_t *t_dev, uint32_t t_off) { return t_dev ? *t_dev - t_off : 0u; }
 
 __global__ void step_inc_kernel(uint32_t *t_dev) { pdl_enter(); *t_dev += 1u; }
+__global__ void step_set_kernel(uint32_t *t_dev, uint32_t t) { pdl_enter(); *t_dev = t; }
 
 template <int MODE>
 __global__ void __launch_bounds__(32 * NM_TY) nm_kernel(NmArgs a, const uint32_t *t_dev, uint32_t t_off)
@@ -394,6 +395,14 @@ int pimd_launch_nm_post(pimd_ctx *c) { return launch_nm<1>(c, c->step_dev, 1u); 
 int pimd_launch_step_inc(pimd_ctx *c)
 {
     pimd_launch(step_inc_kernel, 1, 1, 0, c->stream, c->step_dev);
+    c->launches++;
+    PIMD_CUDA_CHECK(cudaGetLastError());
+    return 0;
+}
+
+int pimd_launch_set_step(pimd_ctx *c, uint32_t t)
+{
+    pimd_launch(step_set_kernel, 1, 1, 0, c->stream, c->step_dev, t);
     c->launches++;
     PIMD_CUDA_CHECK(cudaGetLastError());
     return 0;

@@ -762,10 +762,7 @@ int step_body(pimd_ctx *c)
 
 int sync_step_counter(pimd_ctx *c)
 {
-    const uint32_t t = (uint32_t)c->step;
-    PIMD_CUDA_CHECK(cudaMemcpyAsync(c->step_dev, &t, sizeof(t), cudaMemcpyHostToDevice, c->stream));
-    PIMD_CUDA_CHECK(cudaStreamSynchronize(c->stream));   // (t is a stack variable)
-    return 0;
+    return pimd_launch_set_step(c, (uint32_t)c->step);   // (a kernel argument: no host buffer to keep alive, no synchronisation)
 }
 
 }  // namespace
@@ -913,8 +910,8 @@ extern "C" int pimd_get_state(pimd_ctx *c, double *d_q, double *d_p, int64_t *st
     if (!c) { pimd_set_error("null context"); return PIMD_ERR_ARG; }
     if (int rc = enter(c)) return rc;
     const size_t bytes = sizeof(double) * (size_t)c->rows * 3;
-    if (d_q) PIMD_CUDA_CHECK(cudaMemcpyAsync(d_q, c->q, bytes, cudaMemcpyDeviceToDevice, c->stream));
-    if (d_p) PIMD_CUDA_CHECK(cudaMemcpyAsync(d_p, c->p, bytes, cudaMemcpyDeviceToDevice, c->stream));
+    if (d_q) PIMD_CUDA_CHECK(cudaMemcpyAsync(d_q, c->q, bytes, cudaMemcpyDefault, c->stream));
+    if (d_p) PIMD_CUDA_CHECK(cudaMemcpyAsync(d_p, c->p, bytes, cudaMemcpyDefault, c->stream));
     if (step) *step = c->step;
     return check_device_error(c);
 }
@@ -925,8 +922,8 @@ extern "C" int pimd_set_state(pimd_ctx *c, const double *d_q, const double *d_p,
     if (step < 0 || step > PIMD_MAX_STEP) { pimd_set_error("step %lld outside [0, 2^32 - 1] (the noise counter holds 32 bits)", (long long)step); return PIMD_ERR_ARG; }
     if (int rc = enter(c)) return rc;
     const size_t bytes = sizeof(double) * (size_t)c->rows * 3;
-    if (d_q) PIMD_CUDA_CHECK(cudaMemcpyAsync(c->q, d_q, bytes, cudaMemcpyDeviceToDevice, c->stream));
-    if (d_p) PIMD_CUDA_CHECK(cudaMemcpyAsync(c->p, d_p, bytes, cudaMemcpyDeviceToDevice, c->stream));
+    if (d_q) PIMD_CUDA_CHECK(cudaMemcpyAsync(c->q, d_q, bytes, cudaMemcpyDefault, c->stream));
+    if (d_p) PIMD_CUDA_CHECK(cudaMemcpyAsync(c->p, d_p, bytes, cudaMemcpyDefault, c->stream));
     c->step = step;
     c->forces_valid = 0;
     if (int rc = sync_step_counter(c)) return rc;
@@ -958,7 +955,7 @@ extern "C" int pimd_get_forces_cached(pimd_ctx *c, double *d_F)
     int rc;
     if ((rc = enter(c))) return rc;
     if (!c->forces_valid && (rc = compute_forces(c))) return rc;
-    PIMD_CUDA_CHECK(cudaMemcpyAsync(d_F, c->F, sizeof(double) * (size_t)c->rows * 3, cudaMemcpyDeviceToDevice, c->stream));
+    PIMD_CUDA_CHECK(cudaMemcpyAsync(d_F, c->F, sizeof(double) * (size_t)c->rows * 3, cudaMemcpyDefault, c->stream));
     return 0;
 }
 
@@ -966,7 +963,7 @@ extern "C" int pimd_set_forces_cached(pimd_ctx *c, const double *d_F)
 {
     if (!c || !d_F) { pimd_set_error("null argument"); return PIMD_ERR_ARG; }
     if (int rc = enter(c)) return rc;
-    PIMD_CUDA_CHECK(cudaMemcpyAsync(c->F, d_F, sizeof(double) * (size_t)c->rows * 3, cudaMemcpyDeviceToDevice, c->stream));
+    PIMD_CUDA_CHECK(cudaMemcpyAsync(c->F, d_F, sizeof(double) * (size_t)c->rows * 3, cudaMemcpyDefault, c->stream));
     c->forces_valid = 1;
     return 0;
 }

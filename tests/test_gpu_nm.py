@@ -169,3 +169,33 @@ def test_non_finite_positions_latch_the_nan_error(cuda_device):
     with pytest.raises(pb.PimdError) as e:
         gpu.sync()
     assert e.value.code == -4
+
+
+def test_state_accessors_take_page_locked_host_pointers(cuda_device):
+    """include/pimd.h: q, p and the cached forces may live in device memory or in page-locked host memory.  A trajectory
+    driven from pinned host buffers (set -> step -> get, every step) equals the one kept on the device, bit for bit."""
+    import ctypes as C
+    import torch
+    import paper_2503_23728_b200 as pb
+
+    w = pi.make_workload("fad_p8")
+    a = pb.PIMD.from_workload(w, device="cuda:0")
+    b = pb.PIMD.from_workload(w, device="cuda:0")
+    lib = pb.load_library()
+    a.step(3); b.step(3)
+    q, p, st = b.get_state()
+    F = b.get_forces_cached()
+    hq, hp, hF = q.cpu().pin_memory(), p.cpu().pin_memory(), F.cpu().pin_memory()
+    for i in range(4):
+        assert lib.pimd_set_state(b._h, C.c_void_p(hq.data_ptr()), C.c_void_p(hp.data_ptr()), C.c_int64(st + i)) == 0
+        assert lib.pimd_set_forces_cached(b._h, C.c_void_p(hF.data_ptr())) == 0
+        assert lib.pimd_step(b._h, 1) == 0
+        assert lib.pimd_get_forces_cached(b._h, C.c_void_p(hF.data_ptr())) == 0
+        stc = C.c_int64()
+        assert lib.pimd_get_state(b._h, C.c_void_p(hq.data_ptr()), C.c_void_p(hp.data_ptr()), C.byref(stc)) == 0
+        assert stc.value == st + i + 1
+    a.step(4)
+    qa, pa, sta = a.get_state()
+    assert sta == st + 4
+    assert torch.equal(qa.cpu(), hq) and torch.equal(pa.cpu(), hp)
+    assert torch.equal(a.get_forces_cached().cpu(), hF)
