@@ -143,7 +143,7 @@ struct ProfScope {
     ProfScope(pimd_ctx *ctx, int kind) : c(ctx) { if (c->prof) pimd_prof_begin(c, kind); }
     ~ProfScope() { if (c->prof) pimd_prof_end(c); }
 };
-enum { ATTR_PAIR32 = 1, ATTR_NODE32 = 2, ATTR_PIPE = 4, ATTR_NODETC = 8, ATTR_NM = 256 /* << MODE */ };
+enum { ATTR_PAIR32 = 1, ATTR_NODE32 = 2, ATTR_PIPE = 4, ATTR_NODETC = 8, ATTR_FILL = 16, ATTR_SORT = 32, ATTR_NM = 256 /* << MODE */ };
 enum { PROF_NM = 0, PROF_NLIST = 1, PROF_PAIR = 2, PROF_NODE = 3, PROF_HEAD = 4, PROF_OTHER = 5 };
 
 void pimd_set_error(const char *fmt, ...);

@@ -312,12 +312,13 @@ __global__ void __launch_bounds__(COUNT_THREADS) count_cell_kernel(NlArgs a)
 // bead-system (shared memory, N/32 words) and the set bits are written back in order.  N <= 32768 (checked by pimd_create).
 __global__ void __launch_bounds__(256) sort_candidates_kernel(NlArgs a, int nw)
 { pdl_enter();
-    extern __shared__ unsigned smask[];       // [8][nw]
+    extern __shared__ unsigned smask[];       // [8][nw] bitmask, [8][nw] set bits in the words before, [8][hit_stride] sorted row
     if (!*a.need) return;
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int64_t row = (int64_t)blockIdx.x * 8 + w;
     if (row >= a.rows) return;
-    unsigned *mk = smask + (size_t)w * nw;
+    unsigned *mk = smask + (size_t)w * nw, *pre = smask + (size_t)(8 + w) * nw;
+    int *stage = (int *)(smask + (size_t)16 * nw) + (size_t)w * a.hit_stride;
     const int n = a.d.ncand[row];
     int *hits = a.d.hits + row * a.hit_stride;
     for (int t = lane; t < nw; t += 32) mk[t] = 0u;
@@ -336,29 +337,31 @@ __global__ void __launch_bounds__(256) sort_candidates_kernel(NlArgs a, int nw)
         const int v = __shfl_up_sync(0xffffffffu, inc, o);
         if (lane >= o) inc += v;
     }
+    int run = inc - cnt;
+    for (int t = w0; t < w1; ++t) { pre[t] = (unsigned)run; run += __popc(mk[t]); }
+    __syncwarp();
     // a candidate is stored as j (15 bits) | image shift of the pair at the reference positions, five bits per axis (biased by 16:
     // positions are never wrapped, S:L2, so the shift can be several box lengths) | bit 30 if a shift does not fit (the filter
     // then takes the exact path).  The shift cannot change while the list is in use in a way that matters: a pair whose
     // minimum image flips is at least r_cut apart with either image (box >= 2 (r_cut + skin)).
+    // Every lane packs the candidates it holds; a candidate's place in the row is the number of set bits below it.  The row is
+    // put in order in shared memory and written back in place.
     const int64_t sbase = (row / a.N) * a.N;
     const double qi[3] = {a.q[row * 3], a.q[row * 3 + 1], a.q[row * 3 + 2]};
-    int *colp = hits + (inc - cnt);
-    for (int t = w0; t < w1; ++t) {
-        unsigned bits = mk[t];
-        while (bits) {
-            const int j = t * 32 + (__ffs(bits) - 1);
-            int packed = j;
+    for (int e = lane; e < n; e += 32) {
+        const int j = hits[e];
+        int packed = j;
 #pragma unroll
-            for (int ax = 0; ax < 3; ++ax) {
-                int sh = 0;
-                if (a.periodic) sh = (int)rint((a.q[(sbase + j) * 3 + ax] - qi[ax]) / a.box[ax]);
-                if (sh < -16 || sh > 15) { packed |= 1 << 30; sh = 0; }
-                packed |= (sh + 16) << (15 + 5 * ax);
-            }
-            *colp++ = packed;
-            bits &= bits - 1;
+        for (int ax = 0; ax < 3; ++ax) {
+            int sh = 0;
+            if (a.periodic) sh = (int)rint((a.q[(sbase + j) * 3 + ax] - qi[ax]) / a.box[ax]);
+            if (sh < -16 || sh > 15) { packed |= 1 << 30; sh = 0; }
+            packed |= (sh + 16) << (15 + 5 * ax);
         }
+        stage[(int)pre[j >> 5] + __popc(mk[j >> 5] & ((1u << (j & 31)) - 1u))] = packed;
     }
+    __syncwarp();
+    for (int e = lane; e < n; e += 32) hits[e] = stage[e];
 }
 
 // every step: the exact list from the sorted candidates.  One warp per row; a lane tests candidates e = lane, lane + 32, ...:
@@ -452,16 +455,17 @@ __global__ void __launch_bounds__(1024) scan_block_sums_kernel(NlArgs a, int nbl
 }
 
 // CSR fill with ascending rows and no sort: the row's hits set bits in a per-warp bitmask over the atoms of the bead-system
-// (shared memory, N/32 words), and the set bits are emitted in ascending order.  N <= 32768 (checked by pimd_create).
+// (shared memory, N/32 words); a hit's place in the row is the number of set bits below it (per-word prefix counts, then one
+// popc), so every hit is stored by the lane that holds it -- no serial walk over the set bits.  N <= 32768 (pimd_create).
 __global__ void __launch_bounds__(256) fill_bitmask_kernel(NlArgs a, int nw)
 { pdl_enter();
-    extern __shared__ unsigned smask[];       // [8][nw]
+    extern __shared__ unsigned smask[];       // [8][nw] bitmask, then [8][nw] set bits in the words before
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int64_t row = (int64_t)blockIdx.x * 8 + w;
     if (row >= a.rows) return;
     const int64_t base = row_start(a, row, lane);
     if (a.d.row_ptr[a.rows] == 0) return;     // empty or overflowed list
-    unsigned *mk = smask + (size_t)w * nw;
+    unsigned *mk = smask + (size_t)w * nw, *pre = smask + (size_t)(8 + w) * nw;
     const int n = a.d.nnz[row];
     const int *hits = a.d.hits + row * a.hit_stride;
     for (int t = lane; t < nw; t += 32) mk[t] = 0u;
@@ -480,15 +484,16 @@ __global__ void __launch_bounds__(256) fill_bitmask_kernel(NlArgs a, int nw)
         const int v = __shfl_up_sync(0xffffffffu, inc, o);
         if (lane >= o) inc += v;
     }
-    int *colp = a.d.col + base + (inc - cnt);
-    for (int t = w0; t < w1; ++t) {
-        unsigned bits = mk[t];
-        while (bits) {
-            *colp++ = t * 32 + (__ffs(bits) - 1);
-            bits &= bits - 1;
-        }
+    int run = inc - cnt;
+    for (int t = w0; t < w1; ++t) { pre[t] = (unsigned)run; run += __popc(mk[t]); }
+    __syncwarp();
+    int *col = a.d.col + base, *prow = a.d.pair_row + base;
+    for (int e = lane; e < n; e += 32) {
+        const int j = hits[e];
+        const int pos = (int)pre[j >> 5] + __popc(mk[j >> 5] & ((1u << (j & 31)) - 1u));
+        col[pos] = j;
+        prow[e] = (int)row;                   // coalesced
     }
-    for (int e = lane; e < n; e += 32) a.d.pair_row[base + e] = (int)row;   // coalesced, outside the divergent loop
 }
 
 // CSR fill: the row's hit mask selects from its sorted candidates, so the rows come out in ascending j
@@ -553,7 +558,12 @@ int pimd_launch_nlist(pimd_ctx *c)
         else pimd_launch(count_cell_kernel<false>, (unsigned)(a.nsys * a.nct), COUNT_THREADS, 0, c->stream, a);
         pimd_launch(scan_rows_local_kernel, nblk, 1024, 0, c->stream, a);
         if (nblk > 1) pimd_launch(scan_block_sums_kernel, 1, 1024, 0, c->stream, a, nblk);
-        pimd_launch(fill_bitmask_kernel, gwarp, 256, (size_t)8 * nw * sizeof(unsigned), c->stream, a, nw);
+        const size_t fill_smem = (size_t)16 * nw * sizeof(unsigned);
+        if (fill_smem > 48 * 1024 && !(c->attr_done & ATTR_FILL)) {   // (the first step of a context is never captured)
+            PIMD_CUDA_CHECK(cudaFuncSetAttribute(fill_bitmask_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024));
+            c->attr_done |= ATTR_FILL;
+        }
+        pimd_launch(fill_bitmask_kernel, gwarp, 256, fill_smem, c->stream, a, nw);
         c->launches += 6 + (nblk > 1);
         PIMD_CUDA_CHECK(cudaGetLastError());
         return 0;
@@ -566,7 +576,14 @@ int pimd_launch_nlist(pimd_ctx *c)
     pimd_launch(scatter_kernel, gthr, 256, 0, c->stream, a);
     if (wrap) pimd_launch(count_cell_kernel<true>, (unsigned)(a.nsys * a.nct), COUNT_THREADS, 0, c->stream, a);
     else pimd_launch(count_cell_kernel<false>, (unsigned)(a.nsys * a.nct), COUNT_THREADS, 0, c->stream, a);
-    pimd_launch(sort_candidates_kernel, gwarp, 256, (size_t)8 * nw * sizeof(unsigned), c->stream, a, nw);
+    {
+        const size_t sort_smem = ((size_t)16 * nw + (size_t)8 * c->nl.hit_stride) * sizeof(unsigned);
+        if (sort_smem > 48 * 1024 && !(c->attr_done & ATTR_SORT)) {
+            PIMD_CUDA_CHECK(cudaFuncSetAttribute(sort_candidates_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
+            c->attr_done |= ATTR_SORT;
+        }
+        pimd_launch(sort_candidates_kernel, gwarp, 256, sort_smem, c->stream, a, nw);
+    }
     // exact list of this step, filtered from the candidates
     pimd_launch(filter_count_kernel, gwarp, 256, 0, c->stream, a);
     pimd_launch(scan_rows_local_kernel, nblk, 1024, 0, c->stream, a);
