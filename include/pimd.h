@@ -180,6 +180,20 @@ int pimd_metad_cv(pimd_ctx *ctx, double *d_s, double *d_grad);
 int pimd_metad_gaussians(pimd_ctx *ctx, int replica, double *h_centres, double *h_heights, int cap, int *h_n);
 int pimd_metad_deposit_now(pimd_ctx *ctx);
 
+/* The Debye collective variable (cv 2 above: P:L215) WITHOUT a context and WITHOUT any allocation: for callers that
+ * cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it).  Same sum, block
+ * partition and summation order as pimd_metad_cv (bit-identical results); its per-block partial sums live in a fixed 128 KB
+ * device array inside the library (held by every GPU that loads the library until the process exits).
+ *   d_q        DEVICE double [n_systems][n_atoms][3] A;  d_species DEVICE int32 [n_atoms] (type index 0..n_species-1)
+ *   box        HOST [3] A, all > 0 (orthorhombic, minimum image) or all 0 (open);  f_species HOST [n_species];  Q in 1/A, > 0
+ *   d_s        DEVICE double [n_systems] out;  d_grad DEVICE double [n_systems][n_atoms][3] out, or NULL
+ * Limits: n_systems <= 256, n_atoms <= 8192, n_species <= 16; larger sizes return PIMD_ERR_ARG.  Asynchronous on `cuda_stream`
+ * (two kernel launches; no cudaMalloc, cudaFree or allocating library call).  Every call shares the scratch array: calls that
+ * OVERLAP on the GPU (different streams, parallel graph branches) race on it and must be serialised by the caller.  The
+ * array keeps the last call's contents; nothing in it needs clearing (each call writes every entry it reads). */
+int pimd_debye_cv_static(const double *d_q, const int32_t *d_species, int n_atoms, int n_systems, const double box[3],
+                         const double *f_species, int n_species, double Q, double *d_s, double *d_grad, void *cuda_stream);
+
 /* Waits for the stream and returns any latched device error. */
 int pimd_sync(pimd_ctx *ctx);
 

@@ -4,4 +4,4 @@ All arithmetic runs in the CUDA kernels behind the C-ABI of include/pimd.h; this
 marshals arguments.  PyTorch is used for device memory and the stream.  There is no CPU fallback:
 importing `PIMD` without the compiled library raises.
 """
-from .pimd import PIMD, NetParams, Estimators, load_library, library_path, PimdError, measure_fp32_fma_tflops  # noqa: F401
+from .pimd import PIMD, NetParams, Estimators, load_library, library_path, PimdError, measure_fp32_fma_tflops, debye_cv_static  # noqa: F401

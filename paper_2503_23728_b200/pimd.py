@@ -58,6 +58,7 @@ def load_library():
     L.pimd_metad_cv.argtypes = [vp, vp, vp]
     L.pimd_metad_gaussians.argtypes = [vp, C.c_int, dp, dp, C.c_int, C.POINTER(C.c_int)]
     L.pimd_metad_deposit_now.argtypes = [vp]
+    L.pimd_debye_cv_static.argtypes = [vp, vp, C.c_int, C.c_int, dp, dp, C.c_int, C.c_double, vp, vp, vp]
     L.pimd_set_nlist_skin.argtypes = [vp, C.c_double]
     L.pimd_nlist_rebuilds.argtypes = [vp, C.POINTER(C.c_int64)]
     L.pimd_forces.argtypes = [vp, vp]
@@ -87,6 +88,25 @@ def measure_fp32_fma_tflops(stream=None) -> float:
     v = C.c_double()
     _check(load_library().pimd_measure_fp32_fma_tflops(C.c_void_p(st.cuda_stream), C.byref(v)))
     return float(v.value)
+
+
+def debye_cv_static(q, species, box, f_species, Q, s_out, grad_out=None, stream=None):
+    """pimd_debye_cv_static (include/pimd.h): the Debye CV of every bead-system in q [n_systems][N][3] (float64 device tensor) into
+    s_out [n_systems] (and grad_out, same shape as q), with no device allocation inside the library.  species: int32 device tensor."""
+    import torch
+    assert q.dtype == torch.float64 and q.is_contiguous() and q.dim() == 3 and q.shape[2] == 3
+    assert species.dtype == torch.int32 and species.is_contiguous() and species.numel() == q.shape[1]
+    assert s_out.dtype == torch.float64 and s_out.is_contiguous() and s_out.numel() == q.shape[0]
+    if grad_out is not None:
+        assert grad_out.dtype == torch.float64 and grad_out.is_contiguous() and grad_out.shape == q.shape
+    b = np.ascontiguousarray(box, dtype=np.float64)
+    f = np.ascontiguousarray(f_species, dtype=np.float64)
+    st = stream if stream is not None else torch.cuda.current_stream(q.device)
+    with torch.cuda.device(q.device):
+        _check(load_library().pimd_debye_cv_static(
+            C.c_void_p(q.data_ptr()), C.c_void_p(species.data_ptr()), int(q.shape[1]), int(q.shape[0]),
+            b.ctypes.data_as(C.POINTER(C.c_double)), f.ctypes.data_as(C.POINTER(C.c_double)), int(f.size), float(Q),
+            C.c_void_p(s_out.data_ptr()), C.c_void_p(grad_out.data_ptr() if grad_out is not None else None), C.c_void_p(st.cuda_stream)))
 
 
 def _check(rc):
