@@ -60,6 +60,8 @@ struct NlistDev {
     int *block_sums;                   // [ceil(rows/1024)+1]
     int *col;                          // [pair_cap] local atom index j
     int *pair_row;                     // [pair_cap] global row i
+    float4 *dvec;                      // tcgen05 pipeline only, else null: [pair_cap] r_j - r_i (fp64 difference, minimum image,
+                                       // then fp32) | segment kind of the row inside the pair's 32-pair granule (int bits)
     int64_t pair_cap;
 };
 

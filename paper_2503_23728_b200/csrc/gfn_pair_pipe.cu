@@ -5,7 +5,8 @@
 // One persistent CTA per SM walks 128-pair tiles of the flat CSR pair list.  The roles below run concurrently on
 // different tiles and hand buffers to each other through mbarriers and named barriers only (no CTA-wide barrier in the loop).
 // First pair pass of a force evaluation (MODE 0):
-//   P   4 warps, thread = pair : indices, fp64 minimum image -> distance, cutoff weight, row-segment flags (meta ring);
+//   P   4 warps, thread = pair : row, column, displacement r_j - r_i and segment kind streamed from the neighbour list (the fill
+//                                kernel forms the fp64 minimum-image difference) -> distance, cutoff weight, row-segment flags (meta ring);
 //                                Gaussian RBF tile -> A1 (bf16, K-major, 128-byte swizzle)
 //   MMA 1 thread               : D1 = A1 (W_e1/2)^T  (4 x UMMA 128x128x16);  D2^T = W2 A2^T  (8 x UMMA), W2 = W_e2 or W_f1 W_e2/2
 //   H   4 warps, thread = pair : D1 (TMEM) + b -> SiLU -> A2 (bf16 operand of the second product)
@@ -96,6 +97,7 @@ struct PairArgs {
     double box[3], inv_box[3];
     float r_cut, wscale;
     const int *row_ptr, *col, *pair_row;
+    const float4 *dvec;                   // per pair: r_j - r_i (fp32 of the fp64 minimum-image difference) | segment kind (nlist_kernels.cu)
     int64_t rows;
     const double *q;
     const uint16_t *Wf2img;               // head: bf16 UMMA image of w_f2 replicated on 16 rows ([16][128], 4 KB)
@@ -179,34 +181,30 @@ __device__ __forceinline__ void role_P(const PairArgs &a, unsigned char *S, uint
     const float uc_scale = (float)(K - 1) / a.r_cut * RBF_C;
     const int64_t stride = (int64_t)gridDim.x * TP;
     int64_t pg = (int64_t)blockIdx.x * TP + p;
+    // everything role P needs of a pair is streamed, coalesced, one tile ahead: row, column, and the displacement r_j - r_i with
+    // the row's segment kind (written by the neighbour-list fill kernel: no dependent loads behind the indices)
     int row_n = -1, col_n = 0;
-    if (n_my > 0 && pg < n_pairs) { row_n = __ldg(a.pair_row + pg); col_n = __ldg(a.col + pg); }
+    float4 dv_n = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (n_my > 0 && pg < n_pairs) { row_n = __ldg(a.pair_row + pg); col_n = __ldg(a.col + pg); dv_n = __ldg(a.dvec + pg); }
     for (int it = 0; it < n_my; ++it, pg += stride) {
         const int row = row_n, cj = col_n;
-        if (it + 1 < n_my) {                      // indices of the next tile: in flight during this tile's arithmetic
+        const float4 dv = dv_n;
+        if (it + 1 < n_my) {                      // the next tile: in flight during this tile's arithmetic
             const int64_t pn = pg + stride;
             row_n = -1; col_n = 0;
-            if (pn < n_pairs) { row_n = __ldg(a.pair_row + pn); col_n = __ldg(a.col + pn); }
+            if (pn < n_pairs) { row_n = __ldg(a.pair_row + pn); col_n = __ldg(a.col + pn); dv_n = __ldg(a.dvec + pn); }
         }
         int jrow = 0, kind = 0;
         float w = 0.f, ux = 0.f, uy = 0.f, uz = 0.f, dist = 0.f;
         if (row >= 0) {
             const int sys = row / a.N;
             jrow = sys * a.N + cj;
-            const int rs = __ldg(a.row_ptr + row), re = __ldg(a.row_ptr + row + 1);
-            float f[3];
-#pragma unroll
-            for (int ax = 0; ax < 3; ++ax) {      // fp64 difference and minimum image, fp32 from there on
-                double dx = a.q[(size_t)jrow * 3 + ax] - a.q[(size_t)row * 3 + ax];
-                if (a.periodic) dx = dx - a.box[ax] * rint(dx * a.inv_box[ax]);
-                f[ax] = (float)dx;
-            }
-            const float d2 = fmaf(f[0], f[0], fmaf(f[1], f[1], f[2] * f[2]));
+            const float d2 = fmaf(dv.x, dv.x, fmaf(dv.y, dv.y, dv.z * dv.z));
             const float inv = rsqrtf(fmaxf(d2, 1e-24f));
             dist = d2 * inv;
-            ux = -f[0] * inv; uy = -f[1] * inv; uz = -f[2] * inv;
+            ux = -dv.x * inv; uy = -dv.y * inv; uz = -dv.z * inv;
             w = 0.5f * (cospif(dist * inv_rc) + 1.0f);   // c_ij alone: the record is shared by the message and head passes
-            kind = seg_kind(rs, re, pg & ~(int64_t)(GP - 1), GP);
+            kind = __float_as_int(dv.w);
         }
         int prev = __shfl_up_sync(FULL, row, 1);
         if (lane == 0) prev = -2;                 // a granule is a warp's 32 pairs: its first pair always starts a segment
@@ -979,7 +977,7 @@ int launch_pair_pipe(pimd_ctx *c, bool head, bool first)
     a.N = c->N; a.periodic = c->periodic;
     for (int k = 0; k < 3; ++k) { a.box[k] = c->box[k]; a.inv_box[k] = c->periodic ? 1.0 / c->box[k] : 0.0; }
     a.r_cut = c->net.r_cut; a.wscale = head ? 1.0f : c->net.agg_norm;
-    a.row_ptr = c->nl.row_ptr; a.col = c->nl.col; a.pair_row = c->nl.pair_row; a.rows = c->rows; a.q = c->q;
+    a.row_ptr = c->nl.row_ptr; a.col = c->nl.col; a.pair_row = c->nl.pair_row; a.dvec = c->nl.dvec; a.rows = c->rows; a.q = c->q;
     a.W1img = c->wimg_e1; a.W2img = head ? c->wimg_fe : c->wimg_e2; a.Wf2img = c->wimg_wf2;
     for (int k = 0; k < H; ++k) a.b1h[k] = c->h_be1_half[k];
     a.b2 = head ? c->net.bfe : c->net.be2;

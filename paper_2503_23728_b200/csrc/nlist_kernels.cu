@@ -454,6 +454,24 @@ __global__ void __launch_bounds__(1024) scan_block_sums_kernel(NlArgs a, int nbl
     if (threadIdx.x == 0) store_total(a, carry);
 }
 
+// Geometry of a pair for the tensor-core pair pipeline (gfn_pair_pipe.cu, role P), written where the pair is emitted: r_j - r_i as
+// the fp64 difference with the minimum image, then fp32 (S:G1: the value role P would otherwise form itself behind the dependent
+// load chain pair -> row, column -> positions), and the kind of the row's segment inside the pair's 32-pair granule
+// (0 whole row, 1 began in an earlier granule, 2 continues into a later one).
+__device__ __forceinline__ void store_pair_geometry(const NlArgs &a, const double (&qi)[3], int64_t sbase, int j, int64_t rs, int n, int64_t pos)
+{
+    float f[3];
+#pragma unroll
+    for (int ax = 0; ax < 3; ++ax) {
+        double dx = a.q[(sbase + j) * 3 + ax] - qi[ax];
+        if (a.periodic) dx = dx - a.box[ax] * rint(dx * (1.0 / a.box[ax]));
+        f[ax] = (float)dx;
+    }
+    const int64_t g0 = pos & ~(int64_t)31;
+    const int kind = (rs >= g0 && rs + n <= g0 + 32) ? 0 : ((rs < g0) ? 1 : 2);
+    a.d.dvec[pos] = make_float4(f[0], f[1], f[2], __int_as_float(kind));
+}
+
 // CSR fill with ascending rows and no sort: the row's hits set bits in a per-warp bitmask over the atoms of the bead-system
 // (shared memory, N/32 words); a hit's place in the row is the number of set bits below it (per-word prefix counts, then one
 // popc), so every hit is stored by the lane that holds it -- no serial walk over the set bits.  N <= 32768 (pimd_create).
@@ -488,11 +506,17 @@ __global__ void __launch_bounds__(256) fill_bitmask_kernel(NlArgs a, int nw)
     for (int t = w0; t < w1; ++t) { pre[t] = (unsigned)run; run += __popc(mk[t]); }
     __syncwarp();
     int *col = a.d.col + base, *prow = a.d.pair_row + base;
+    const int64_t sbase = (row / a.N) * a.N;
+    const double qi[3] = {a.q[row * 3], a.q[row * 3 + 1], a.q[row * 3 + 2]};
     for (int e = lane; e < n; e += 32) {
         const int j = hits[e];
         const int pos = (int)pre[j >> 5] + __popc(mk[j >> 5] & ((1u << (j & 31)) - 1u));
         col[pos] = j;
         prow[e] = (int)row;                   // coalesced
+    }
+    if (a.d.dvec) {                           // second walk, in list order: coalesced 16-byte stores, ascending j
+        __syncwarp();
+        for (int e = lane; e < n; e += 32) store_pair_geometry(a, qi, sbase, col[e], base, n, base + e);
     }
 }
 
@@ -507,13 +531,18 @@ __global__ void __launch_bounds__(256) filter_fill_kernel(NlArgs a)
     if (a.d.row_ptr[a.rows] == 0) return;     // empty or overflowed list
     const int n = a.d.ncand[row];
     const int *cand = a.d.hits + row * a.hit_stride;
+    const int64_t rs = base, sbase = (row / a.N) * a.N;
+    const int nn = a.d.nnz[row];
+    const double qi[3] = {a.q[row * 3], a.q[row * 3 + 1], a.q[row * 3 + 2]};
     for (int e0 = 0; e0 < n; e0 += 32) {
         const unsigned m = a.d.hitmask[row * MASK_WORDS + (e0 >> 5)];
         const int e = e0 + lane;
         if ((m >> lane) & 1u) {
             const int pos = __popc(m & ((1u << lane) - 1u));
-            a.d.col[base + pos] = cand[e] & 0x7FFF;
+            const int j = cand[e] & 0x7FFF;
+            a.d.col[base + pos] = j;
             a.d.pair_row[base + pos] = (int)row;
+            if (a.d.dvec) store_pair_geometry(a, qi, sbase, j, rs, nn, base + pos);
         }
         base += __popc(m);
     }

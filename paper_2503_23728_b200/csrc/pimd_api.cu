@@ -61,7 +61,7 @@ namespace {
 
 struct Layout {
     size_t q, p, F, species, mass, C, CT, omega, lam, gam, Tstage, pileg_partial, pileg_alpha, md_n, md_gc, md_gh, md_s, md_dV, md_grad, md_partial, err, est_partial, est_out;
-    size_t cell_id, cell_count, cell_start, cell_cursor, sorted_atom, sorted_q, nnz, ncand, hits, hitmask, q_ref, q32, need, row_ptr, block_sums, col, pair_row;
+    size_t cell_id, cell_count, cell_start, cell_cursor, sorted_atom, sorted_q, nnz, ncand, hits, hitmask, q_ref, q32, need, row_ptr, block_sums, col, pair_row, dvec;
     size_t wimg, wimg_node, xs0, h1_img, meta_img, weights, nfeat, xfeat, mfeat, Efeat, Gfeat, carry_m, carry_f, Fraw;
     size_t total;
     int ncell[3], nct;
@@ -189,6 +189,7 @@ int compute_layout(int N, int R, int P, const double box[3], const pimd_net_para
         L->block_sums = take(cur, sizeof(int) * ((rows + 1023) / 1024 + 1));
         L->col = take(cur, sizeof(int) * L->pair_cap);
         L->pair_row = take(cur, sizeof(int) * L->pair_cap);
+        L->dvec = (net->gemm_dtype == 1 && net->n_rbf == 64 && H == 128) ? take(cur, sizeof(float) * 4 * L->pair_cap) : (size_t)-1;
         L->weights = take(cur, sizeof(float) * L->n_wfloats);
         L->wimg = take(cur, 5 * 16384 + 4096);   // bf16 UMMA images: W_e1 (16 KB), W_e2 (32 KB), W_f1 W_e2 (32 KB)
         L->wimg_node = take(cur, (size_t)(net->n_layers > 0 ? net->n_layers : 1) * 20 * 16384);   // 20 half-images (16 KB) per layer: gfn_node_tc.cu
@@ -538,7 +539,7 @@ extern "C" int pimd_create(pimd_ctx **out, int n_atoms, int n_replicas, const in
         nl.q_ref = (double *)(ws + L.q_ref); nl.q32 = (float4 *)(ws + L.q32); nl.need = (int *)(ws + L.need); nl.skin = 0.0;
         CREATE_CHECK(cudaMemsetAsync(nl.need, 0, sizeof(int) * 4, st));
         nl.hits = (int *)(ws + L.hits); nl.hit_stride = L.hit_stride; nl.row_ptr = (int *)(ws + L.row_ptr); nl.block_sums = (int *)(ws + L.block_sums);
-        nl.col = (int *)(ws + L.col); nl.pair_row = (int *)(ws + L.pair_row); nl.pair_cap = L.pair_cap;
+        nl.col = (int *)(ws + L.col); nl.pair_row = (int *)(ws + L.pair_row); nl.dvec = (L.dvec == (size_t)-1) ? nullptr : (float4 *)(ws + L.dvec); nl.pair_cap = L.pair_cap;
         c->weights_dev = (float *)(ws + L.weights);
         c->nfeat = (float *)(ws + L.nfeat); c->xfeat = (float *)(ws + L.xfeat); c->mfeat = (float *)(ws + L.mfeat);
         c->Efeat = (float *)(ws + L.Efeat); c->Gfeat = (float *)(ws + L.Gfeat);

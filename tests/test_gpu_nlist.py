@@ -138,3 +138,21 @@ def test_skin_is_limited_by_the_box(cuda_device):
     with pytest.raises(pb.PimdError):
         g.set_nlist_skin(0.5)      # 2 (6 + 0.5) > 12.42
     g.set_nlist_skin(0.1)
+
+
+def test_list_reuse_on_the_tensor_core_path_is_bitwise_the_direct_path(cuda_device):
+    """On the tcgen05 configs both fill kernels (direct and filtered) also write the per-pair displacement and segment kind that
+    the first pair pass streams (nlist_kernels.cu: store_pair_geometry): with and without list reuse the trajectory must be the
+    same bit for bit, across rebuilds."""
+    w = pi.make_workload("ice512")
+    w.P = 2
+    a = pb.PIMD.from_workload(w, device="cuda:0")
+    b = pb.PIMD.from_workload(w, device="cuda:0")
+    a.set_nlist_skin(0.5)
+    b.set_nlist_skin(0.0)
+    for it in range(3):
+        a.step(8); b.step(8)
+        qa, pa, _ = a.get_state(); qb, pb_, _ = b.get_state()
+        assert torch.equal(qa, qb) and torch.equal(pa, pb_)
+    na, nb = a.nlist_rebuilds(), b.nlist_rebuilds()
+    assert nb >= 24 and 2 <= na < nb, (na, nb)
