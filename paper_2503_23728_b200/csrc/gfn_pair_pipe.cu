@@ -224,12 +224,23 @@ __device__ __forceinline__ void role_P(const PairArgs &a, unsigned char *S, uint
         // ---- RBF tile -> A1 (bf16, K-major rows of 128 B, 16-byte chunks XOR-swizzled by row & 7)
         unsigned char *A1 = S + OFF_A1 + (it & 1) * 16384 + p * 128;
         const float uc = dist * uc_scale;         // C d / delta
+        // Only the basis functions within 8 widths of d are evaluated: three 8-function chunks starting at chunk c0 cover every
+        // k with |k - d/delta| <= 8; the others are below exp(-32) = 1.3e-14 of the largest and are stored as zeros.  (Per-thread
+        // chunk index, warp-uniform control flow: the pairs of a warp have unrelated distances.)
+        const int c0 = min(max((int)floorf((uc * (1.0f / RBF_C) - 8.0f) * 0.125f), 0), 5);
 #pragma unroll
-        for (int ch = 0; ch < 8; ++ch) {
+        for (int z = 0; z < 5; ++z) {
+            const int ch = (z < c0) ? z : z + 3;
+            *(uint4 *)(A1 + ((ch ^ (p & 7)) << 4)) = make_uint4(0u, 0u, 0u, 0u);
+        }
+#pragma unroll
+        for (int c3 = 0; c3 < 3; ++c3) {
+            const int ch = c0 + c3;
+            const float ub = uc - (RBF_C * 8.0f) * (float)ch;
             float g[8];
 #pragma unroll
             for (int e = 0; e < 8; ++e) {
-                const float t = uc - RBF_C * (float)(ch * 8 + e);
+                const float t = ub - RBF_C * (float)e;
                 g[e] = ex2_approx(-t * t);
             }
             *(uint4 *)(A1 + ((ch ^ (p & 7)) << 4)) =
