@@ -165,6 +165,8 @@ void pimd_set_error(const char *fmt, ...);
 // pdl_enter() (griddepcontrol.wait returns when the grids before it have completed and flushed): it is the first statement of
 // every such kernel.  No kernel triggers its dependents early (griddepcontrol.launch_dependents): measured, early-resident
 // blocks of the next kernel cost fad_x64_p32 +26 % per step and ice512 gained nothing over the implicit trigger at exit.
+// Nor does it pay in the two big persistent kernels alone (trigger at entry, wait after barrier initialisation, TMEM allocation and
+// the copies of the static weights, so that the next kernel's blocks set themselves up on SMs whose block has finished): ice512 +4 %.
 #if defined(__CUDACC__)
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void pdl_enter() { pdl_wait(); }
