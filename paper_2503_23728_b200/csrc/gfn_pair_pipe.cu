@@ -355,7 +355,7 @@ __device__ __forceinline__ void role_E_msg(const PairArgs &a, unsigned char *S, 
         const int64_t gidx = (tile0 >> 5) + qt;
         const uint32_t td2 = tmem + 256 + (it & 1) * 128 + lane_field;
         st.s1 = 0.f; st.s2 = 0.f;
-#pragma unroll 1
+#pragma unroll
         for (int cc = 0; cc < 2; ++cc) {
             const int q0 = qt * 32 + cc * 16, slot = qt * 2 + cc;   // ring slot = 16 pairs
             if (poller) {
@@ -598,7 +598,7 @@ __device__ __forceinline__ void role_E_head_tc(const PairArgs &a, unsigned char 
         const uint32_t td2 = tmem + 256 + (it & 1) * 128 + lane_field;
         float be = 0.f;
         int cur_row = -2;
-#pragma unroll 1
+#pragma unroll
         for (int cc = 0; cc < 2; ++cc) {
             const int q0 = qt * 32 + cc * 16, slot = qt * 2 + cc;
             if (poller) {
