@@ -229,3 +229,25 @@ def test_tensor_core_path_edge_state_magnitudes(cuda_device, scale_a):
     assert np.isfinite(Fg).all() and np.abs(Fr).max() > 1e-3
     for k in range(Fg.shape[1]):
         assert_forces_bf16_spec(Fg[0, k], Fr[0, k], f"scale_a {scale_a} bead {k}")
+
+
+def test_tensor_core_path_window_of_the_radial_basis_at_its_ends(cuda_device):
+    """Role P evaluates only the 24 Gaussian basis functions around the pair distance (gfn_pair_pipe.cu).  Pairs at the two ends
+    of the basis -- 0.05 A apart and just inside the cutoff -- exercise the clamped windows; a pair just outside contributes nothing."""
+    K, H, L = 64, 128, 2
+    rc = 3.0
+    base = np.array([[0.0, 0.0, 0.0], [0.05, 0.0, 0.0],                 # almost on top of each other
+                     [0.0, 4.0, 0.0], [rc - 1e-4, 4.0, 0.0],            # just inside r_cut
+                     [0.0, 8.0, 0.0], [rc + 1e-4, 8.0, 0.0],            # just outside: no pair
+                     [0.0, 12.0, 0.0], [1.47, 12.0, 0.0], [0.3, 13.1, 0.0]])
+    pos = np.stack([base, base + np.array([0.01, -0.02, 0.03])])
+    sp = np.array([0, 1, 2, 0, 1, 2, 0, 1, 2], dtype=np.int32)
+    spec = _biased_spec(K, H, L, rc, 1.0 / 12.0, 0.2)
+    spec.gemm_dtype = 1
+    gpu, ref = make_pair(sp, pos, np.zeros(3), 2, 300.0, 0.25, 1.0, 0, spec)
+    Fg, Fr = _forces_pair(gpu, ref)
+    assert np.isfinite(Fg).all()
+    assert np.all(Fg[:, :, 4:6] == 0.0) and np.all(Fr[:, :, 4:6] == 0.0)
+    for rr in range(2):
+        for k in range(2):
+            assert_forces_bf16_spec(Fg[rr, k], Fr[rr, k], f"replica {rr} bead {k}")
