@@ -19,7 +19,7 @@ namespace {
 struct NlArgs {
     int N, nsys, periodic;
     int64_t rows;
-    double box[3];
+    double box[3], inv_box[3];     // inv_box = 1 / box (0 when not periodic)
     double rc2;
     double rl2;                    // (r_cut + skin)^2: candidate radius of the cell-list pass
     float rc2_lo, rc2_hi;          // fp32 pre-filter band around the candidate radius^2 (exact fp64 test inside the band)
@@ -464,7 +464,7 @@ __device__ __forceinline__ void store_pair_geometry(const NlArgs &a, const doubl
 #pragma unroll
     for (int ax = 0; ax < 3; ++ax) {
         double dx = a.q[(sbase + j) * 3 + ax] - qi[ax];
-        if (a.periodic) dx = dx - a.box[ax] * rint(dx * (1.0 / a.box[ax]));
+        if (a.periodic) dx = dx - a.box[ax] * rint(dx * a.inv_box[ax]);
         f[ax] = (float)dx;
     }
     const int64_t g0 = pos & ~(int64_t)31;
@@ -556,7 +556,7 @@ int pimd_launch_nlist(pimd_ctx *c)
 {
     NlArgs a;
     a.N = c->N; a.nsys = c->R * c->P; a.periodic = c->periodic; a.rows = c->rows;
-    for (int k = 0; k < 3; ++k) { a.box[k] = c->box[k]; a.nc[k] = c->nl.ncell[k]; }
+    for (int k = 0; k < 3; ++k) { a.box[k] = c->box[k]; a.inv_box[k] = c->periodic ? 1.0 / c->box[k] : 0.0; a.nc[k] = c->nl.ncell[k]; }
     a.rc2 = (double)c->net.r_cut * (double)c->net.r_cut;
     const double rl = (double)c->net.r_cut + c->nl.skin;
     a.rl2 = rl * rl;
