@@ -520,6 +520,69 @@ __global__ void __launch_bounds__(256) fill_bitmask_kernel(NlArgs a, int nw)
     }
 }
 
+// ---- small open clusters (one cell per bead-system, N <= BRUTE_MAX_N: the FAD configs): the cell machinery above is seven launches
+// for a list that one thread per row writes directly.  Thread = row i; j runs over the bead-system in ascending order with the
+// exact S:L3 predicate (the definition itself: S:L1), so the rows are ascending by construction.
+//   SINGLE: rows <= 1024, one block is the whole list: count, block scan, fill in one launch.
+//   else  : brute_count_kernel (count + block-local scan + block sums), scan_block_sums_kernel, brute_fill_kernel.
+constexpr int BRUTE_MAX_N = 128;
+
+__device__ __forceinline__ int brute_row(const NlArgs &a, int64_t row, int64_t base, bool write)
+{
+    const int64_t sbase = (row / a.N) * a.N;
+    const int i = (int)(row - sbase);
+    const double qi[3] = {a.q[row * 3], a.q[row * 3 + 1], a.q[row * 3 + 2]};
+    int n = 0;
+    for (int j = 0; j < a.N; ++j) {
+        if (j == i || !within_cutoff(qi, a.q + (sbase + j) * 3, a, a.rc2)) continue;
+        if (write) { a.d.col[base + n] = j; a.d.pair_row[base + n] = (int)row; }
+        ++n;
+    }
+    return n;
+}
+
+__device__ __forceinline__ void brute_geometry(const NlArgs &a, int64_t row, int64_t base, int n)
+{
+    if (!a.d.dvec) return;
+    const int64_t sbase = (row / a.N) * a.N;
+    const double qi[3] = {a.q[row * 3], a.q[row * 3 + 1], a.q[row * 3 + 2]};
+    for (int e = 0; e < n; ++e) store_pair_geometry(a, qi, sbase, a.d.col[base + e], base, n, base + e);
+}
+
+template <bool SINGLE>
+__global__ void __launch_bounds__(1024) brute_count_kernel(NlArgs a)
+{ pdl_enter();
+    __shared__ int tot;
+    const int64_t row = (int64_t)blockIdx.x * 1024 + threadIdx.x;
+    if (row == 0) a.need_w[1] += 1;            // rebuild counter (pimd_nlist_rebuilds)
+    const int n = (row < a.rows) ? brute_row(a, row, 0, false) : 0;
+    const int ex = block_exclusive_scan(n, &tot);
+    if (!SINGLE) {
+        if (row < a.rows) { a.d.nnz[row] = n; a.d.row_ptr[row] = ex; }
+        if (threadIdx.x == 0) a.d.block_sums[blockIdx.x] = tot;
+        return;
+    }
+    // the whole list is this block's
+    const bool fits = (long long)tot <= a.d.pair_cap;
+    if (threadIdx.x == 0) { a.d.block_sums[0] = 0; store_total(a, tot); }
+    if (row < a.rows) {
+        a.d.nnz[row] = n;
+        a.d.row_ptr[row] = fits ? ex : 0;
+        if (fits && n > 0) { brute_row(a, row, ex, true); brute_geometry(a, row, ex, n); }
+    }
+}
+
+__global__ void __launch_bounds__(256) brute_fill_kernel(NlArgs a)
+{ pdl_enter();
+    const int64_t row = (int64_t)blockIdx.x * 256 + threadIdx.x;
+    if (row >= a.rows) return;
+    const int base = a.d.row_ptr[row] + a.d.block_sums[row >> 10];
+    a.d.row_ptr[row] = base;
+    if (a.d.row_ptr[a.rows] == 0) return;      // empty or overflowed list
+    const int n = a.d.nnz[row];
+    if (n > 0) { brute_row(a, row, base, true); brute_geometry(a, row, base, n); }
+}
+
 // CSR fill: the row's hit mask selects from its sorted candidates, so the rows come out in ascending j
 __global__ void __launch_bounds__(256) filter_fill_kernel(NlArgs a)
 { pdl_enter();
@@ -571,6 +634,20 @@ int pimd_launch_nlist(pimd_ctx *c)
     const int nblk = (int)((rows + 1023) / 1024);
     const int nw = (c->N + 31) / 32;
     const bool wrap = a.periodic && (a.nc[0] < 4 || a.nc[1] < 4 || a.nc[2] < 4);
+    if (c->nl.skin == 0.0 && a.nct == 1 && c->N <= BRUTE_MAX_N) {
+        // small open clusters: one thread per row, one launch up to 1024 rows, three above
+        if (nblk == 1) {
+            pimd_launch(brute_count_kernel<true>, 1, 1024, 0, c->stream, a);
+            c->launches += 1;
+        } else {
+            pimd_launch(brute_count_kernel<false>, nblk, 1024, 0, c->stream, a);
+            pimd_launch(scan_block_sums_kernel, 1, 1024, 0, c->stream, a, nblk);
+            pimd_launch(brute_fill_kernel, gthr, 256, 0, c->stream, a);
+            c->launches += 3;
+        }
+        PIMD_CUDA_CHECK(cudaGetLastError());
+        return 0;
+    }
     if (c->nl.skin == 0.0) {
         // no reuse: the cell-list pass at r_cut IS the list of this step (count -> scan -> fill through the bitmask, ascending j)
         a.d.nnz = a.d.ncand;           // the count kernel's output is the row length
