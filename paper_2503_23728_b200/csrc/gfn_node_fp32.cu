@@ -60,6 +60,17 @@ __global__ void __launch_bounds__(NT, 1) node_kernel(NodeArgs a)
     const int64_t row0 = (int64_t)blockIdx.x * TP;
     const int n_pairs = a.row_ptr[a.rows];
 
+    // The weight matrices go through one shared-memory slab, each load in front of its product.  A layer's matrices are touched
+    // once per step: their lines are requested into L2 now, so that the five loads below do not each pay a DRAM round trip.
+    {
+        const float *mats[5] = {a.mode == 1 ? a.WvnT : nullptr, a.mode == 1 ? a.WvmT : nullptr, a.mode == 1 ? a.Wv2T : nullptr,
+                                a.mode == 1 ? a.WaT : nullptr, a.WnextT};
+#pragma unroll
+        for (int m = 0; m < 5; ++m)
+            if (mats[m])
+                for (int i = tid * 32; i < H * H; i += NT * 32) asm volatile("prefetch.global.L2 [%0];" ::"l"(mats[m] + i));
+    }
+
     // ---- load the tile transposed into the k-major buffers
     for (int idx = tid; idx < TP * H / 4; idx += NT) {
         const int r = idx / (H / 4), c4 = idx % (H / 4), c0 = c4 * 4;
