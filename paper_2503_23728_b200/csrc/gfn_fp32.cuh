@@ -26,38 +26,40 @@ struct Tile {
 };
 
 // acc[p][c] += sum_k A[k][p] * W[k][c];  A swizzled [KD][TP], W [KD][H]
-template <int KD, int H>
+// RP = rows per thread: 8 (the whole 128-row tile) or 4 (only rows 0..63 of the buffers are in use: half tiles, for
+// configurations with fewer tiles than SMs)
+template <int KD, int H, int RP = 8>
 __device__ __forceinline__ void tile_gemm(const float *__restrict__ sA, const float *__restrict__ sW,
-                                          float (&acc)[8][Tile<H>::CPT], int tx, int ty)
+                                          float (&acc)[RP][Tile<H>::CPT], int tx, int ty)
 {
     constexpr int CPT = Tile<H>::CPT;
 #pragma unroll 4
     for (int k = 0; k < KD; ++k) {
         const int sw = swz(k);
-        float a[8], b[CPT];
+        float a[RP], b[CPT];
         *(float4 *)&a[0] = *(const float4 *)&sA[k * TP + ((ty * 4) ^ sw)];
-        *(float4 *)&a[4] = *(const float4 *)&sA[k * TP + ((TP / 2 + ty * 4) ^ sw)];
+        if (RP == 8) *(float4 *)&a[RP - 4] = *(const float4 *)&sA[k * TP + ((TP / 2 + ty * 4) ^ sw)];
         *(float4 *)&b[0] = *(const float4 *)&sW[k * H + tx * 4];
         if (CPT == 8) *(float4 *)&b[CPT - 4] = *(const float4 *)&sW[k * H + H / 2 + tx * 4];
 #pragma unroll
-        for (int p = 0; p < 8; ++p)
+        for (int p = 0; p < RP; ++p)
 #pragma unroll
             for (int c = 0; c < CPT; ++c) acc[p][c] = fmaf(a[p], b[c], acc[p][c]);
     }
 }
 
-template <int H>
-__device__ __forceinline__ void zero_acc(float (&acc)[8][Tile<H>::CPT])
+template <int H, int RP = 8>
+__device__ __forceinline__ void zero_acc(float (&acc)[RP][Tile<H>::CPT])
 {
 #pragma unroll
-    for (int p = 0; p < 8; ++p)
+    for (int p = 0; p < RP; ++p)
 #pragma unroll
         for (int c = 0; c < Tile<H>::CPT; ++c) acc[p][c] = 0.f;
 }
 
 // writes v[p][c] (this thread's 8 x CPT sub-tile) into a swizzled k-major buffer as A[c][p]
-template <int H>
-__device__ __forceinline__ void store_as_A(float *sA, const float (&v)[8][Tile<H>::CPT], int tx, int ty)
+template <int H, int RP = 8>
+__device__ __forceinline__ void store_as_A(float *sA, const float (&v)[RP][Tile<H>::CPT], int tx, int ty)
 {
     constexpr int CPT = Tile<H>::CPT;
 #pragma unroll
@@ -65,7 +67,7 @@ __device__ __forceinline__ void store_as_A(float *sA, const float (&v)[8][Tile<H
         const int ch = Tile<H>::chan(tx, c >> 2, c & 3);
         const int sw = swz(ch);
         *(float4 *)&sA[ch * TP + ((ty * 4) ^ sw)] = make_float4(v[0][c], v[1][c], v[2][c], v[3][c]);
-        *(float4 *)&sA[ch * TP + ((TP / 2 + ty * 4) ^ sw)] = make_float4(v[4][c], v[5][c], v[6][c], v[7][c]);
+        if (RP == 8) *(float4 *)&sA[ch * TP + ((TP / 2 + ty * 4) ^ sw)] = make_float4(v[RP - 4][c], v[RP - 3][c], v[RP - 2][c], v[RP - 1][c]);
     }
 }
 

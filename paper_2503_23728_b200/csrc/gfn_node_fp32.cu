@@ -50,14 +50,16 @@ __device__ __forceinline__ float4 assemble_m(const NodeArgs &a, int64_t row, int
     return v;
 }
 
-template <int H>
+// RP = 8: 128-row tiles; RP = 4: 64-row tiles (rows 0..63 of the same buffers) when there are fewer 128-row tiles than SMs
+template <int H, int RP>
 __global__ void __launch_bounds__(NT, 1) node_kernel(NodeArgs a)
 { pdl_enter();
     extern __shared__ __align__(16) unsigned char smem_raw[];
     NodeSmem<H> &S = *reinterpret_cast<NodeSmem<H> *>(smem_raw);
     constexpr int CPT = Tile<H>::CPT;
     const int tid = threadIdx.x, tx = tid % TX, ty = tid / TX;
-    const int64_t row0 = (int64_t)blockIdx.x * TP;
+    constexpr int TPv = 16 * RP;                   // rows of this CTA's tile
+    const int64_t row0 = (int64_t)blockIdx.x * TPv;
     const int n_pairs = a.row_ptr[a.rows];
 
     // The weight matrices go through one shared-memory slab, each load in front of its product.  A layer's matrices are touched
@@ -72,7 +74,7 @@ __global__ void __launch_bounds__(NT, 1) node_kernel(NodeArgs a)
     }
 
     // ---- load the tile transposed into the k-major buffers
-    for (int idx = tid; idx < TP * H / 4; idx += NT) {
+    for (int idx = tid; idx < TPv * H / 4; idx += NT) {
         const int r = idx / (H / 4), c4 = idx % (H / 4), c0 = c4 * 4;
         const int64_t row = row0 + r;
         float4 nv = make_float4(0.f, 0.f, 0.f, 0.f), mv = nv;
@@ -94,45 +96,45 @@ __global__ void __launch_bounds__(NT, 1) node_kernel(NodeArgs a)
             S.B[(c0 + 2) * TP + col] = mv.z; S.B[(c0 + 3) * TP + col] = mv.w;
         }
     }
-    float acc[8][CPT];
+    float acc[RP][CPT];
 
     if (a.mode == 1) {
         for (int i = tid; i < H; i += NT) { S.bv1[i] = a.bv1[i]; S.bv2[i] = a.bv2[i]; S.ba[i] = a.ba[i]; }
         load_matrix<H>(S.W, a.WvnT, H);
         __syncthreads();
-        zero_acc<H>(acc);
-        tile_gemm<H, H>(S.A, S.W, acc, tx, ty);          // W_vn n
+        zero_acc<H, RP>(acc);
+        tile_gemm<H, H, RP>(S.A, S.W, acc, tx, ty);          // W_vn n
         __syncthreads();
         load_matrix<H>(S.W, a.WvmT, H);
         __syncthreads();
-        tile_gemm<H, H>(S.B, S.W, acc, tx, ty);          // + W_vm m
+        tile_gemm<H, H, RP>(S.B, S.W, acc, tx, ty);          // + W_vm m
         __syncthreads();
 #pragma unroll
         for (int c = 0; c < CPT; ++c) {
             const float b = S.bv1[Tile<H>::chan(tx, c >> 2, c & 3)];
 #pragma unroll
-            for (int p = 0; p < 8; ++p) acc[p][c] = silu_f(acc[p][c] + b);
+            for (int p = 0; p < RP; ++p) acc[p][c] = silu_f(acc[p][c] + b);
         }
-        store_as_A<H>(S.B, acc, tx, ty);                 // h
+        store_as_A<H, RP>(S.B, acc, tx, ty);                 // h
         load_matrix<H>(S.W, a.Wv2T, H);
         __syncthreads();
-        zero_acc<H>(acc);
-        tile_gemm<H, H>(S.B, S.W, acc, tx, ty);          // W_v2 h
+        zero_acc<H, RP>(acc);
+        tile_gemm<H, H, RP>(S.B, S.W, acc, tx, ty);          // W_v2 h
         // n <- n + W_v2 h + b_v2   (this thread's own elements of A; A is not read by the GEMM above)
 #pragma unroll
         for (int c = 0; c < CPT; ++c) {
             const int ch = Tile<H>::chan(tx, c >> 2, c & 3);
             const float b = S.bv2[ch];
 #pragma unroll
-            for (int p = 0; p < 8; ++p) {
+            for (int p = 0; p < RP; ++p) {
                 const int pr = Tile<H>::pair(ty, p >> 2, p & 3);
                 acc[p][c] += S.A[ch * TP + (pr ^ swz(ch))] + b;
             }
         }
         __syncthreads();
-        store_as_A<H>(S.A, acc, tx, ty);                 // updated n
+        store_as_A<H, RP>(S.A, acc, tx, ty);                 // updated n
 #pragma unroll
-        for (int p = 0; p < 8; ++p) {
+        for (int p = 0; p < RP; ++p) {
             const int64_t row = row0 + Tile<H>::pair(ty, p >> 2, p & 3);
             if (row < a.rows)
 #pragma unroll
@@ -142,10 +144,10 @@ __global__ void __launch_bounds__(NT, 1) node_kernel(NodeArgs a)
         }
         load_matrix<H>(S.W, a.WaT, H);
         __syncthreads();
-        zero_acc<H>(acc);
-        tile_gemm<H, H>(S.A, S.W, acc, tx, ty);          // a = W_a n + b_a ; E += a
+        zero_acc<H, RP>(acc);
+        tile_gemm<H, H, RP>(S.A, S.W, acc, tx, ty);          // a = W_a n + b_a ; E += a
 #pragma unroll
-        for (int p = 0; p < 8; ++p) {
+        for (int p = 0; p < RP; ++p) {
             const int64_t row = row0 + Tile<H>::pair(ty, p >> 2, p & 3);
 #pragma unroll
             for (int g = 0; g < CPT / 4; ++g) {
@@ -159,16 +161,16 @@ __global__ void __launch_bounds__(NT, 1) node_kernel(NodeArgs a)
                         make_float4(acc[p][g * 4], acc[p][g * 4 + 1], acc[p][g * 4 + 2], acc[p][g * 4 + 3]);
             }
         }
-        if (a.last) store_as_A<H>(S.B, acc, tx, ty);     // E as the operand of G = W_f1 E
+        if (a.last) store_as_A<H, RP>(S.B, acc, tx, ty);     // E as the operand of G = W_f1 E
         __syncthreads();
     }
     // ---- x = W_s n   (or G = W_f1 E)
     load_matrix<H>(S.W, a.WnextT, H);
     __syncthreads();
-    zero_acc<H>(acc);
-    tile_gemm<H, H>((a.mode == 1 && a.last) ? S.B : S.A, S.W, acc, tx, ty);
+    zero_acc<H, RP>(acc);
+    tile_gemm<H, H, RP>((a.mode == 1 && a.last) ? S.B : S.A, S.W, acc, tx, ty);
 #pragma unroll
-    for (int p = 0; p < 8; ++p) {
+    for (int p = 0; p < RP; ++p) {
         const int64_t row = row0 + Tile<H>::pair(ty, p >> 2, p & 3);
         if (row < a.rows)
 #pragma unroll
@@ -205,11 +207,14 @@ int launch_node_t(pimd_ctx *c, const NodeArgs &a)
 {
     size_t smem = sizeof(NodeSmem<H>);
     if (!(c->attr_done & ATTR_NODE32)) {
-        PIMD_CUDA_CHECK(cudaFuncSetAttribute(node_kernel<H>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        PIMD_CUDA_CHECK(cudaFuncSetAttribute(node_kernel<H, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        PIMD_CUDA_CHECK(cudaFuncSetAttribute(node_kernel<H, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         c->attr_done |= ATTR_NODE32;
     }
-    unsigned grid = (unsigned)((c->rows + TP - 1) / TP);
-    pimd_launch(node_kernel<H>, grid, NT, smem, c->stream, a);
+    if (c->rows < (int64_t)TP * c->num_sms)        // fewer 128-row tiles than SMs: half tiles, twice the CTAs
+        pimd_launch(node_kernel<H, 4>, (unsigned)((c->rows + TP / 2 - 1) / (TP / 2)), NT, smem, c->stream, a);
+    else
+        pimd_launch(node_kernel<H, 8>, (unsigned)((c->rows + TP - 1) / TP), NT, smem, c->stream, a);
     c->launches++;
     PIMD_CUDA_CHECK(cudaGetLastError());
     return 0;
