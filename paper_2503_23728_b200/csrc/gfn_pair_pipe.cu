@@ -93,13 +93,11 @@ struct Warps {
 
 struct PairArgs {
     alignas(64) CUtensorMap gmap;         // the gathered table (XE or G) as a 2-D tensor [rows][128 x 32 bit] for TMA tile::gather4
-    int N, periodic;
-    double box[3], inv_box[3];
+    int N;
     float r_cut, wscale;
     const int *row_ptr, *col, *pair_row;
     const float4 *dvec;                   // per pair: r_j - r_i (fp32 of the fp64 minimum-image difference) | segment kind (nlist_kernels.cu)
     int64_t rows;
-    const double *q;
     const uint16_t *Wf2img;               // head: bf16 UMMA image of w_f2 replicated on 16 rows ([16][128], 4 KB)
     const uint16_t *W1img, *W2img;        // bf16 UMMA images: 0.5 W_e1 [128][64]; W_e2 (message) or 0.5 W_f1 W_e2 (head), 2 x [128][64]
     float b1h[H];                         // b_e1 / 2 (kernel-parameter constant bank: immediate operands in role H)
@@ -985,10 +983,9 @@ __global__ void __launch_bounds__(Warps<HEAD, MODE>::THREADS, 1) pair_pipe_kerne
 int launch_pair_pipe(pimd_ctx *c, bool head, bool first)
 {
     PairArgs a;
-    a.N = c->N; a.periodic = c->periodic;
-    for (int k = 0; k < 3; ++k) { a.box[k] = c->box[k]; a.inv_box[k] = c->periodic ? 1.0 / c->box[k] : 0.0; }
+    a.N = c->N;
     a.r_cut = c->net.r_cut; a.wscale = head ? 1.0f : c->net.agg_norm;
-    a.row_ptr = c->nl.row_ptr; a.col = c->nl.col; a.pair_row = c->nl.pair_row; a.dvec = c->nl.dvec; a.rows = c->rows; a.q = c->q;
+    a.row_ptr = c->nl.row_ptr; a.col = c->nl.col; a.pair_row = c->nl.pair_row; a.dvec = c->nl.dvec; a.rows = c->rows;
     a.W1img = c->wimg_e1; a.W2img = head ? c->wimg_fe : c->wimg_e2; a.Wf2img = c->wimg_wf2;
     for (int k = 0; k < H; ++k) a.b1h[k] = c->h_be1_half[k];
     a.b2 = head ? c->net.bfe : c->net.be2;
