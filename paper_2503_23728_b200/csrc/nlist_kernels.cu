@@ -244,7 +244,7 @@ __global__ void __launch_bounds__(COUNT_THREADS) count_cell_kernel(NlArgs a)
 #pragma unroll
             for (int ax = 0; ax < 3; ++ax) {
                 double d = a.d.sorted_q[pos * 3 + ax] - ref[ax];          // once per candidate and cell: fp64 image shift, then fp32
-                if (a.periodic) d -= a.box[ax] * rint(d / a.box[ax]);
+                if (a.periodic) d -= a.box[ax] * rint(d * a.inv_box[ax]);   // (fp32 estimate only: the exact test is within_cutoff)
                 rel[ax] = (float)d;
             }
             sc[t] = make_float4(rel[0], rel[1], rel[2], __int_as_float(a.d.sorted_atom[pos]));   // one 128-bit load per test
@@ -263,7 +263,7 @@ __global__ void __launch_bounds__(COUNT_THREADS) count_cell_kernel(NlArgs a)
 #pragma unroll
             for (int ax = 0; ax < 3; ++ax) {
                 double d = ((act && in_s) ? hq[ax][ha] : a.d.sorted_q[posi * 3 + ax]) - ref[ax];
-                if (a.periodic) d -= a.box[ax] * rint(d / a.box[ax]);
+                if (a.periodic) d -= a.box[ax] * rint(d * a.inv_box[ax]);   // (fp32 estimate only: the exact test is within_cutoff)
                 qif[ax] = (float)d;
             }
 #pragma unroll 4
