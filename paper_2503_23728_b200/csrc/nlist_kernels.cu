@@ -266,34 +266,52 @@ __global__ void __launch_bounds__(COUNT_THREADS) count_cell_kernel(NlArgs a)
                 if (a.periodic) d -= a.box[ax] * rint(d * a.inv_box[ax]);   // (fp32 estimate only: the exact test is within_cutoff)
                 qif[ax] = (float)d;
             }
-#pragma unroll 4
-            for (int s0 = warp; s0 < n; s0 += COUNT_THREADS / 32) {
-                const float4 cj = sc[s0];
-                const float cq[3] = {cj.x, cj.y, cj.z};
-                const int j = __float_as_int(cj.w);
-                // fp32 estimate of d^2 from the relative coordinates: its error is orders of magnitude below the 1e-3 band;
-                // inside the band the exact S:L3 sequence decides
-                float d2 = 0.f;
+            // 32 of this warp's candidates at a time (s = sb + 4 k).  The tests only set a bit per candidate -- clear hit, or inside
+            // the band; nearly every candidate is a hit for SOME lane of the warp, so a branch per candidate would send the whole warp
+            // through the append path every time.  The set bits (13 % of a lane's candidates) are handled after the block.
+            constexpr int NWARP = COUNT_THREADS / 32;
+            for (int sb = warp; sb < n; sb += 32 * NWARP) {
+                unsigned hitm = 0u, bandm = 0u;
 #pragma unroll
-                for (int ax = 0; ax < 3; ++ax) {
-                    float dx = cq[ax] - qif[ax];
-                    if (WRAP) {
-                        float sh = (dx > hbx[ax]) ? bxf[ax] : 0.f;      // selects, not branches (hbx = +inf when not periodic)
-                        sh = (dx < -hbx[ax]) ? -bxf[ax] : sh;
-                        dx -= sh;
+                for (int k = 0; k < 32; ++k) {
+                    const int s0 = sb + k * NWARP;
+                    const float4 cj = sc[s0 < n ? s0 : n - 1];
+                    float d2 = 0.f;
+#pragma unroll
+                    for (int ax = 0; ax < 3; ++ax) {
+                        float dx = (ax == 0 ? cj.x : (ax == 1 ? cj.y : cj.z)) - qif[ax];
+                        if (WRAP) {
+                            float sh = (dx > hbx[ax]) ? bxf[ax] : 0.f;      // selects, not branches (hbx = +inf when not periodic)
+                            sh = (dx < -hbx[ax]) ? -bxf[ax] : sh;
+                            dx -= sh;
+                        }
+                        d2 = fmaf(dx, dx, d2);
                     }
-                    d2 = fmaf(dx, dx, d2);
+                    const bool cand = (s0 < n) && (__float_as_int(cj.w) != i);
+                    d2 = cand ? d2 : inf;        // not a candidate: neither a hit nor in the band
+                    // (predicated ORs: written as selects, the two masks cost more than the branch they replace)
+                    asm("{\n\t.reg .pred ph, pb;\n\t"
+                        "setp.lt.f32 ph, %2, %3;\n\t"
+                        "setp.le.and.f32 pb, %2, %4, !ph;\n\t"
+                        "@ph or.b32 %0, %0, %5;\n\t"
+                        "@pb or.b32 %1, %1, %5;\n\t}"
+                        : "+r"(hitm), "+r"(bandm) : "f"(d2), "f"(rc2_lo), "f"(rc2_hi), "r"(1u << k));
                 }
-                if (act && j != i && d2 <= rc2_hi) {
-                    bool hit = d2 < rc2_lo;
-                    if (!hit) {                  // in the band (about 0.2 % of the candidates): fp64 positions
-                        const double qi[3] = {in_s ? hq[0][ha] : a.d.sorted_q[posi * 3], in_s ? hq[1][ha] : a.d.sorted_q[posi * 3 + 1],
-                                              in_s ? hq[2][ha] : a.d.sorted_q[posi * 3 + 2]};
-                        hit = within_cutoff(qi, a.d.sorted_q + (sbase + sp[s0]) * 3, a, a.rl2);
-                    }
-                    if (hit) {
-                        const int idx = in_s ? atomicAdd(&scnt[ha], 1) : atomicAdd(&a.d.nnz[row], 1);
-                        if (idx < a.hit_stride) buf[idx] = j;
+                if (!act) { hitm = 0u; bandm = 0u; }
+                while (bandm) {                  // in the band (about 0.2 % of the candidates): fp64 positions, exact S:L3 sequence
+                    const int k = __ffs(bandm) - 1;
+                    bandm &= bandm - 1;
+                    const double qi[3] = {in_s ? hq[0][ha] : a.d.sorted_q[posi * 3], in_s ? hq[1][ha] : a.d.sorted_q[posi * 3 + 1],
+                                          in_s ? hq[2][ha] : a.d.sorted_q[posi * 3 + 2]};
+                    if (within_cutoff(qi, a.d.sorted_q + (sbase + sp[sb + k * NWARP]) * 3, a, a.rl2)) hitm |= 1u << k;
+                }
+                if (hitm) {
+                    int idx = in_s ? atomicAdd(&scnt[ha], __popc(hitm)) : atomicAdd(&a.d.nnz[row], __popc(hitm));
+                    while (hitm) {
+                        const int k = __ffs(hitm) - 1;
+                        hitm &= hitm - 1;
+                        if (idx < a.hit_stride) buf[idx] = __float_as_int(sc[sb + k * NWARP].w);
+                        ++idx;
                     }
                 }
             }
