@@ -87,15 +87,28 @@ __device__ __forceinline__ void xform(const double *__restrict__ M, const double
     }
 }
 
-__device__ __forceinline__ void pile_O(const NmArgs &a, double *pt, int r, int col, uint32_t t, uint32_t tag)
+// per-mode coefficients, formed once per CTA (they do not depend on the atom): exp(-gamma_k dt/2), sqrt(1 - that^2) for the O
+// step; cos(w_k dt), sin(w_k dt) for the A step.  Same functions, same arguments as a per-thread evaluation: the same bits.
+struct ModeTab { double c1[PIMD_MAX_P], c2[PIMD_MAX_P], cs[PIMD_MAX_P], sn[PIMD_MAX_P]; };
+
+__device__ __forceinline__ void fill_mode_tab(const NmArgs &a, ModeTab &T, bool with_rotation)
+{
+    const double hdt = 0.5 * a.dt;
+    for (int k = threadIdx.y * blockDim.x + threadIdx.x; k < a.P; k += blockDim.x * blockDim.y) {
+        const double c1 = exp(-a.gam_k[k] * hdt);
+        T.c1[k] = c1; T.c2[k] = sqrt(1.0 - c1 * c1);
+        if (with_rotation) { double sn, cs; sincos(a.omega_k[k] * a.dt, &sn, &cs); T.cs[k] = cs; T.sn[k] = sn; }
+    }
+}
+
+__device__ __forceinline__ void pile_O(const NmArgs &a, const ModeTab &T, double *pt, int r, int col, uint32_t t, uint32_t tag)
 {
     const int c = threadIdx.x;
     const int atom = col / 3, dim = col - 3 * atom;
-    const double hdt = 0.5 * a.dt;
     for (int k = threadIdx.y; k < a.P; k += NM_TY) {
         if (k == 0 && a.thermostat == 1) { pt[c] = a.alpha[r] * pt[c]; continue; }   // PILE-G: one factor for the replica's free modes
         const double sig = sqrt(a.mass[atom] * a.lam[k] * a.kT_P);
-        double c1 = exp(-a.gam_k[k] * hdt), c2 = sqrt(1.0 - c1 * c1);
+        const double c1 = T.c1[k], c2 = T.c2[k];
         double xi = normal_component(a.seed, (uint32_t)atom, (uint32_t)(r * a.P + k), t, tag, dim);
         pt[k * a.TC + c] = c1 * pt[k * a.TC + c] + sig * c2 * xi;
     }
@@ -145,6 +158,8 @@ __global__ void __launch_bounds__(32 * NM_TY) nm_kernel(NmArgs a, const uint32_t
         return;
     }
 
+    __shared__ ModeTab tab;
+    fill_mode_tab(a, tab, MODE == 0);              // (read after at least one __syncthreads below)
     bool bad = false;
     const bool prim = a.transform == 2;
     const double mi = a.mass[colc / 3];
@@ -166,7 +181,7 @@ __global__ void __launch_bounds__(32 * NM_TY) nm_kernel(NmArgs a, const uint32_t
     if (thermo) {
         xform(a.Tp_fwd, bP, bT, P, TC);
         __syncthreads();
-        pile_O(a, bT, r, colc, t, MODE == 0 ? 0u : 1u);
+        pile_O(a, tab, bT, r, colc, t, MODE == 0 ? 0u : 1u);
         __syncthreads();
         xform(a.Tp_inv, bT, bP, P, TC);
         __syncthreads();
@@ -194,8 +209,7 @@ __global__ void __launch_bounds__(32 * NM_TY) nm_kernel(NmArgs a, const uint32_t
             if (w == 0.0) {
                 qt = qt + a.dt * pt / mu;
             } else {
-                double sn, cs;
-                sincos(w * a.dt, &sn, &cs);
+                const double sn = tab.sn[k], cs = tab.cs[k];
                 double pn = cs * pt - mu * w * sn * qt;
                 double qn = sn / (mu * w) * pt + cs * qt;
                 pt = pn; qt = qn;
