@@ -25,8 +25,12 @@ struct Tile {
     __device__ static __forceinline__ int pair(int ty, int g, int e) { return g * (TP / 2) + ty * 4 + e; }
 };
 
+// local row of element p of a thread's RP rows (RP = 8: two groups of four, 64 rows apart; 4: one group of four; 2: two rows)
+template <int RP>
+__device__ __forceinline__ int tile_row(int ty, int p) { return RP == 2 ? ty * 2 + p : (p >> 2) * (TP / 2) + ty * 4 + (p & 3); }
+
 // acc[p][c] += sum_k A[k][p] * W[k][c];  A swizzled [KD][TP], W [KD][H]
-// RP = rows per thread: 8 (the whole 128-row tile) or 4 (only rows 0..63 of the buffers are in use: half tiles, for
+// RP = rows per thread: 8 (the whole 128-row tile), 4 or 2 (only rows 0..63 / 0..31 of the buffers are in use: partial tiles for
 // configurations with fewer tiles than SMs)
 template <int KD, int H, int RP = 8>
 __device__ __forceinline__ void tile_gemm(const float *__restrict__ sA, const float *__restrict__ sW,
@@ -37,8 +41,12 @@ __device__ __forceinline__ void tile_gemm(const float *__restrict__ sA, const fl
     for (int k = 0; k < KD; ++k) {
         const int sw = swz(k);
         float a[RP], b[CPT];
-        *(float4 *)&a[0] = *(const float4 *)&sA[k * TP + ((ty * 4) ^ sw)];
-        if (RP == 8) *(float4 *)&a[RP - 4] = *(const float4 *)&sA[k * TP + ((TP / 2 + ty * 4) ^ sw)];
+        if constexpr (RP == 2) {
+            *(float2 *)&a[0] = *(const float2 *)&sA[k * TP + ((ty * 2) ^ sw)];
+        } else {
+            *(float4 *)&a[0] = *(const float4 *)&sA[k * TP + ((ty * 4) ^ sw)];
+            if constexpr (RP == 8) *(float4 *)&a[RP - 4] = *(const float4 *)&sA[k * TP + ((TP / 2 + ty * 4) ^ sw)];
+        }
         *(float4 *)&b[0] = *(const float4 *)&sW[k * H + tx * 4];
         if (CPT == 8) *(float4 *)&b[CPT - 4] = *(const float4 *)&sW[k * H + H / 2 + tx * 4];
 #pragma unroll
@@ -66,8 +74,12 @@ __device__ __forceinline__ void store_as_A(float *sA, const float (&v)[RP][Tile<
     for (int c = 0; c < CPT; ++c) {
         const int ch = Tile<H>::chan(tx, c >> 2, c & 3);
         const int sw = swz(ch);
-        *(float4 *)&sA[ch * TP + ((ty * 4) ^ sw)] = make_float4(v[0][c], v[1][c], v[2][c], v[3][c]);
-        if (RP == 8) *(float4 *)&sA[ch * TP + ((TP / 2 + ty * 4) ^ sw)] = make_float4(v[RP - 4][c], v[RP - 3][c], v[RP - 2][c], v[RP - 1][c]);
+        if constexpr (RP == 2) {
+            *(float2 *)&sA[ch * TP + ((ty * 2) ^ sw)] = make_float2(v[0][c], v[1][c]);
+        } else {
+            *(float4 *)&sA[ch * TP + ((ty * 4) ^ sw)] = make_float4(v[0][c], v[1][c], v[2][c], v[3][c]);
+            if constexpr (RP == 8) *(float4 *)&sA[ch * TP + ((TP / 2 + ty * 4) ^ sw)] = make_float4(v[RP - 4][c], v[RP - 3][c], v[RP - 2][c], v[RP - 1][c]);
+        }
     }
 }
 

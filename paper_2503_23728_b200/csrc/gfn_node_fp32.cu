@@ -50,7 +50,7 @@ __device__ __forceinline__ float4 assemble_m(const NodeArgs &a, int64_t row, int
     return v;
 }
 
-// RP = 8: 128-row tiles; RP = 4: 64-row tiles (rows 0..63 of the same buffers) when there are fewer 128-row tiles than SMs
+// RP = 8: 128-row tiles; RP = 4 / 2: 64- / 32-row tiles (the first rows of the same buffers) when there are fewer tiles than SMs
 template <int H, int RP>
 __global__ void __launch_bounds__(NT, 1) node_kernel(NodeArgs a)
 { pdl_enter();
@@ -127,7 +127,7 @@ __global__ void __launch_bounds__(NT, 1) node_kernel(NodeArgs a)
             const float b = S.bv2[ch];
 #pragma unroll
             for (int p = 0; p < RP; ++p) {
-                const int pr = Tile<H>::pair(ty, p >> 2, p & 3);
+                const int pr = tile_row<RP>(ty, p);
                 acc[p][c] += S.A[ch * TP + (pr ^ swz(ch))] + b;
             }
         }
@@ -135,7 +135,7 @@ __global__ void __launch_bounds__(NT, 1) node_kernel(NodeArgs a)
         store_as_A<H, RP>(S.A, acc, tx, ty);                 // updated n
 #pragma unroll
         for (int p = 0; p < RP; ++p) {
-            const int64_t row = row0 + Tile<H>::pair(ty, p >> 2, p & 3);
+            const int64_t row = row0 + tile_row<RP>(ty, p);
             if (row < a.rows)
 #pragma unroll
                 for (int g = 0; g < CPT / 4; ++g)
@@ -148,7 +148,7 @@ __global__ void __launch_bounds__(NT, 1) node_kernel(NodeArgs a)
         tile_gemm<H, H, RP>(S.A, S.W, acc, tx, ty);          // a = W_a n + b_a ; E += a
 #pragma unroll
         for (int p = 0; p < RP; ++p) {
-            const int64_t row = row0 + Tile<H>::pair(ty, p >> 2, p & 3);
+            const int64_t row = row0 + tile_row<RP>(ty, p);
 #pragma unroll
             for (int g = 0; g < CPT / 4; ++g) {
                 const int c0 = Tile<H>::chan(tx, g, 0);
@@ -171,7 +171,7 @@ __global__ void __launch_bounds__(NT, 1) node_kernel(NodeArgs a)
     tile_gemm<H, H, RP>((a.mode == 1 && a.last) ? S.B : S.A, S.W, acc, tx, ty);
 #pragma unroll
     for (int p = 0; p < RP; ++p) {
-        const int64_t row = row0 + Tile<H>::pair(ty, p >> 2, p & 3);
+        const int64_t row = row0 + tile_row<RP>(ty, p);
         if (row < a.rows)
 #pragma unroll
             for (int g = 0; g < CPT / 4; ++g)
@@ -209,9 +209,12 @@ int launch_node_t(pimd_ctx *c, const NodeArgs &a)
     if (!(c->attr_done & ATTR_NODE32)) {
         PIMD_CUDA_CHECK(cudaFuncSetAttribute(node_kernel<H, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         PIMD_CUDA_CHECK(cudaFuncSetAttribute(node_kernel<H, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        PIMD_CUDA_CHECK(cudaFuncSetAttribute(node_kernel<H, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         c->attr_done |= ATTR_NODE32;
     }
-    if (c->rows < (int64_t)TP * c->num_sms)        // fewer 128-row tiles than SMs: half tiles, twice the CTAs
+    if (c->rows <= (int64_t)(TP / 4) * c->num_sms) // quarter tiles still fit one per SM
+        pimd_launch(node_kernel<H, 2>, (unsigned)((c->rows + TP / 4 - 1) / (TP / 4)), NT, smem, c->stream, a);
+    else if (c->rows < (int64_t)TP * c->num_sms)   // fewer 128-row tiles than SMs: half tiles, twice the CTAs
         pimd_launch(node_kernel<H, 4>, (unsigned)((c->rows + TP / 2 - 1) / (TP / 2)), NT, smem, c->stream, a);
     else
         pimd_launch(node_kernel<H, 8>, (unsigned)((c->rows + TP - 1) / TP), NT, smem, c->stream, a);
