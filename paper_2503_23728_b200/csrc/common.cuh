@@ -108,7 +108,7 @@ struct pimd_ctx {
     double *omega_k, *lam_k, *gam_k;   // [P] mode frequency, mass factor, friction
     double *pileg_partial, *pileg_alpha;   // [R][64][2], [R]
     int *err;                          // [4] device error word
-    uint32_t *step_dev;                // device copy of the step counter (read by the noise kernels: a captured step does not depend on it)
+    uint32_t *step_dev;                // two device words of the step counter (read by the noise kernels: a captured step does not depend on it)
     cudaGraphExec_t step_graph;        // one whole step, captured at the first pimd_step (null: not captured yet)
     int graph_state;                   // 0 not tried, 1 captured, -1 capture not available
     int warm;                          // a step has run with plain launches (every lazy kernel attribute is set)
@@ -186,10 +186,9 @@ static inline cudaError_t pimd_launch(void (*kernel)(KArgs...), dim3 grid, dim3 
 
 // kernel launchers (each returns 0 or PIMD_ERR_CUDA)
 int pimd_launch_init_momenta(pimd_ctx *c);
-int pimd_launch_nm_pre(pimd_ctx *c);                 // O B A with the noise of step *step_dev
-int pimd_launch_step_inc(pimd_ctx *c);               // *step_dev += 1
-int pimd_launch_set_step(pimd_ctx *c, uint32_t t);   // *step_dev = t
-int pimd_launch_nm_post(pimd_ctx *c);                // B O with the noise of step *step_dev - 1
+int pimd_launch_nm_pre(pimd_ctx *c);                 // O B A with the noise of step step_dev[0]; leaves step_dev[1] = that + 1
+int pimd_launch_set_step(pimd_ctx *c, uint32_t t);   // step_dev[0] = step_dev[1] = t
+int pimd_launch_nm_post(pimd_ctx *c);                // B O with the noise of step step_dev[1] - 1; leaves step_dev[0] = step_dev[1]
 int pimd_launch_simple_forces(pimd_ctx *c);          // kinds 1, 2
 int pimd_launch_estimators(pimd_ctx *c);
 int pimd_launch_nlist(pimd_ctx *c);

@@ -127,13 +127,16 @@ __device__ __forceinline__ double spring_force(const NmArgs &a, const double *bQ
 // of one step does not depend on the step and can be captured once as a CUDA graph and replayed.
 __device__ __forceinline__ uint32_t step_of(const uint32_t *t_dev, uint32_t t_off) { return t_dev ? *t_dev - t_off : 0u; }
 
-__global__ void step_inc_kernel(uint32_t *t_dev) { pdl_enter(); *t_dev += 1u; }
-__global__ void step_set_kernel(uint32_t *t_dev, uint32_t t) { pdl_enter(); *t_dev = t; }
+__global__ void step_set_kernel(uint32_t *t_dev, uint32_t t) { pdl_enter(); t_dev[0] = t; t_dev[1] = t; }
 
 template <int MODE>
-__global__ void __launch_bounds__(32 * NM_TY) nm_kernel(NmArgs a, const uint32_t *t_dev, uint32_t t_off)
+__global__ void __launch_bounds__(32 * NM_TY) nm_kernel(NmArgs a, const uint32_t *t_dev, uint32_t t_off, uint32_t *t_next)
 { pdl_enter();
     const uint32_t t = step_of(t_dev, t_off);
+    // The step counter lives in two device words that the two halves of a step hand to each other: the first half reads word 0 and
+    // leaves t + 1 in word 1, the second half reads word 1 (minus one) and leaves t + 1 in word 0.  Nothing reads the word a kernel
+    // writes while that kernel runs, and no separate increment kernel is needed.
+    if (t_next && blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0 && threadIdx.y == 0) *t_next = t + 1u;
     extern __shared__ double sm[];
     const int P = a.P, TC = a.TC;
     double *bP = sm, *bT = sm + (size_t)P * TC, *bQ = bT + (size_t)P * TC, *bQ2 = bQ + (size_t)P * TC;
@@ -302,7 +305,7 @@ NmArgs make_args(const pimd_ctx *c)
 }
 
 template <int MODE>
-int launch_nm(pimd_ctx *c, const uint32_t *t_dev, uint32_t t_off)
+int launch_nm(pimd_ctx *c, const uint32_t *t_dev, uint32_t t_off, uint32_t *t_next)
 {
     NmArgs a = make_args(c);
     if (MODE != 2 && c->thermostat == 1 && c->gamma_fs >= 0.0) {   // PILE-G: the replica's scale factor for this half-step
@@ -319,7 +322,7 @@ int launch_nm(pimd_ctx *c, const uint32_t *t_dev, uint32_t t_off)
         c->attr_done |= ATTR_NM;
     }
     dim3 grid((3 * c->N + a.TC - 1) / a.TC, c->R), block(a.TC, NM_TY);
-    pimd_launch(nm_kernel<MODE>, grid, block, smem, c->stream, a, t_dev, t_off);
+    pimd_launch(nm_kernel<MODE>, grid, block, smem, c->stream, a, t_dev, t_off, t_next);
     c->launches++;
     PIMD_CUDA_CHECK(cudaGetLastError());
     return 0;
@@ -402,18 +405,10 @@ __global__ void estimators_final_kernel(int R, int N, int P, int kind, double kT
 
 }  // namespace
 
-int pimd_launch_init_momenta(pimd_ctx *c) { return launch_nm<2>(c, nullptr, 0u); }
-// the device step counter holds t before pimd_launch_step_inc and t + 1 after it
-int pimd_launch_nm_pre(pimd_ctx *c) { return launch_nm<0>(c, c->step_dev, 0u); }
-int pimd_launch_nm_post(pimd_ctx *c) { return launch_nm<1>(c, c->step_dev, 1u); }
-int pimd_launch_step_inc(pimd_ctx *c)
-{
-    pimd_launch(step_inc_kernel, 1, 1, 0, c->stream, c->step_dev);
-    c->launches++;
-    PIMD_CUDA_CHECK(cudaGetLastError());
-    return 0;
-}
-
+int pimd_launch_init_momenta(pimd_ctx *c) { return launch_nm<2>(c, nullptr, 0u, nullptr); }
+// device step counter: word 0 holds t at the start of a step, word 1 holds t + 1 between the two halves (see nm_kernel)
+int pimd_launch_nm_pre(pimd_ctx *c) { return launch_nm<0>(c, c->step_dev, 0u, c->step_dev + 1); }
+int pimd_launch_nm_post(pimd_ctx *c) { return launch_nm<1>(c, c->step_dev + 1, 1u, c->step_dev); }
 int pimd_launch_set_step(pimd_ctx *c, uint32_t t)
 {
     pimd_launch(step_set_kernel, 1, 1, 0, c->stream, c->step_dev, t);

@@ -754,7 +754,6 @@ int step_body(pimd_ctx *c)
     {
         ProfScope ps(c, PROF_NM);
         if ((rc = pimd_launch_nm_pre(c))) return rc;
-        if ((rc = pimd_launch_step_inc(c))) return rc;
     }
     if ((rc = compute_forces(c))) return rc;
     ProfScope ps(c, PROF_NM);
